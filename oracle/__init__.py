@@ -1,0 +1,170 @@
+"""ORACLE -- TEST INFRASTRUCTURE ONLY (see oracle/oracle.cpp header).
+
+ctypes wrapper around the plain fp64 CPU implementation in oracle/oracle.cpp.  Imported only by
+tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` leg.  Nothing in
+paper_2403_16862_b200 (the product) imports this package, and this package imports nothing from
+the product except nothing at all: inputs arrive as numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+T_MIN = 1e-4   # transmittance cut-off (BASELINE.json north_star; not in the paper)
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off (the canonical fp32 projection must not be contracted to FMA)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c++17",
+                               "-shared", "-fPIC", "-o", _LIB, _SRC])
+    return _LIB
+
+
+class _Camera(C.Structure):
+    _fields_ = [("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float), ("cy", C.c_float),
+                ("R", C.c_float * 9), ("t", C.c_float * 3),
+                ("near_z", C.c_float), ("far_z", C.c_float),
+                ("width", C.c_int32), ("height", C.c_int32)]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build())
+        lib.oracle_create.restype = C.c_void_p
+        lib.oracle_create.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]
+        lib.oracle_create_uv.restype = C.c_void_p
+        lib.oracle_create_uv.argtypes = [C.c_void_p] * 5 + [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
+        lib.oracle_free.argtypes = [C.c_void_p]
+        for name in ("oracle_total", "oracle_kept", "oracle_border_dropped"):
+            getattr(lib, name).restype = C.c_int64
+            getattr(lib, name).argtypes = [C.c_void_p]
+        lib.oracle_counts.argtypes = [C.c_void_p, C.c_void_p]
+        lib.oracle_sorted.argtypes = [C.c_void_p] * 5
+        lib.oracle_blend.argtypes = [C.c_void_p, C.c_double] + [C.c_void_p] * 4
+        lib.oracle_backward.restype = C.c_int
+        lib.oracle_backward.argtypes = [C.c_void_p] * 6
+        lib.oracle_count_fp64_projection_changes.restype = C.c_int64
+        lib.oracle_count_fp64_projection_changes.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def _cam_struct(cam) -> _Camera:
+    c = _Camera()
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    R = np.asarray(cam.R, dtype=np.float32).reshape(9)
+    t = np.asarray(cam.t, dtype=np.float32).reshape(3)
+    for i in range(9):
+        c.R[i] = float(R[i])
+    for i in range(3):
+        c.t[i] = float(t[i])
+    c.near_z, c.far_z = float(cam.near_z), float(cam.far_z)
+    c.width, c.height = int(cam.width), int(cam.height)
+    return c
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class Raster:
+    """One rasterisation problem held by the oracle: buckets built and sorted at construction."""
+
+    def __init__(self, handle, N, D, W, H):
+        self._h, self.N, self.D, self.W, self.H = handle, N, D, W, H
+        self.P = W * H
+
+    @classmethod
+    def from_points(cls, pos, opacity, feat, cam) -> "Raster":
+        lib = _load()
+        pos = np.ascontiguousarray(pos, dtype=np.float32).reshape(-1, 3)
+        opacity = np.ascontiguousarray(opacity, dtype=np.float32).reshape(-1)
+        feat = np.ascontiguousarray(feat, dtype=np.float32)
+        N, D = pos.shape[0], (feat.shape[1] if feat.ndim == 2 else 0)
+        assert opacity.shape[0] == N and feat.shape[0] == N
+        cs = _cam_struct(cam)
+        h = lib.oracle_create(_p(pos), _p(opacity), _p(feat), N, D, C.byref(cs))
+        return cls(h, N, D, int(cam.width), int(cam.height))
+
+    @classmethod
+    def from_uv(cls, u, v, depth, opacity, feat, W, H) -> "Raster":
+        lib = _load()
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        depth = np.ascontiguousarray(depth, dtype=np.float32)
+        opacity = np.ascontiguousarray(opacity, dtype=np.float32)
+        feat = np.ascontiguousarray(feat, dtype=np.float32)
+        N, D = u.shape[0], feat.shape[1]
+        h = lib.oracle_create_uv(_p(u), _p(v), _p(depth), _p(opacity), _p(feat), N, D, int(W), int(H))
+        return cls(h, N, D, int(W), int(H))
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.oracle_free(self._h)
+            self._h = None
+
+    @property
+    def total(self) -> int:
+        return int(_lib.oracle_total(self._h))
+
+    @property
+    def kept(self) -> int:
+        return int(_lib.oracle_kept(self._h))
+
+    @property
+    def border_dropped(self) -> int:
+        return int(_lib.oracle_border_dropped(self._h))
+
+    def counts(self) -> np.ndarray:
+        c = np.empty(self.P, dtype=np.uint32)
+        _lib.oracle_counts(self._h, _p(c))
+        return c.reshape(self.H, self.W)
+
+    def sorted_fragments(self):
+        """offsets[P+1], point_idx[total], depth_bits[total], weight[total] in pixel-major sorted order."""
+        tot = self.total
+        off = np.empty(self.P + 1, dtype=np.int64)
+        idx = np.empty(tot, dtype=np.int64)
+        dep = np.empty(tot, dtype=np.uint32)
+        w = np.empty(tot, dtype=np.float64)
+        _lib.oracle_sorted(self._h, _p(off), _p(idx), _p(dep), _p(w))
+        return off, idx, dep, w
+
+    def blend(self, t_min: float = T_MIN):
+        """-> img[H,W,D] f64, alpha[H,W] f64, nb[H,W] u32, margin[H,W] f64."""
+        img = np.empty((self.H, self.W, self.D), dtype=np.float64)
+        alpha = np.empty((self.H, self.W), dtype=np.float64)
+        nb = np.empty((self.H, self.W), dtype=np.uint32)
+        margin = np.empty((self.H, self.W), dtype=np.float64)
+        _lib.oracle_blend(self._h, float(t_min), _p(img), _p(alpha), _p(nb), _p(margin))
+        return img, alpha, nb, margin
+
+    def backward(self, g_img, g_alpha=None):
+        """Gradients of <g_img, img> + <g_alpha, alpha>; call blend() first (same t_min).
+        -> d_feat[N,D], d_opacity[N], d_uv[N,2], all f64."""
+        g_img = np.ascontiguousarray(g_img, dtype=np.float64).reshape(self.H, self.W, self.D)
+        ga = None if g_alpha is None else np.ascontiguousarray(g_alpha, dtype=np.float64).reshape(self.H, self.W)
+        d_feat = np.empty((self.N, self.D), dtype=np.float64)
+        d_op = np.empty(self.N, dtype=np.float64)
+        d_uv = np.empty((self.N, 2), dtype=np.float64)
+        rc = _lib.oracle_backward(self._h, _p(g_img), None if ga is None else _p(ga),
+                                  _p(d_feat), _p(d_op), _p(d_uv))
+        if rc != 0:
+            raise RuntimeError("oracle_backward: blend() has not been called")
+        return d_feat, d_op, d_uv
+
+
+def fp64_projection_changes(pos, cam) -> int:
+    lib = _load()
+    pos = np.ascontiguousarray(pos, dtype=np.float32).reshape(-1, 3)
+    cs = _cam_struct(cam)
+    return int(lib.oracle_count_fp64_projection_changes(_p(pos), pos.shape[0], C.byref(cs)))
