@@ -1,0 +1,115 @@
+/* inpc_raster.h -- C ABI of the B200-native differentiable bilinear point rasterizer.
+ *
+ * What it computes (INPC, arXiv 2403.16862; citations are lines of the paper text PAPER.md):
+ *   RASTERIZE(C, P, A, F) -> I of Algorithm 1 (App. A.6): every point is projected
+ *   with a pinhole camera (Eq. 6), splatted to the 2x2 nearest pixel centres with
+ *   opacity alpha = alpha_h (1-|u-u_i|)(1-|v-v_i|) (Eq. 7), each pixel's fragments are
+ *   ordered by depth ("blend all points in depth order"; ties by point index) and
+ *   composited front to back, C = sum_i T_i alpha_i c_i, T_i = prod_{j<i}(1-alpha_j) (Eq. 1,
+ *   PAPER.md:34), stopping once T < 1e-4 (BASELINE.json north_star; the paper has no cut-off).
+ *   The backward pass returns gradients w.r.t. features, opacities and the projected
+ *   screen position (u, v) of every point.  DESIGN.md section 3 lists every reading of the paper.
+ *
+ * Conventions
+ *   - Pixel (i, j) has its centre at (i+0.5, j+0.5); +z forward, +y down; p_c = R p_w + t.
+ *   - A point is kept iff near_z < z_c < far_z and u, v are finite; each of its four fragments is kept
+ *     iff its pixel is inside [0,W)x[0,H).  Zero-weight / zero-opacity fragments are kept and counted.
+ *   - The discrete quantities (cull, pixel, depth key) come from a fixed sequence of individually
+ *     rounded fp32 operations (no FMA): x_c = ((R0 x + R1 y) + R2 z) + t0, ..., u = (fx x_c)/z_c + cx.
+ *   - All arithmetic is fp32.  Images are [H][W][D] (pixel-interleaved), alpha is [H][W].
+ *
+ * Memory, ownership, streams
+ *   - Every pointer is DEVICE memory owned by the caller unless marked "host".  The library allocates
+ *     no device memory and keeps no state between calls: scratch and the state saved for the backward
+ *     pass live in the caller's `workspace`.  Device pointers must be 16-byte aligned.
+ *   - Outputs and gradient buffers are OVERWRITTEN (not accumulated into).
+ *   - All work is enqueued on `cuda_stream` (a cudaStream_t; NULL = the default stream).  Calls return
+ *     without synchronising, except inpc_raster_get_stats and inpc_raster_get_sorted (they read back).
+ *
+ * Errors: every entry point returns INPC_OK (0) or a negative inpc_status; nothing aborts, throws or
+ * prints.  There is no CPU fallback: without a CUDA device every compute call returns INPC_ERR_CUDA.
+ */
+#ifndef INPC_RASTER_H
+#define INPC_RASTER_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct inpc_camera {
+    float   fx, fy, cx, cy;  /* intrinsics, in pixels                                            */
+    float   R[9], t[3];      /* world -> camera, row-major: p_c = R p_w + t                      */
+    float   near_z, far_z;   /* kept iff near_z < z_c < far_z (paper: 0.01 / 100)  */
+    int32_t width, height;
+} inpc_camera;
+
+typedef enum inpc_status {
+    INPC_OK                      =  0,
+    INPC_ERR_INVALID_ARG         = -1,  /* NULL / misaligned pointer, N < 0, W/H <= 0, near >= far, N >= 2^30 */
+    INPC_ERR_WORKSPACE_TOO_SMALL = -2,
+    INPC_ERR_CUDA                = -3,  /* launch failure or sticky error; see inpc_raster_last_cuda_error   */
+    INPC_ERR_NO_SAVED_STATE      = -4,  /* backward / get_* on a workspace no matching forward has filled     */
+    INPC_ERR_UNSUPPORTED         = -5   /* D not in {4, 8}, W or H > 4095                                     */
+} inpc_status;
+
+/* flags of inpc_raster_forward / inpc_raster_workspace_bytes */
+#define INPC_SAVE_FOR_BACKWARD 1u  /* keep what inpc_raster_backward needs in the workspace                 */
+#define INPC_SAVE_SORTED       2u  /* also materialise every pixel's sorted fragment list (for get_sorted)  */
+
+typedef struct inpc_stats {          /* host struct filled by inpc_raster_get_stats                          */
+    uint64_t n_points;               /* N of the last forward                                                 */
+    uint64_t n_kept;                 /* points that survived the cull (= records binned)                      */
+    uint64_t n_fragments;            /* emitted fragments = sum over pixels of count[p]                       */
+    uint64_t n_tile_items;           /* screen-tile work items built for the blend kernel                     */
+    uint64_t n_big_pixels;           /* pixels deeper than the in-tile limit, handled by the long-run path    */
+    uint64_t n_big_fragments;        /* fragments in those pixels                                             */
+} inpc_stats;
+
+/* Upper bound (for 4N fragments) of the workspace needed for N points; 0 on invalid arguments. */
+size_t inpc_raster_workspace_bytes(int64_t n_points, int32_t D, int32_t W, int32_t H, uint32_t flags);
+
+/* Forward pass, Algorithm 1.
+ *   pos[N][3], opacity[N] (in [0,1], not clamped), feat[N][D]; cam: host pointer, copied at call time.
+ *   out_feat[H][W][D] = premultiplied composited features, out_alpha[H][W] = sum of blended T*alpha.
+ *   N = 0 is valid (zero image).  `workspace_bytes` >= inpc_raster_workspace_bytes(N, D, W, H, flags). */
+int inpc_raster_forward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                        const inpc_camera* cam, float* out_feat, float* out_alpha,
+                        void* workspace, size_t workspace_bytes, uint32_t flags, void* cuda_stream);
+
+/* Backward pass of L = <grad_out_feat, out_feat> + <grad_out_alpha, out_alpha>.
+ *   Same pos / opacity / feat / N / D / cam and the workspace as left by a forward that had
+ *   INPC_SAVE_FOR_BACKWARD set.  grad_out_alpha may be NULL (= 0).
+ *   grad_feat[N][D], grad_opacity[N], grad_uv[N][2] = dL/d(u, v) in pixels; all three required.
+ *   Culled points and fragments behind the cut-off get exactly 0. */
+int inpc_raster_backward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                         const inpc_camera* cam,
+                         const float* grad_out_feat, const float* grad_out_alpha,
+                         float* grad_feat, float* grad_opacity, float* grad_uv,
+                         void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Parity introspection: all read the workspace of the last forward on it.
+ * counts[H*W] = per-pixel fragment counts (step a2 of the path). */
+int inpc_raster_get_counts(const void* workspace, int32_t W, int32_t H, uint32_t* counts, void* cuda_stream);
+
+/* Needs a forward with INPC_SAVE_SORTED.  *total (host) = number of fragments; synchronises.
+ * With offsets == NULL only *total is returned.  Otherwise offsets[H*W+1] = exclusive sum of counts,
+ * point_idx[total] / depth_bits[total] = every pixel's fragments in blend order (pixel-major). */
+int inpc_raster_get_sorted(const void* workspace, int32_t W, int32_t H, uint32_t* offsets,
+                           uint32_t* point_idx, uint32_t* depth_bits, uint64_t* total, void* cuda_stream);
+
+/* Fills *stats (host) from the workspace of the last forward; synchronises the stream. */
+int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_stream);
+
+const char* inpc_raster_strerror(int status);
+/* CUDA error string of the last INPC_ERR_CUDA on this thread ("" if none). */
+const char* inpc_raster_last_cuda_error(void);
+/* Number of kernels this library has launched so far in this process (all entry points). */
+uint64_t inpc_raster_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* INPC_RASTER_H */

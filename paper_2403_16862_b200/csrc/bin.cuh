@@ -1,0 +1,294 @@
+// bin.cuh -- steps a1/a2 of the hot path: projection, per-cell counting, device-wide scan, record
+// scatter, per-pixel classification and tile work-list construction.
+//
+// Path rows (SURVEY.md section 8a / DESIGN.md section 1):
+//   a1  k_project_count + k_scatter : Eq. 6 projection, cull, bilinear cell + fractions (Eq. 7 inputs)
+//   a2  k_project_count (count), k_scan_u32 (device-wide exclusive scan, decoupled look-back),
+//       k_classify_pixels (per-pixel fragment counts = 2x2 box sum of the cell counts)
+#pragma once
+#include "common.cuh"
+
+namespace inpc {
+
+constexpr int kBinThreads = 256;
+constexpr int kBinPPT     = 4;                          // points per thread
+constexpr int kBinChunk   = kBinThreads * kBinPPT;      // points per CTA iteration
+
+// Coalesced, vectorised staging of a chunk of positions: 3*chunk floats = 768 float4 -> smem.
+__device__ __forceinline__ void stage_positions(const float* __restrict__ pos, long long base, long long N,
+                                                float* s_pos) {
+    const long long f0 = base * 3;                      // first float of the chunk (multiple of 4)
+    const long long fend = N * 3;
+    for (int v = threadIdx.x; v < kBinChunk * 3 / 4; v += kBinThreads) {
+        const long long f = f0 + 4ll * v;
+        float4 q;
+        if (f + 3 < fend) {
+            q = __ldcs(reinterpret_cast<const float4*>(pos + f));
+        } else {
+            q.x = f + 0 < fend ? pos[f + 0] : 0.f;
+            q.y = f + 1 < fend ? pos[f + 1] : 0.f;
+            q.z = f + 2 < fend ? pos[f + 2] : 0.f;
+            q.w = 0.f;
+        }
+        reinterpret_cast<float4*>(s_pos)[v] = q;
+    }
+}
+
+// a1 + a2: project every point, bump its cell counter; the returned old value is the point's rank
+// inside its cell (its slot in the counting sort), stored so that the scatter pass needs no second
+// atomic.  One global atomic per POINT (not per fragment): the 2x2 footprint is implied by the cell.
+__global__ void __launch_bounds__(kBinThreads) k_project_count(const float* __restrict__ pos, long long N,
+                                                                Camera cam, uint32_t* __restrict__ cellcnt,
+                                                                uint32_t* __restrict__ rank) {
+    __shared__ __align__(16) float s_pos[kBinChunk * 3];
+    for (long long base = (long long)blockIdx.x * kBinChunk; base < N; base += (long long)gridDim.x * kBinChunk) {
+        __syncthreads();
+        stage_positions(pos, base, N, s_pos);
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kBinPPT; ++k) {
+            const int l = k * kBinThreads + threadIdx.x;
+            const long long i = base + l;
+            if (i < N) {
+                const Proj p = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]);
+                uint32_t r = 0xFFFFFFFFu;
+                if (p.cell >= 0) r = atomicAdd(&cellcnt[p.cell], 1u);
+                __stcs(&rank[i], r);
+            }
+        }
+    }
+}
+
+// a1 (emission): re-project (bit-identical), slot = celloff[cell] + rank, write the record once.
+template <int D>
+__global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict__ pos,
+                                                          const float* __restrict__ opacity,
+                                                          const float* __restrict__ feat, long long N, Camera cam,
+                                                          const uint32_t* __restrict__ celloff,
+                                                          const uint32_t* __restrict__ rank,
+                                                          float4* __restrict__ rec, float* __restrict__ rop) {
+    constexpr int RV = 1 + D / 4;                        // float4 per record
+    __shared__ __align__(16) float s_pos[kBinChunk * 3];
+    for (long long base = (long long)blockIdx.x * kBinChunk; base < N; base += (long long)gridDim.x * kBinChunk) {
+        __syncthreads();
+        stage_positions(pos, base, N, s_pos);
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kBinPPT; ++k) {
+            const int l = k * kBinThreads + threadIdx.x;
+            const long long i = base + l;
+            if (i >= N) continue;
+            const uint32_t r = __ldcs(&rank[i]);
+            if (r == 0xFFFFFFFFu) continue;
+            const Proj p = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]);
+            const uint32_t slot = __ldg(&celloff[p.cell]) + r;
+            float4 key;
+            key.x = __uint_as_float(p.depth_bits);
+            key.y = __uint_as_float((uint32_t)i);
+            key.z = p.tx;
+            key.w = p.ty;
+            float4* dst = rec + (size_t)slot * RV;
+            dst[0] = key;
+#pragma unroll
+            for (int q = 0; q < D / 4; ++q)
+                dst[1 + q] = __ldcs(reinterpret_cast<const float4*>(feat + (size_t)i * D) + q);
+            rop[slot] = __ldcs(&opacity[i]);
+        }
+    }
+}
+
+// ---- a2: device-wide exclusive scan, single pass with decoupled look-back ---------------------------
+// data[0..n) -> exclusive prefix sums in place; data[n] = total.  status[] (one u64 per tile) and
+// *tile_counter must be zero on entry.  Tiles are claimed through an atomic ticket so that a tile only
+// ever waits on tiles that are already running (forward progress without co-residency assumptions).
+constexpr int kScanThreads = 256;
+constexpr int kScanItems   = 16;
+constexpr int kScanTile    = kScanThreads * kScanItems;
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_u32(uint32_t* __restrict__ data, uint32_t n,
+                                                            unsigned long long* __restrict__ status,
+                                                            uint32_t* __restrict__ tile_counter,
+                                                            uint32_t* __restrict__ total_out) {
+    __shared__ uint32_t s_tile;
+    __shared__ uint32_t s_warp[kScanThreads / 32];
+    __shared__ uint32_t s_prefix;
+    if (threadIdx.x == 0) s_tile = atomicAdd(tile_counter, 1u);
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const uint32_t base = tile * kScanTile + threadIdx.x * kScanItems;
+    uint32_t v[kScanItems];
+    if (base + kScanItems <= n) {
+#pragma unroll
+        for (int q = 0; q < kScanItems / 4; ++q) {
+            const uint4 t = reinterpret_cast<const uint4*>(data + base)[q];
+            v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < kScanItems; ++q) v[q] = base + q < n ? data[base + q] : 0u;
+    }
+    uint32_t sum = 0;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) { const uint32_t t = v[q]; v[q] = sum; sum += t; }
+    // block-wide exclusive scan of the per-thread sums
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = lane < kScanThreads / 32 ? s_warp[lane] : 0u;
+#pragma unroll
+        for (int d = 1; d < kScanThreads / 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, w, d); if (lane >= d) w += t; }
+        if (lane < kScanThreads / 32) s_warp[lane] = w;                       // inclusive over warps
+        const uint32_t aggregate = __shfl_sync(0xffffffffu, w, kScanThreads / 32 - 1);
+        // publish the aggregate, then look back
+        volatile unsigned long long* st = status;
+        if (lane == 0) {
+            const unsigned long long flag = tile == 0 ? 2ull : 1ull;
+            st[tile] = (flag << 62) | aggregate;
+            __threadfence();
+        }
+        uint32_t prefix = 0;
+        if (tile > 0) {
+            int look = (int)tile - 1;
+            while (true) {                                                     // warp-wide window of 32 predecessors
+                const int idx = look - lane;
+                unsigned long long s = idx >= 0 ? st[idx] : (2ull << 62);
+                while (__any_sync(0xffffffffu, (s >> 62) == 0ull)) { s = idx >= 0 ? st[idx] : (2ull << 62); }
+                const uint32_t incl_mask = __ballot_sync(0xffffffffu, (s >> 62) == 2ull);
+                const int first_incl = incl_mask ? __ffs(incl_mask) - 1 : 32;  // nearest tile with an inclusive prefix
+                uint32_t contrib = lane <= first_incl ? (uint32_t)(s & 0xffffffffull) : 0u;
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, d);
+                prefix += contrib;
+                if (incl_mask) break;
+                look -= 32;
+            }
+            if (lane == 0) {
+                __threadfence();
+                st[tile] = (2ull << 62) | (unsigned long long)(prefix + aggregate);
+            }
+        }
+        if (lane == 0) {
+            s_prefix = prefix;
+            if ((tile + 1) * (unsigned long long)kScanTile >= n) {             // last tile: total
+                data[n] = prefix + aggregate;
+                if (total_out) *total_out = prefix + aggregate;
+            }
+        }
+    }
+    __syncthreads();
+    const uint32_t off = s_prefix + (warp > 0 ? s_warp[warp - 1] : 0u) + (inc - sum);
+    if (base + kScanItems <= n) {
+#pragma unroll
+        for (int q = 0; q < kScanItems / 4; ++q)
+            reinterpret_cast<uint4*>(data + base)[q] =
+                make_uint4(v[4 * q] + off, v[4 * q + 1] + off, v[4 * q + 2] + off, v[4 * q + 3] + off);
+    } else {
+#pragma unroll
+        for (int q = 0; q < kScanItems; ++q)
+            if (base + q < n) data[base + q] = v[q] + off;
+    }
+}
+
+// ---- a2: per-pixel fragment counts (2x2 box sum of the cell counts) ---------------------------------
+__device__ __forceinline__ uint32_t pixel_count(const uint32_t* __restrict__ celloff, int W, int x, int y) {
+    const uint32_t c0 = (uint32_t)y * (W + 1) + x, c1 = c0 + (W + 1);
+    return (__ldg(&celloff[c0 + 2]) - __ldg(&celloff[c0])) + (__ldg(&celloff[c1 + 2]) - __ldg(&celloff[c1]));
+}
+
+// One thread per pixel: total fragment count, long-run ("big") pixel list, optional count image.
+__global__ void __launch_bounds__(256) k_classify_pixels(const uint32_t* __restrict__ celloff, int W, int H,
+                                                          Header* __restrict__ hdr, BigEntry* __restrict__ big,
+                                                          uint32_t* __restrict__ pixcnt) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t n = 0;
+    if (p < W * H) {
+        const int y = p / W, x = p - y * W;
+        n = pixel_count(celloff, W, x, y);
+        if (pixcnt) pixcnt[p] = n;
+        if (n > (uint32_t)kPixMax) {
+            const unsigned long long old = atomicAdd(&hdr->big_packed, (1ull << 40) | (unsigned long long)n);
+            const uint32_t b = (uint32_t)(old >> 40);
+            const uint32_t start = (uint32_t)(old & ((1ull << 40) - 1));
+            BigEntry e;
+            e.pix = (uint32_t)p; e.n = n; e.start = start; e.nb = 0;
+            e.tin_base = (start >> 5) + b;               // disjoint per-chunk slots (see big.cuh)
+            e.pad[0] = e.pad[1] = e.pad[2] = 0;
+            big[b] = e;
+        }
+    }
+    // block reduction of n -> one 64-bit atomic per CTA
+    unsigned long long s = n;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+    __shared__ unsigned long long s_sum[8];
+    if ((threadIdx.x & 31) == 0) s_sum[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+        for (int w = 0; w < 8; ++w) t += s_sum[w];
+        if (t) atomicAdd(&hdr->n_fragments, t);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_counts_out(const uint32_t* __restrict__ celloff, int W, int H,
+                                                     uint32_t* __restrict__ counts) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < W * H) { const int y = p / W; counts[p] = pixel_count(celloff, W, p - y * W, y); }
+}
+
+// Records a tile item of tw x th pixels at (X, Y) stages into shared memory: each of its th+1 cell
+// rows is one contiguous record range, widened to multiples of 4 records (16-byte bulk copies).
+__device__ __forceinline__ uint32_t tile_padded_records(const uint32_t* __restrict__ celloff, int W, int H, int X,
+                                                        int Y, int tw, int th) {
+    uint32_t tot = 0;
+    for (int r = 0; r <= th; ++r) {
+        const int j = Y + r;
+        if (j > H) break;
+        const uint32_t rowbase = (uint32_t)j * (W + 1);
+        const uint32_t a = __ldg(&celloff[rowbase + min(X, W + 1)]);
+        const uint32_t b = __ldg(&celloff[rowbase + min(X + tw + 1, W + 1)]);
+        tot += ((b + 3u) & ~3u) - (a & ~3u);
+    }
+    return tot;
+}
+
+// One thread per base tile: emit it if its records fit the shared-memory capacity, otherwise split
+// (16x8 -> 8x4 -> 4x2 -> 2x1 -> 1x1).  A 1x1 leaf deeper than kPixMax belongs to the long-run path.
+__global__ void __launch_bounds__(128) k_build_items(const uint32_t* __restrict__ celloff, int W, int H, int cap,
+                                                      Header* __restrict__ hdr, uint32_t* __restrict__ items) {
+    const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntx * nty) return;
+    const int X0 = (t % ntx) * kTileW, Y0 = (t / ntx) * kTileH;
+    // explicit DFS stack: (X, Y, lw, lh); depth <= 5, at most 3 siblings pending per level
+    uint32_t stack[20];
+    int sp = 0;
+    stack[sp++] = encode_item(X0, Y0, kTileLW, kTileLH);
+    while (sp > 0) {
+        const uint32_t it = stack[--sp];
+        const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
+        if (X >= W || Y >= H) continue;
+        const int tw = 1 << lw, th = 1 << lh;
+        const uint32_t n = tile_padded_records(celloff, W, H, X, Y, tw, th);
+        if (lw == 0 && lh == 0) {
+            if (pixel_count(celloff, W, X, Y) <= (uint32_t)kPixMax) items[atomicAdd(&hdr->n_items, 1u)] = it;
+            continue;
+        }
+        if (n <= (uint32_t)cap) {
+            items[atomicAdd(&hdr->n_items, 1u)] = it;
+            continue;
+        }
+        const int nlw = lw > 0 ? lw - 1 : 0, nlh = lh > 0 ? lh - 1 : 0;
+        const int hw = 1 << nlw, hh = 1 << nlh;
+        stack[sp++] = encode_item(X, Y, nlw, nlh);
+        if (lw > 0) stack[sp++] = encode_item(X + hw, Y, nlw, nlh);
+        if (lh > 0) stack[sp++] = encode_item(X, Y + hh, nlw, nlh);
+        if (lw > 0 && lh > 0) stack[sp++] = encode_item(X + hw, Y + hh, nlw, nlh);
+    }
+}
+
+}  // namespace inpc

@@ -1,0 +1,406 @@
+// inpc_raster.cu -- C ABI (include/inpc_raster.h) over the sm_100a kernels in bin.cuh / tile.cuh / big.cuh.
+//
+// Forward  = memset | k_project_count | k_scan_u32 | k_scatter | k_classify_pixels | [k_scan_u32] |
+//            k_build_items | k_big<fwd> | k_tile<fwd>           (all on the caller's stream, no sync)
+// Backward = memset x3 | k_tile<bwd> | k_big<bwd>
+// No device memory is allocated here; there is no CPU fallback.
+#include "../../include/inpc_raster.h"
+
+#include <atomic>
+#include <mutex>
+#include <string>
+#include <unordered_map>
+
+#include "bin.cuh"
+#include "big.cuh"
+#include "common.cuh"
+#include "tile.cuh"
+
+namespace inpc {
+
+static thread_local std::string t_cuda_error;
+static std::atomic<uint64_t> g_launches{0};
+
+struct Layout {
+    size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
+    size_t rank, rec, rop, items, big, bigkeys, bigtin;
+    size_t pixoff, sorted_idx, sorted_depth;              // only with INPC_SAVE_SORTED
+    size_t total;
+    uint32_t C, P, max_big, n_status;
+};
+
+static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
+    Layout L{};
+    const size_t n = (size_t)N;
+    L.C = (uint32_t)((W + 1) * (H + 1));
+    L.P = (uint32_t)(W * H);
+    L.n_status = (uint32_t)((std::max(L.C, L.P) + kScanTile - 1) / kScanTile + 1);
+    const size_t four_n = 4 * n;
+    L.max_big = (uint32_t)std::min<size_t>(L.P, four_n / (kPixMax + 1) + 1);
+    size_t o = 0;
+    L.header = o;  o = align_up(o + sizeof(Header));
+    L.status0 = o; o = align_up(o + (size_t)L.n_status * 8);
+    L.status1 = o; o = align_up(o + (size_t)L.n_status * 8);
+    L.cellcnt = o; o = align_up(o + ((size_t)L.C + 1) * 4);
+    L.zero_end = o;
+    L.rank = o;    o = align_up(o + n * 4 + 16);
+    L.rec = o;     o = align_up(o + (n + 8) * (size_t)(16 + 4 * D));
+    L.rop = o;     o = align_up(o + (n + 8) * 4);
+    const size_t nbase = (size_t)((W + kTileW - 1) / kTileW) * ((H + kTileH - 1) / kTileH);
+    L.items = o;   o = align_up(o + ((size_t)L.P + nbase + 16) * 4);
+    L.big = o;     o = align_up(o + ((size_t)L.max_big + 1) * sizeof(BigEntry));
+    L.bigkeys = o; o = align_up(o + (four_n + 8) * 8);
+    L.bigtin = o;  o = align_up(o + (four_n / 32 + L.max_big + 8) * 4);
+    if (flags & INPC_SAVE_SORTED) {
+        L.pixoff = o;       o = align_up(o + ((size_t)L.P + 1) * 4);
+        L.sorted_idx = o;   o = align_up(o + (four_n + 8) * 4);
+        L.sorted_depth = o; o = align_up(o + (four_n + 8) * 4);
+    }
+    L.total = o;
+    return L;
+}
+
+// Host-side note of what the last forward left in a workspace (argument validation only; the
+// library keeps no device state and allocates nothing).
+struct Saved { int64_t N; int D, W, H; uint32_t flags; };
+static std::mutex g_mu;
+static std::unordered_map<const void*, Saved> g_saved;
+
+struct DeviceInfo { int sms = 0; bool ok = false; };
+static DeviceInfo device_info() {
+    static DeviceInfo cached[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return DeviceInfo{};
+    if (!cached[dev].ok) {
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return DeviceInfo{};
+        cached[dev].sms = sms; cached[dev].ok = true;
+    }
+    return cached[dev];
+}
+
+static int cuda_fail(cudaError_t e) {
+    t_cuda_error = cudaGetErrorString(e);
+    return INPC_ERR_CUDA;
+}
+#define INPC_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
+#define INPC_LAUNCHED() do { g_launches.fetch_add(1, std::memory_order_relaxed); cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int check_common(int64_t N, int D, const inpc_camera* cam) {
+    if (!cam || N < 0 || N >= (1ll << 30)) return INPC_ERR_INVALID_ARG;
+    if (cam->width <= 0 || cam->height <= 0 || !(cam->near_z < cam->far_z)) return INPC_ERR_INVALID_ARG;
+    if (D != 4 && D != 8) return INPC_ERR_UNSUPPORTED;
+    if (cam->width > 4095 || cam->height > 4095) return INPC_ERR_UNSUPPORTED;
+    return INPC_OK;
+}
+
+static Camera to_camera(const inpc_camera* c) {
+    Camera k;
+    k.fx = c->fx; k.fy = c->fy; k.cx = c->cx; k.cy = c->cy;
+    for (int i = 0; i < 9; ++i) k.R[i] = c->R[i];
+    for (int i = 0; i < 3; ++i) k.t[i] = c->t[i];
+    k.near_z = c->near_z; k.far_z = c->far_z; k.W = c->width; k.H = c->height;
+    return k;
+}
+
+template <typename K>
+static int persistent_grid(K kernel, int threads, size_t smem, int sms, int* out) {
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (per_sm < 1) per_sm = 1;
+    *out = per_sm * sms;
+    return INPC_OK;
+}
+
+template <int D, int MODE>
+static int launch_tile(const TileArgs& A, int sms, cudaStream_t st) {
+    constexpr size_t smem = tile_smem_bytes<D, MODE>();
+    static bool configured = false;
+    static int grid = 0;
+    if (!configured) {
+        INPC_CUDA(cudaFuncSetAttribute(k_tile<D, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int rc = persistent_grid(k_tile<D, MODE>, kTileThreads, smem, sms, &grid);
+        if (rc != INPC_OK) return rc;
+        configured = true;
+    }
+    k_tile<D, MODE><<<grid, kTileThreads, smem, st>>>(A);
+    INPC_LAUNCHED();
+    return INPC_OK;
+}
+
+template <int D, int MODE>
+static int launch_big(const BigArgs& A, int sms, uint32_t max_big, cudaStream_t st) {
+    constexpr size_t smem = MODE == kBwd ? 0 : (size_t)kBigChunk * 8;
+    static bool configured = false;
+    static int grid = 0;
+    if (!configured) {
+        if (smem > 48 * 1024)
+            INPC_CUDA(cudaFuncSetAttribute(k_big<D, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int rc = persistent_grid(k_big<D, MODE>, kBigThreads, smem, sms, &grid);
+        if (rc != INPC_OK) return rc;
+        configured = true;
+    }
+    const int g = (int)std::min<uint32_t>((uint32_t)grid, std::max<uint32_t>(max_big, 1u));
+    k_big<D, MODE><<<g, kBigThreads, smem, st>>>(A);
+    INPC_LAUNCHED();
+    return INPC_OK;
+}
+
+__global__ void k_write_header(Header* h, uint32_t flags, int W, int H, int D, uint32_t N) {
+    h->magic = kMagic; h->flags = flags; h->W = W; h->H = H; h->D = D; h->n_points = N;
+}
+
+template <int D>
+static int forward_impl(const float* pos, const float* opacity, const float* feat, int64_t N, const inpc_camera* cam,
+                        float* out_feat, float* out_alpha, unsigned char* ws, const Layout& L, uint32_t flags,
+                        cudaStream_t st) {
+    const DeviceInfo di = device_info();
+    if (!di.ok) return cuda_fail(cudaGetLastError() == cudaSuccess ? cudaErrorNoDevice : cudaErrorNoDevice);
+    const Camera camk = to_camera(cam);
+    const int W = cam->width, H = cam->height;
+    Header* hdr = reinterpret_cast<Header*>(ws + L.header);
+    uint32_t* cellcnt = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
+    uint32_t* rank = reinterpret_cast<uint32_t*>(ws + L.rank);
+    float4* rec = reinterpret_cast<float4*>(ws + L.rec);
+    float* rop = reinterpret_cast<float*>(ws + L.rop);
+    uint32_t* items = reinterpret_cast<uint32_t*>(ws + L.items);
+    BigEntry* big = reinterpret_cast<BigEntry*>(ws + L.big);
+    const bool dump = (flags & INPC_SAVE_SORTED) != 0;
+    uint32_t* pixoff = dump ? reinterpret_cast<uint32_t*>(ws + L.pixoff) : nullptr;
+
+    INPC_CUDA(cudaMemsetAsync(ws + L.header, 0, L.zero_end - L.header, st));
+    k_write_header<<<1, 1, 0, st>>>(hdr, flags, W, H, D, (uint32_t)N);
+    INPC_LAUNCHED();
+    if (N > 0) {
+        const int grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
+        k_project_count<<<grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, rank);
+        INPC_LAUNCHED();
+    }
+    k_scan_u32<<<(L.C + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
+        cellcnt, L.C, reinterpret_cast<unsigned long long*>(ws + L.status0), &hdr->scan_tile_counter, &hdr->nrec);
+    INPC_LAUNCHED();
+    if (N > 0) {
+        const int grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
+        k_scatter<D><<<grid, kBinThreads, 0, st>>>(pos, opacity, feat, (long long)N, camk, cellcnt, rank, rec, rop);
+        INPC_LAUNCHED();
+    }
+    k_classify_pixels<<<(L.P + 255) / 256, 256, 0, st>>>(cellcnt, W, H, hdr, big, pixoff);
+    INPC_LAUNCHED();
+    if (dump) {
+        k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
+            pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr);
+        INPC_LAUNCHED();
+    }
+    const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
+    k_build_items<<<(ntx * nty + 127) / 128, 128, 0, st>>>(cellcnt, W, H, TileCfg<D>::kCap, hdr, items);
+    INPC_LAUNCHED();
+
+    BigArgs B{};
+    B.hdr = hdr; B.big_cursor = &hdr->big_cursor; B.big = big; B.celloff = cellcnt; B.rec = rec; B.rop = rop;
+    B.bigkeys = reinterpret_cast<unsigned long long*>(ws + L.bigkeys);
+    B.bigtin = reinterpret_cast<float*>(ws + L.bigtin);
+    B.W = W; B.H = H; B.out_feat = out_feat; B.out_alpha = out_alpha;
+    TileArgs A{};
+    A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = items; A.celloff = cellcnt; A.rec = rec; A.rop = rop;
+    A.W = W; A.H = H; A.out_feat = out_feat; A.out_alpha = out_alpha;
+    if (dump) {
+        B.pixoff = A.pixoff = pixoff;
+        B.sorted_idx = A.sorted_idx = reinterpret_cast<uint32_t*>(ws + L.sorted_idx);
+        B.sorted_depth = A.sorted_depth = reinterpret_cast<uint32_t*>(ws + L.sorted_depth);
+    }
+    int rc;
+    if (N > 0) {
+        rc = dump ? launch_big<D, kFwdDump>(B, di.sms, L.max_big, st) : launch_big<D, kFwd>(B, di.sms, L.max_big, st);
+        if (rc != INPC_OK) return rc;
+    }
+    rc = dump ? launch_tile<D, kFwdDump>(A, di.sms, st) : launch_tile<D, kFwd>(A, di.sms, st);
+    return rc;
+}
+
+template <int D>
+static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat, const float* g_alpha, float* d_feat,
+                         float* d_opacity, float* d_uv, unsigned char* ws, const Layout& L, cudaStream_t st) {
+    const DeviceInfo di = device_info();
+    if (!di.ok) return cuda_fail(cudaErrorNoDevice);
+    const int W = cam->width, H = cam->height;
+    Header* hdr = reinterpret_cast<Header*>(ws + L.header);
+    if (N > 0) {
+        INPC_CUDA(cudaMemsetAsync(d_feat, 0, (size_t)N * D * 4, st));
+        INPC_CUDA(cudaMemsetAsync(d_opacity, 0, (size_t)N * 4, st));
+        INPC_CUDA(cudaMemsetAsync(d_uv, 0, (size_t)N * 8, st));
+    }
+    INPC_CUDA(cudaMemsetAsync(&hdr->item_cursor, 0, 8, st));     // item_cursor + big_cursor
+    TileArgs A{};
+    A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = reinterpret_cast<uint32_t*>(ws + L.items);
+    A.celloff = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
+    A.rec = reinterpret_cast<float4*>(ws + L.rec); A.rop = reinterpret_cast<float*>(ws + L.rop);
+    A.W = W; A.H = H; A.g_feat = g_feat; A.g_alpha = g_alpha; A.d_feat = d_feat; A.d_opacity = d_opacity; A.d_uv = d_uv;
+    int rc = launch_tile<D, kBwd>(A, di.sms, st);
+    if (rc != INPC_OK) return rc;
+    if (N > 0) {
+        BigArgs B{};
+        B.hdr = hdr; B.big_cursor = &hdr->big_cursor; B.big = reinterpret_cast<BigEntry*>(ws + L.big);
+        B.celloff = A.celloff; B.rec = A.rec; B.rop = A.rop;
+        B.bigkeys = reinterpret_cast<unsigned long long*>(ws + L.bigkeys);
+        B.bigtin = reinterpret_cast<float*>(ws + L.bigtin);
+        B.W = W; B.H = H; B.g_feat = g_feat; B.g_alpha = g_alpha; B.d_feat = d_feat; B.d_opacity = d_opacity; B.d_uv = d_uv;
+        rc = launch_big<D, kBwd>(B, di.sms, L.max_big, st);
+    }
+    return rc;
+}
+
+}  // namespace inpc
+
+using namespace inpc;
+
+extern "C" {
+
+size_t inpc_raster_workspace_bytes(int64_t n_points, int32_t D, int32_t W, int32_t H, uint32_t flags) {
+    if (n_points < 0 || n_points >= (1ll << 30) || (D != 4 && D != 8) || W <= 0 || H <= 0 || W > 4095 || H > 4095) return 0;
+    return make_layout(n_points, D, W, H, flags).total;
+}
+
+int inpc_raster_forward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                        const inpc_camera* cam, float* out_feat, float* out_alpha, void* workspace,
+                        size_t workspace_bytes, uint32_t flags, void* cuda_stream) {
+    int rc = check_common(N, D, cam);
+    if (rc != INPC_OK) return rc;
+    if (!out_feat || !out_alpha || !workspace) return INPC_ERR_INVALID_ARG;
+    if (N > 0 && (!pos || !opacity || !feat)) return INPC_ERR_INVALID_ARG;
+    if (!aligned16(pos) || !aligned16(opacity) || !aligned16(feat) || !aligned16(out_feat) || !aligned16(out_alpha) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 255u))
+        return INPC_ERR_INVALID_ARG;
+    const Layout L = make_layout(N, D, cam->width, cam->height, flags);
+    if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        g_saved.erase(workspace);
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    rc = D == 4 ? forward_impl<4>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st)
+                : forward_impl<8>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st);
+    if (rc == INPC_OK) {
+        std::lock_guard<std::mutex> lk(g_mu);
+        g_saved[workspace] = Saved{N, D, cam->width, cam->height, flags};
+    }
+    return rc;
+}
+
+int inpc_raster_backward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                         const inpc_camera* cam, const float* grad_out_feat, const float* grad_out_alpha,
+                         float* grad_feat, float* grad_opacity, float* grad_uv, void* workspace,
+                         size_t workspace_bytes, void* cuda_stream) {
+    (void)pos; (void)opacity; (void)feat;   // the records saved by the forward hold what the backward needs
+    int rc = check_common(N, D, cam);
+    if (rc != INPC_OK) return rc;
+    if (!grad_out_feat || !grad_feat || !grad_opacity || !grad_uv || !workspace) return INPC_ERR_INVALID_ARG;
+    if (!aligned16(grad_out_feat) || !aligned16(grad_out_alpha) || !aligned16(grad_feat) || !aligned16(grad_opacity) ||
+        !aligned16(grad_uv))
+        return INPC_ERR_INVALID_ARG;
+    Saved s;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        auto it = g_saved.find(workspace);
+        if (it == g_saved.end()) return INPC_ERR_NO_SAVED_STATE;
+        s = it->second;
+    }
+    if (!(s.flags & INPC_SAVE_FOR_BACKWARD)) return INPC_ERR_NO_SAVED_STATE;
+    if (s.N != N || s.D != D || s.W != cam->width || s.H != cam->height) return INPC_ERR_INVALID_ARG;
+    const Layout L = make_layout(N, D, s.W, s.H, s.flags);
+    if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    return D == 4 ? backward_impl<4>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, ws, L, st)
+                  : backward_impl<8>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, ws, L, st);
+}
+
+static int find_saved(const void* workspace, int32_t W, int32_t H, Saved* out) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto it = g_saved.find(workspace);
+    if (it == g_saved.end()) return INPC_ERR_NO_SAVED_STATE;
+    if (W > 0 && (it->second.W != W || it->second.H != H)) return INPC_ERR_INVALID_ARG;
+    *out = it->second;
+    return INPC_OK;
+}
+
+int inpc_raster_get_counts(const void* workspace, int32_t W, int32_t H, uint32_t* counts, void* cuda_stream) {
+    if (!workspace || !counts || W <= 0 || H <= 0) return INPC_ERR_INVALID_ARG;
+    Saved s;
+    int rc = find_saved(workspace, W, H, &s);
+    if (rc != INPC_OK) return rc;
+    const Layout L = make_layout(s.N, s.D, s.W, s.H, s.flags);
+    const unsigned char* ws = static_cast<const unsigned char*>(workspace);
+    k_counts_out<<<(L.P + 255) / 256, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        reinterpret_cast<const uint32_t*>(ws + L.cellcnt), W, H, counts);
+    INPC_LAUNCHED();
+    return INPC_OK;
+}
+
+int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_stream) {
+    if (!workspace || !stats) return INPC_ERR_INVALID_ARG;
+    Saved s;
+    int rc = find_saved(workspace, 0, 0, &s);
+    if (rc != INPC_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Header h;
+    INPC_CUDA(cudaMemcpyAsync(&h, workspace, sizeof(Header), cudaMemcpyDeviceToHost, st));
+    INPC_CUDA(cudaStreamSynchronize(st));
+    if (h.magic != kMagic) return INPC_ERR_NO_SAVED_STATE;
+    stats->n_points = h.n_points;
+    stats->n_kept = h.nrec;
+    stats->n_fragments = h.n_fragments;
+    stats->n_tile_items = h.n_items;
+    stats->n_big_pixels = h.big_packed >> 40;
+    stats->n_big_fragments = h.big_packed & ((1ull << 40) - 1);
+    return INPC_OK;
+}
+
+int inpc_raster_get_sorted(const void* workspace, int32_t W, int32_t H, uint32_t* offsets, uint32_t* point_idx,
+                           uint32_t* depth_bits, uint64_t* total, void* cuda_stream) {
+    if (!workspace || !total || W <= 0 || H <= 0) return INPC_ERR_INVALID_ARG;
+    Saved s;
+    int rc = find_saved(workspace, W, H, &s);
+    if (rc != INPC_OK) return rc;
+    if (!(s.flags & INPC_SAVE_SORTED)) return INPC_ERR_NO_SAVED_STATE;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const Layout L = make_layout(s.N, s.D, s.W, s.H, s.flags);
+    const unsigned char* ws = static_cast<const unsigned char*>(workspace);
+    Header h;
+    INPC_CUDA(cudaMemcpyAsync(&h, ws, sizeof(Header), cudaMemcpyDeviceToHost, st));
+    INPC_CUDA(cudaStreamSynchronize(st));
+    if (h.magic != kMagic) return INPC_ERR_NO_SAVED_STATE;
+    *total = h.n_fragments;
+    if (!offsets) return INPC_OK;
+    if (!point_idx || !depth_bits) return INPC_ERR_INVALID_ARG;
+    INPC_CUDA(cudaMemcpyAsync(offsets, ws + L.pixoff, ((size_t)L.P + 1) * 4, cudaMemcpyDeviceToDevice, st));
+    if (h.n_fragments) {
+        INPC_CUDA(cudaMemcpyAsync(point_idx, ws + L.sorted_idx, (size_t)h.n_fragments * 4, cudaMemcpyDeviceToDevice, st));
+        INPC_CUDA(cudaMemcpyAsync(depth_bits, ws + L.sorted_depth, (size_t)h.n_fragments * 4, cudaMemcpyDeviceToDevice, st));
+    }
+    INPC_CUDA(cudaStreamSynchronize(st));
+    return INPC_OK;
+}
+
+const char* inpc_raster_strerror(int status) {
+    switch (status) {
+        case INPC_OK: return "ok";
+        case INPC_ERR_INVALID_ARG: return "invalid argument";
+        case INPC_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+        case INPC_ERR_CUDA: return "CUDA error (see inpc_raster_last_cuda_error)";
+        case INPC_ERR_NO_SAVED_STATE: return "workspace holds no matching forward state";
+        case INPC_ERR_UNSUPPORTED: return "unsupported D or image size";
+        default: return "unknown status";
+    }
+}
+
+const char* inpc_raster_last_cuda_error(void) { return t_cuda_error.c_str(); }
+
+uint64_t inpc_raster_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+}  // extern "C"

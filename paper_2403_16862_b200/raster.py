@@ -1,0 +1,202 @@
+"""Thin ctypes binding over the C ABI in include/inpc_raster.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of csrc/; PyTorch is used for device memory and
+streams.  There is no CPU fallback: if libinpc_raster.so is missing (run
+`python -m paper_2403_16862_b200.build` or `__graft_entry__.build()`), loading raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libinpc_raster.so")
+
+SAVE_FOR_BACKWARD = 1
+SAVE_SORTED = 2
+
+EXPORTS = (
+    "inpc_raster_workspace_bytes", "inpc_raster_forward", "inpc_raster_backward",
+    "inpc_raster_get_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
+    "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count",
+)
+
+
+class InpcCamera(C.Structure):
+    _fields_ = [("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float), ("cy", C.c_float),
+                ("R", C.c_float * 9), ("t", C.c_float * 3),
+                ("near_z", C.c_float), ("far_z", C.c_float),
+                ("width", C.c_int32), ("height", C.c_int32)]
+
+
+class InpcStats(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("n_points", "n_kept", "n_fragments", "n_tile_items",
+                                          "n_big_pixels", "n_big_fragments")]
+
+
+class InpcError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        lib = load()
+        msg = lib.inpc_raster_strerror(status).decode()
+        if status == -3:
+            msg += ": " + lib.inpc_raster_last_cuda_error().decode()
+        super().__init__(f"{where} failed ({status}): {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """dlopen libinpc_raster.so; raises (loudly) when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: the CUDA library has not been built "
+                              "(python -m paper_2403_16862_b200.build); there is no CPU fallback")
+        lib = C.CDLL(LIB_PATH)
+        vp, i64, i32, u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint32
+        lib.inpc_raster_workspace_bytes.restype = C.c_size_t
+        lib.inpc_raster_workspace_bytes.argtypes = [i64, i32, i32, i32, u32]
+        lib.inpc_raster_forward.restype = C.c_int
+        lib.inpc_raster_forward.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, C.c_size_t, u32, vp]
+        lib.inpc_raster_backward.restype = C.c_int
+        lib.inpc_raster_backward.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        lib.inpc_raster_get_counts.restype = C.c_int
+        lib.inpc_raster_get_counts.argtypes = [vp, i32, i32, vp, vp]
+        lib.inpc_raster_get_sorted.restype = C.c_int
+        lib.inpc_raster_get_sorted.argtypes = [vp, i32, i32, vp, vp, vp, C.POINTER(C.c_uint64), vp]
+        lib.inpc_raster_get_stats.restype = C.c_int
+        lib.inpc_raster_get_stats.argtypes = [vp, C.POINTER(InpcStats), vp]
+        lib.inpc_raster_strerror.restype = C.c_char_p
+        lib.inpc_raster_strerror.argtypes = [C.c_int]
+        lib.inpc_raster_last_cuda_error.restype = C.c_char_p
+        lib.inpc_raster_launch_count.restype = C.c_uint64
+        _lib = lib
+    return _lib
+
+
+def camera_struct(cam) -> InpcCamera:
+    """cam: any object with fx, fy, cx, cy, R (3x3), t (3), near_z, far_z, width, height."""
+    c = InpcCamera()
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    R = [float(x) for row in cam.R for x in (row if hasattr(row, "__len__") else [row])]
+    t = [float(x) for x in cam.t]
+    for i in range(9):
+        c.R[i] = R[i]
+    for i in range(3):
+        c.t[i] = t[i]
+    c.near_z, c.far_z = float(cam.near_z), float(cam.far_z)
+    c.width, c.height = int(cam.width), int(cam.height)
+    return c
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check(t, dtype, name):
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise ValueError(f"{name} must be a contiguous CUDA tensor of dtype {dtype}")
+
+
+def inpc_raster_workspace_bytes(N: int, D: int, W: int, H: int, flags: int = SAVE_FOR_BACKWARD) -> int:
+    return int(load().inpc_raster_workspace_bytes(N, D, W, H, flags))
+
+
+def alloc_workspace(N: int, D: int, W: int, H: int, flags: int = SAVE_FOR_BACKWARD, device="cuda") -> torch.Tensor:
+    nbytes = inpc_raster_workspace_bytes(N, D, W, H, flags)
+    if nbytes == 0:
+        raise ValueError("unsupported problem size / D")
+    return torch.empty(nbytes, dtype=torch.uint8, device=device)
+
+
+def inpc_raster_forward(pos, opacity, feat, cam, out_feat=None, out_alpha=None, workspace=None,
+                        flags: int = SAVE_FOR_BACKWARD, stream=None):
+    """-> (out_feat[H,W,D], out_alpha[H,W], workspace).  Enqueues on the current stream; no sync."""
+    lib = load()
+    _check(pos, torch.float32, "pos"); _check(opacity, torch.float32, "opacity"); _check(feat, torch.float32, "feat")
+    N, D = int(pos.shape[0]), int(feat.shape[1])
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    W, H = cs.width, cs.height
+    if workspace is None:
+        workspace = alloc_workspace(N, D, W, H, flags, pos.device)
+    if out_feat is None:
+        out_feat = torch.empty((H, W, D), dtype=torch.float32, device=pos.device)
+    if out_alpha is None:
+        out_alpha = torch.empty((H, W), dtype=torch.float32, device=pos.device)
+    rc = lib.inpc_raster_forward(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(out_feat),
+                                 _ptr(out_alpha), _ptr(workspace), workspace.numel(), flags, _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_forward")
+    return out_feat, out_alpha, workspace
+
+
+def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha, workspace,
+                         grad_feat=None, grad_opacity=None, grad_uv=None, stream=None):
+    """-> (grad_feat[N,D], grad_opacity[N], grad_uv[N,2]).  Enqueues on the current stream; no sync."""
+    lib = load()
+    N, D = int(pos.shape[0]), int(feat.shape[1])
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    _check(grad_out_feat, torch.float32, "grad_out_feat")
+    if grad_out_alpha is not None:
+        _check(grad_out_alpha, torch.float32, "grad_out_alpha")
+    dev = pos.device
+    if grad_feat is None:
+        grad_feat = torch.empty((N, D), dtype=torch.float32, device=dev)
+    if grad_opacity is None:
+        grad_opacity = torch.empty((N,), dtype=torch.float32, device=dev)
+    if grad_uv is None:
+        grad_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
+    rc = lib.inpc_raster_backward(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(grad_out_feat),
+                                  _ptr(grad_out_alpha), _ptr(grad_feat), _ptr(grad_opacity), _ptr(grad_uv),
+                                  _ptr(workspace), workspace.numel(), _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_backward")
+    return grad_feat, grad_opacity, grad_uv
+
+
+def inpc_raster_get_counts(workspace, W: int, H: int, stream=None) -> torch.Tensor:
+    counts = torch.empty((H, W), dtype=torch.int32, device=workspace.device)
+    rc = load().inpc_raster_get_counts(_ptr(workspace), W, H, _ptr(counts), _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_get_counts")
+    return counts
+
+
+def inpc_raster_get_sorted(workspace, W: int, H: int, stream=None):
+    """-> offsets[H*W+1], point_idx[total], depth_bits[total] (int32 tensors holding the u32 bit patterns)."""
+    lib = load()
+    total = C.c_uint64(0)
+    rc = lib.inpc_raster_get_sorted(_ptr(workspace), W, H, None, None, None, C.byref(total), _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_get_sorted")
+    n = int(total.value)
+    dev = workspace.device
+    offsets = torch.empty(W * H + 1, dtype=torch.int32, device=dev)
+    idx = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    depth = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    rc = lib.inpc_raster_get_sorted(_ptr(workspace), W, H, _ptr(offsets), _ptr(idx), _ptr(depth), C.byref(total),
+                                    _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_get_sorted")
+    return offsets, idx[:n], depth[:n]
+
+
+def inpc_raster_get_stats(workspace, stream=None) -> dict:
+    st = InpcStats()
+    rc = load().inpc_raster_get_stats(_ptr(workspace), C.byref(st), _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_get_stats")
+    return {n: int(getattr(st, n)) for n, _ in InpcStats._fields_}
+
+
+def inpc_raster_launch_count() -> int:
+    return int(load().inpc_raster_launch_count())
