@@ -109,6 +109,16 @@ const char* inpc_raster_last_cuda_error(void);
 /* Number of kernels this library has launched so far in this process (all entry points). */
 uint64_t inpc_raster_launch_count(void);
 
+/* Profiling aid (bench.py's roofline).  With timing enabled every stage the library enqueues is
+ * bracketed by two cudaEvents on the caller's stream (a few microseconds per stage; off by default).
+ * inpc_raster_get_kernel_times waits for the recorded events and returns, per stage i in
+ * [0, inpc_raster_kernel_count()), the summed device time ms[i] (milliseconds) and the number of
+ * timed launches since the last reset; ms / launches are HOST arrays of that length. */
+int         inpc_raster_set_kernel_timing(int enable);
+int         inpc_raster_kernel_count(void);
+const char* inpc_raster_kernel_name(int i);
+int         inpc_raster_get_kernel_times(double* ms, uint64_t* launches, int reset);
+
 #ifdef __cplusplus
 }
 #endif

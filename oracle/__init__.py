@@ -41,6 +41,8 @@ def _load():
         lib = C.CDLL(build())
         lib.oracle_create.restype = C.c_void_p
         lib.oracle_create.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]
+        lib.oracle_create_window.restype = C.c_void_p
+        lib.oracle_create_window.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p] + [C.c_int32] * 4
         lib.oracle_create_uv.restype = C.c_void_p
         lib.oracle_create_uv.argtypes = [C.c_void_p] * 5 + [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
         lib.oracle_free.argtypes = [C.c_void_p]
@@ -84,7 +86,8 @@ class Raster:
         self.P = W * H
 
     @classmethod
-    def from_points(cls, pos, opacity, feat, cam) -> "Raster":
+    def from_points(cls, pos, opacity, feat, cam, window=None) -> "Raster":
+        """window = (x0, y0, x1, y1): only pixels in [x0,x1) x [y0,y1) are bucketed (others stay empty)."""
         lib = _load()
         pos = np.ascontiguousarray(pos, dtype=np.float32).reshape(-1, 3)
         opacity = np.ascontiguousarray(opacity, dtype=np.float32).reshape(-1)
@@ -92,7 +95,10 @@ class Raster:
         N, D = pos.shape[0], (feat.shape[1] if feat.ndim == 2 else 0)
         assert opacity.shape[0] == N and feat.shape[0] == N
         cs = _cam_struct(cam)
-        h = lib.oracle_create(_p(pos), _p(opacity), _p(feat), N, D, C.byref(cs))
+        if window is None:
+            h = lib.oracle_create(_p(pos), _p(opacity), _p(feat), N, D, C.byref(cs))
+        else:
+            h = lib.oracle_create_window(_p(pos), _p(opacity), _p(feat), N, D, C.byref(cs), *[int(x) for x in window])
         return cls(h, N, D, int(cam.width), int(cam.height))
 
     @classmethod

@@ -58,6 +58,10 @@ struct State {
     int64_t kept = 0;                        // points that passed the depth / finiteness / range cull
     int64_t border_dropped = 0;              // fragments of kept points that fell outside the image
     bool blended = false;
+    // Optional pixel window [wx0,wx1) x [wy0,wy1): fragments of in-image pixels OUTSIDE it are not
+    // bucketed (their pixels stay empty).  Lets full-size parity tests evaluate sampled pixels one
+    // window at a time without holding every bucket.  Default = whole image.
+    long wx0 = 0, wy0 = 0, wx1 = 1L << 40, wy1 = 1L << 40;
 };
 
 // S2: the (up to) four fragments of one projected point.  fu = u - 0.5, fv = v - 0.5 and
@@ -70,6 +74,7 @@ void emit(State& s, double fu, double fv, double x0, double y0, uint32_t depth_b
         for (int dx = 0; dx < 2; ++dx) {
             const long px = (long)x0 + dx, py = (long)y0 + dy;
             if (px < 0 || px >= s.W || py < 0 || py >= s.H) { s.border_dropped++; continue; }
+            if (px < s.wx0 || px >= s.wx1 || py < s.wy0 || py >= s.wy1) continue;   // outside the test window
             const double wx = dx ? tx : 1.0 - tx;
             const double wy = dy ? ty : 1.0 - ty;
             Frag f;
@@ -109,9 +114,10 @@ extern "C" {
 // S1 + S2 + S3 from world-space points.  The projection is the canonical fp32 sequence:
 // every operation below is one IEEE fp32 operation, in this order, never fused.
 // Follows Eq. 6 with the pinhole divide (reading A2), near/far of PAPER.md:310.
-void* oracle_create(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
-                    const Camera* cam) {
+void* oracle_create_window(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                           const Camera* cam, int32_t wx0, int32_t wy0, int32_t wx1, int32_t wy1) {
     State* s = new_state(N, D, cam->width, cam->height, opacity, feat);
+    if (wx1 > wx0 && wy1 > wy0) { s->wx0 = wx0; s->wy0 = wy0; s->wx1 = wx1; s->wy1 = wy1; }
     const float* R = cam->R;
     const float Wm1 = (float)(cam->width - 1), Hm1 = (float)(cam->height - 1);
     for (int64_t i = 0; i < N; ++i) {
@@ -133,6 +139,11 @@ void* oracle_create(const float* pos, const float* opacity, const float* feat, i
     }
     sort_buckets(*s);
     return s;
+}
+
+void* oracle_create(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                    const Camera* cam) {
+    return oracle_create_window(pos, opacity, feat, N, D, cam, 0, 0, 0, 0);   // whole image
 }
 
 // Same pipeline from already-projected image coordinates in fp64 (no camera, no cull except the

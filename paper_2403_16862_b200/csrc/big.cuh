@@ -26,7 +26,7 @@ struct BigArgs {
     const float4* rec;
     const float* rop;
     unsigned long long* bigkeys;
-    float* bigtin;
+    double* bigtin;
     int W, H;
     float* out_feat;
     float* out_alpha;
@@ -46,6 +46,17 @@ __device__ __forceinline__ bool big_less(unsigned long long a, unsigned long lon
     const uint32_t ia = __float_as_uint(__ldg(&rec[(size_t)(((uint32_t)a) >> 2) * RV]).y);
     const uint32_t ib = __float_as_uint(__ldg(&rec[(size_t)(((uint32_t)b) >> 2) * RV]).y);
     return ia < ib;
+}
+
+// Long runs carry the transmittance and the backward recurrence in fp64: an fp32 product of tens of
+// thousands of (1 - a) factors drifts past the 1e-5 gradient floor.
+__device__ __forceinline__ double warp_incl_prod_d(double v, int lane) {
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const double t = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v *= t;
+    }
+    return v;
 }
 
 // merge stages j = j0, j0/2, ..., 1 of the all-ascending network on s[0..m) (m <= kBigChunk)
@@ -99,7 +110,7 @@ __global__ void __launch_bounds__(kBigThreads) k_big(BigArgs A) {
         const uint32_t n = e.n;
         const int y = e.pix / W, x = e.pix - y * W;
         unsigned long long* keys = A.bigkeys + e.start;
-        float* tin = A.bigtin + e.tin_base;
+        double* tin = A.bigtin + e.tin_base;
 
         if (MODE != kBwd) {
             const uint32_t c0 = (uint32_t)y * (W + 1) + x, c1 = c0 + (W + 1);
@@ -195,20 +206,20 @@ __global__ void __launch_bounds__(kBigThreads) k_big(BigArgs A) {
             float acc[D]; float accA = 0.f;
 #pragma unroll
             for (int d = 0; d < D; ++d) acc[d] = 0.f;
-            float T_in = 1.f;
+            double T_in = 1.0;
             uint32_t nchunk_blended = 0;
             for (uint32_t cb = 0; cb < n; cb += 32) {
-                if (T_in < kTMin) break;
+                if (T_in < (double)kTMin) break;
                 if (lane == 0) tin[cb >> 5] = T_in;
                 nchunk_blended = (cb >> 5) + 1;
                 uint32_t g, corner; float a, op; float4 k4;
                 const bool valid = fetch(cb, g, corner, a, op, k4);
-                const float incl = warp_incl_prod(1.f - a, lane);
-                float excl = __shfl_up_sync(0xffffffffu, incl, 1);
-                if (lane == 0) excl = 1.f;
-                const float T = T_in * excl;
-                if (valid && T >= kTMin) {
-                    const float c = T * a;
+                const double incl = warp_incl_prod_d(1.0 - (double)a, lane);
+                double excl = __shfl_up_sync(0xffffffffu, incl, 1);
+                if (lane == 0) excl = 1.0;
+                const double T = T_in * excl;
+                if (valid && T >= (double)kTMin) {
+                    const float c = (float)(T * (double)a);
                     accA += c;
 #pragma unroll
                     for (int v = 0; v < D / 4; ++v) {
@@ -244,16 +255,16 @@ __global__ void __launch_bounds__(kBigThreads) k_big(BigArgs A) {
                 gf[4 * v] = t.x; gf[4 * v + 1] = t.y; gf[4 * v + 2] = t.z; gf[4 * v + 3] = t.w;
             }
             const float gA = A.g_alpha ? __ldg(A.g_alpha + pix) : 0.f;
-            float B_in = 0.f;
+            double B_in = 0.0;
             for (int c = (int)e.nb - 1; c >= 0; --c) {
-                const float Tc = __ldcg(&tin[c]);
+                const double Tc = __ldcg(&tin[c]);
                 uint32_t g, corner; float a, op; float4 k4;
                 const bool valid = fetch((uint32_t)c << 5, g, corner, a, op, k4);
-                const float incl = warp_incl_prod(1.f - a, lane);
-                float excl = __shfl_up_sync(0xffffffffu, incl, 1);
-                if (lane == 0) excl = 1.f;
-                const float T = Tc * excl;
-                const bool bl = valid && T >= kTMin;
+                const double incl = warp_incl_prod_d(1.0 - (double)a, lane);
+                double excl = __shfl_up_sync(0xffffffffu, incl, 1);
+                if (lane == 0) excl = 1.0;
+                const double T = Tc * excl;
+                const bool bl = valid && T >= (double)kTMin;
                 float G = gA;
                 if (bl) {
 #pragma unroll
@@ -262,17 +273,17 @@ __global__ void __launch_bounds__(kBigThreads) k_big(BigArgs A) {
                         G += f.x * gf[4 * v] + f.y * gf[4 * v + 1] + f.z * gf[4 * v + 2] + f.w * gf[4 * v + 3];
                     }
                 }
-                float M = bl ? 1.f - a : 1.f, C = bl ? a * G : 0.f;
+                double M = bl ? 1.0 - (double)a : 1.0, C = bl ? (double)a * (double)G : 0.0;
 #pragma unroll
                 for (int d = 1; d < 32; d <<= 1) {
-                    const float M2 = __shfl_down_sync(0xffffffffu, M, d);
-                    const float C2 = __shfl_down_sync(0xffffffffu, C, d);
+                    const double M2 = __shfl_down_sync(0xffffffffu, M, d);
+                    const double C2 = __shfl_down_sync(0xffffffffu, C, d);
                     if (lane + d < 32) { C = C + M * C2; M = M * M2; }
                 }
-                const float Mn = __shfl_down_sync(0xffffffffu, M, 1), Cn = __shfl_down_sync(0xffffffffu, C, 1);
-                const float B = lane < 31 ? Cn + Mn * B_in : B_in;
+                const double Mn = __shfl_down_sync(0xffffffffu, M, 1), Cn = __shfl_down_sync(0xffffffffu, C, 1);
+                const double B = lane < 31 ? Cn + Mn * B_in : B_in;
                 if (bl) {
-                    const float Ta = T * a, dLda = T * (G - B);
+                    const float Ta = (float)(T * (double)a), dLda = (float)(T * ((double)G - B));
                     const uint32_t idx = __float_as_uint(k4.y);
                     const int dx = corner & 1, dy = corner >> 1;
                     const float wx = dx ? k4.z : 1.f - k4.z, wy = dy ? k4.w : 1.f - k4.w;

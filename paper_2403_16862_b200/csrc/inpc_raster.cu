@@ -10,6 +10,7 @@
 #include <mutex>
 #include <string>
 #include <unordered_map>
+#include <vector>
 
 #include "bin.cuh"
 #include "big.cuh"
@@ -20,6 +21,42 @@ namespace inpc {
 
 static thread_local std::string t_cuda_error;
 static std::atomic<uint64_t> g_launches{0};
+
+// ---- optional per-stage device timing (inpc_raster_set_kernel_timing) ---------------------------------
+// Every stage the library enqueues is bracketed by two cudaEvents on the caller's stream; the
+// elapsed times are summed per stage when inpc_raster_get_kernel_times is called.  Off by default.
+enum Stage { kStZeroFwd = 0, kStProjectCount, kStScan, kStScatter, kStClassify, kStBuildItems, kStBigFwd, kStTileFwd,
+             kStZeroBwd, kStTileBwd, kStBigBwd, kStOther, kNumStages };
+static const char* const kStageNames[kNumStages] = {
+    "zero_fwd", "k_project_count", "k_scan_u32", "k_scatter", "k_classify_pixels", "k_build_items", "k_big_fwd", "k_tile_fwd",
+    "zero_bwd", "k_tile_bwd", "k_big_bwd", "other"};
+struct Pending { int stage; cudaEvent_t a, b; };
+static std::mutex g_tmu;
+static bool g_timing = false;
+static std::vector<Pending> g_pending;
+static std::vector<cudaEvent_t> g_event_pool;
+static double g_stage_ms[kNumStages];
+static uint64_t g_stage_n[kNumStages];
+
+static cudaEvent_t take_event() {
+    if (!g_event_pool.empty()) { cudaEvent_t e = g_event_pool.back(); g_event_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+struct StageTimer {                       // RAII: start event now, stop event at scope exit
+    bool on; int stage; cudaStream_t st; cudaEvent_t a = nullptr;
+    StageTimer(int stage_, cudaStream_t st_) : on(g_timing), stage(stage_), st(st_) {
+        if (on) { std::lock_guard<std::mutex> lk(g_tmu); a = take_event(); if (a) cudaEventRecord(a, st); }
+    }
+    ~StageTimer() {
+        if (on && a) {
+            std::lock_guard<std::mutex> lk(g_tmu);
+            cudaEvent_t b = take_event();
+            if (b) { cudaEventRecord(b, st); g_pending.push_back(Pending{stage, a, b}); }
+        }
+    }
+};
 
 struct Layout {
     size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
@@ -52,7 +89,7 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     L.items = o;   o = align_up(o + ((size_t)L.P + nbase + 16) * 4);
     L.big = o;     o = align_up(o + ((size_t)L.max_big + 1) * sizeof(BigEntry));
     L.bigkeys = o; o = align_up(o + (four_n + 8) * 8);
-    L.bigtin = o;  o = align_up(o + (four_n / 32 + L.max_big + 8) * 4);
+    L.bigtin = o;  o = align_up(o + (four_n / 32 + L.max_big + 8) * 8);
     if (flags & INPC_SAVE_SORTED) {
         L.pixoff = o;       o = align_up(o + ((size_t)L.P + 1) * 4);
         L.sorted_idx = o;   o = align_up(o + (four_n + 8) * 4);
@@ -128,7 +165,8 @@ static int launch_tile(const TileArgs& A, int sms, cudaStream_t st) {
         if (rc != INPC_OK) return rc;
         configured = true;
     }
-    k_tile<D, MODE><<<grid, kTileThreads, smem, st>>>(A);
+    { StageTimer tm(MODE == kBwd ? kStTileBwd : kStTileFwd, st);
+      k_tile<D, MODE><<<grid, kTileThreads, smem, st>>>(A); }
     INPC_LAUNCHED();
     return INPC_OK;
 }
@@ -146,7 +184,8 @@ static int launch_big(const BigArgs& A, int sms, uint32_t max_big, cudaStream_t 
         configured = true;
     }
     const int g = (int)std::min<uint32_t>((uint32_t)grid, std::max<uint32_t>(max_big, 1u));
-    k_big<D, MODE><<<g, kBigThreads, smem, st>>>(A);
+    { StageTimer tm(MODE == kBwd ? kStBigBwd : kStBigFwd, st);
+      k_big<D, MODE><<<g, kBigThreads, smem, st>>>(A); }
     INPC_LAUNCHED();
     return INPC_OK;
 }
@@ -173,37 +212,44 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     const bool dump = (flags & INPC_SAVE_SORTED) != 0;
     uint32_t* pixoff = dump ? reinterpret_cast<uint32_t*>(ws + L.pixoff) : nullptr;
 
-    INPC_CUDA(cudaMemsetAsync(ws + L.header, 0, L.zero_end - L.header, st));
-    k_write_header<<<1, 1, 0, st>>>(hdr, flags, W, H, D, (uint32_t)N);
+    { StageTimer tm(kStZeroFwd, st);
+      INPC_CUDA(cudaMemsetAsync(ws + L.header, 0, L.zero_end - L.header, st));
+      k_write_header<<<1, 1, 0, st>>>(hdr, flags, W, H, D, (uint32_t)N); }
     INPC_LAUNCHED();
     if (N > 0) {
         const int grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
-        k_project_count<<<grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, rank);
+        { StageTimer tm(kStProjectCount, st);
+          k_project_count<<<grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, rank); }
         INPC_LAUNCHED();
     }
-    k_scan_u32<<<(L.C + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
-        cellcnt, L.C, reinterpret_cast<unsigned long long*>(ws + L.status0), &hdr->scan_tile_counter, &hdr->nrec);
+    { StageTimer tm(kStScan, st);
+      k_scan_u32<<<(L.C + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
+          cellcnt, L.C, reinterpret_cast<unsigned long long*>(ws + L.status0), &hdr->scan_tile_counter, &hdr->nrec); }
     INPC_LAUNCHED();
     if (N > 0) {
         const int grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
-        k_scatter<D><<<grid, kBinThreads, 0, st>>>(pos, opacity, feat, (long long)N, camk, cellcnt, rank, rec, rop);
+        { StageTimer tm(kStScatter, st);
+          k_scatter<D><<<grid, kBinThreads, 0, st>>>(pos, opacity, feat, (long long)N, camk, cellcnt, rank, rec, rop); }
         INPC_LAUNCHED();
     }
-    k_classify_pixels<<<(L.P + 255) / 256, 256, 0, st>>>(cellcnt, W, H, hdr, big, pixoff);
+    { StageTimer tm(kStClassify, st);
+      k_classify_pixels<<<(L.P + 255) / 256, 256, 0, st>>>(cellcnt, W, H, hdr, big, pixoff); }
     INPC_LAUNCHED();
     if (dump) {
-        k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
-            pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr);
+        { StageTimer tm(kStOther, st);
+          k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
+              pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr); }
         INPC_LAUNCHED();
     }
     const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
-    k_build_items<<<(ntx * nty + 127) / 128, 128, 0, st>>>(cellcnt, W, H, TileCfg<D>::kCap, hdr, items);
+    { StageTimer tm(kStBuildItems, st);
+      k_build_items<<<(ntx * nty + 127) / 128, 128, 0, st>>>(cellcnt, W, H, TileCfg<D>::kCap, hdr, items); }
     INPC_LAUNCHED();
 
     BigArgs B{};
     B.hdr = hdr; B.big_cursor = &hdr->big_cursor; B.big = big; B.celloff = cellcnt; B.rec = rec; B.rop = rop;
     B.bigkeys = reinterpret_cast<unsigned long long*>(ws + L.bigkeys);
-    B.bigtin = reinterpret_cast<float*>(ws + L.bigtin);
+    B.bigtin = reinterpret_cast<double*>(ws + L.bigtin);
     B.W = W; B.H = H; B.out_feat = out_feat; B.out_alpha = out_alpha;
     TileArgs A{};
     A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = items; A.celloff = cellcnt; A.rec = rec; A.rop = rop;
@@ -229,12 +275,15 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     if (!di.ok) return cuda_fail(cudaErrorNoDevice);
     const int W = cam->width, H = cam->height;
     Header* hdr = reinterpret_cast<Header*>(ws + L.header);
-    if (N > 0) {
-        INPC_CUDA(cudaMemsetAsync(d_feat, 0, (size_t)N * D * 4, st));
-        INPC_CUDA(cudaMemsetAsync(d_opacity, 0, (size_t)N * 4, st));
-        INPC_CUDA(cudaMemsetAsync(d_uv, 0, (size_t)N * 8, st));
+    {
+        StageTimer tm(kStZeroBwd, st);
+        if (N > 0) {
+            INPC_CUDA(cudaMemsetAsync(d_feat, 0, (size_t)N * D * 4, st));
+            INPC_CUDA(cudaMemsetAsync(d_opacity, 0, (size_t)N * 4, st));
+            INPC_CUDA(cudaMemsetAsync(d_uv, 0, (size_t)N * 8, st));
+        }
+        INPC_CUDA(cudaMemsetAsync(&hdr->item_cursor, 0, 8, st));     // item_cursor + big_cursor
     }
-    INPC_CUDA(cudaMemsetAsync(&hdr->item_cursor, 0, 8, st));     // item_cursor + big_cursor
     TileArgs A{};
     A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = reinterpret_cast<uint32_t*>(ws + L.items);
     A.celloff = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
@@ -247,7 +296,7 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
         B.hdr = hdr; B.big_cursor = &hdr->big_cursor; B.big = reinterpret_cast<BigEntry*>(ws + L.big);
         B.celloff = A.celloff; B.rec = A.rec; B.rop = A.rop;
         B.bigkeys = reinterpret_cast<unsigned long long*>(ws + L.bigkeys);
-        B.bigtin = reinterpret_cast<float*>(ws + L.bigtin);
+        B.bigtin = reinterpret_cast<double*>(ws + L.bigtin);
         B.W = W; B.H = H; B.g_feat = g_feat; B.g_alpha = g_alpha; B.d_feat = d_feat; B.d_opacity = d_opacity; B.d_uv = d_uv;
         rc = launch_big<D, kBwd>(B, di.sms, L.max_big, st);
     }
@@ -299,7 +348,8 @@ int inpc_raster_backward(const float* pos, const float* opacity, const float* fe
     (void)pos; (void)opacity; (void)feat;   // the records saved by the forward hold what the backward needs
     int rc = check_common(N, D, cam);
     if (rc != INPC_OK) return rc;
-    if (!grad_out_feat || !grad_feat || !grad_opacity || !grad_uv || !workspace) return INPC_ERR_INVALID_ARG;
+    if (!grad_out_feat || !workspace) return INPC_ERR_INVALID_ARG;
+    if (N > 0 && (!grad_feat || !grad_opacity || !grad_uv)) return INPC_ERR_INVALID_ARG;
     if (!aligned16(grad_out_feat) || !aligned16(grad_out_alpha) || !aligned16(grad_feat) || !aligned16(grad_opacity) ||
         !aligned16(grad_uv))
         return INPC_ERR_INVALID_ARG;
@@ -397,6 +447,37 @@ const char* inpc_raster_strerror(int status) {
         case INPC_ERR_UNSUPPORTED: return "unsupported D or image size";
         default: return "unknown status";
     }
+}
+
+int inpc_raster_set_kernel_timing(int enable) {
+    std::lock_guard<std::mutex> lk(g_tmu);
+    g_timing = enable != 0;
+    return INPC_OK;
+}
+
+int inpc_raster_kernel_count(void) { return kNumStages; }
+
+const char* inpc_raster_kernel_name(int i) { return (i >= 0 && i < kNumStages) ? kStageNames[i] : ""; }
+
+int inpc_raster_get_kernel_times(double* ms, uint64_t* launches, int reset) {
+    if (!ms || !launches) return INPC_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lk(g_tmu);
+    for (const Pending& p : g_pending) {
+        cudaError_t e = cudaEventSynchronize(p.b);
+        float t = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, p.a, p.b);
+        if (e != cudaSuccess) { g_pending.clear(); return cuda_fail(e); }
+        g_stage_ms[p.stage] += (double)t;
+        g_stage_n[p.stage] += 1;
+        g_event_pool.push_back(p.a);
+        g_event_pool.push_back(p.b);
+    }
+    g_pending.clear();
+    for (int i = 0; i < kNumStages; ++i) {
+        ms[i] = g_stage_ms[i]; launches[i] = g_stage_n[i];
+        if (reset) { g_stage_ms[i] = 0.0; g_stage_n[i] = 0; }
+    }
+    return INPC_OK;
 }
 
 const char* inpc_raster_last_cuda_error(void) { return t_cuda_error.c_str(); }

@@ -21,6 +21,8 @@ EXPORTS = (
     "inpc_raster_workspace_bytes", "inpc_raster_forward", "inpc_raster_backward",
     "inpc_raster_get_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
     "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count",
+    "inpc_raster_set_kernel_timing", "inpc_raster_kernel_count", "inpc_raster_kernel_name",
+    "inpc_raster_get_kernel_times",
 )
 
 
@@ -74,6 +76,10 @@ def load() -> C.CDLL:
         lib.inpc_raster_strerror.argtypes = [C.c_int]
         lib.inpc_raster_last_cuda_error.restype = C.c_char_p
         lib.inpc_raster_launch_count.restype = C.c_uint64
+        lib.inpc_raster_set_kernel_timing.argtypes = [C.c_int]
+        lib.inpc_raster_kernel_name.restype = C.c_char_p
+        lib.inpc_raster_kernel_name.argtypes = [C.c_int]
+        lib.inpc_raster_get_kernel_times.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_uint64), C.c_int]
         _lib = lib
     return _lib
 
@@ -200,3 +206,19 @@ def inpc_raster_get_stats(workspace, stream=None) -> dict:
 
 def inpc_raster_launch_count() -> int:
     return int(load().inpc_raster_launch_count())
+
+
+def inpc_raster_set_kernel_timing(enable: bool) -> None:
+    load().inpc_raster_set_kernel_timing(1 if enable else 0)
+
+
+def inpc_raster_get_kernel_times(reset: bool = True) -> dict:
+    """-> {stage name: (summed device ms, timed launches)} since the last reset (waits for the events)."""
+    lib = load()
+    n = lib.inpc_raster_kernel_count()
+    ms = (C.c_double * n)()
+    cnt = (C.c_uint64 * n)()
+    rc = lib.inpc_raster_get_kernel_times(ms, cnt, 1 if reset else 0)
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_get_kernel_times")
+    return {lib.inpc_raster_kernel_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(n)}

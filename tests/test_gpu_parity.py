@@ -1,0 +1,227 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C ABI, against the oracle.
+
+Sizes: whole-image element-by-element parity where the oracle finishes in seconds (Tiny, 1M, and
+reduced draws of the octree / cluster samplers that still span many tiles, ragged tile edges and
+the long-run path); at BASELINE.json's full sizes (8M / 16M / 33M) whole-image counts + sampled
+pixel windows the oracle evaluates one by one (tests/test_gpu_fullsize.py).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2403_16862_b200 import raster
+from paper_2403_16862_b200.workloads import Camera, Workload, make_workload, second_pose
+
+from harness import (check_backward, check_counts_and_order, check_forward, full_parity, gpu_backward,
+                     gpu_forward)
+
+pytestmark = pytest.mark.gpu
+
+TINY = dict(fx=64.0, fy=64.0, cx=32.0, cy=32.0, width=64, height=64)
+
+
+def _wl(pos, op, feat, cam, seed=0, name="custom"):
+    pos = np.ascontiguousarray(pos, np.float32).reshape(-1, 3)
+    n = pos.shape[0]
+    feat = np.ascontiguousarray(feat, np.float32).reshape(n, -1)
+    rng = np.random.Generator(np.random.PCG64(seed + 1000))
+    g_img = rng.standard_normal((cam.height, cam.width, feat.shape[1])).astype(np.float32)
+    g_alpha = rng.standard_normal((cam.height, cam.width)).astype(np.float32)
+    return Workload(name, pos, np.ascontiguousarray(op, np.float32).reshape(n), feat, cam, g_img, g_alpha, True, seed)
+
+
+# ------------------------------------------------------------------------------ BASELINE configs
+
+def test_tiny_full_parity():
+    rep = full_parity(make_workload("tiny"))
+    assert rep["stats"]["n_fragments"] > 4 * 4096 * 0.9
+
+
+def test_tiny_second_pose_and_no_alpha_grad():
+    wl = make_workload("tiny")
+    R, t = second_pose()
+    wl.cam = wl.cam.with_pose(R, t)
+    full_parity(wl, g_alpha=False)
+
+
+def test_tiny_d8():
+    full_parity(make_workload("tiny", D=8))
+
+
+def test_1m_full_parity():
+    rep = full_parity(make_workload("1m"))
+    assert rep["stats"]["n_kept"] == 1 << 20
+
+
+def test_1m_second_pose():
+    wl = make_workload("1m", n_points=1 << 18)
+    R, t = second_pose()
+    wl.cam = wl.cam.with_pose(R, t)
+    full_parity(wl)
+
+
+def test_train_sampler_reduced():
+    # octree sampler, 1M draws: same camera / structure as config 3, deep enough to split tiles
+    rep = full_parity(make_workload("train", n_points=1 << 20))
+    assert rep["stats"]["n_tile_items"] > 0
+
+
+def test_infer_sampler_reduced_d8():
+    full_parity(make_workload("infer", n_points=1 << 20), backward=False)
+
+
+def test_infer_sampler_reduced_d8_backward():
+    full_parity(make_workload("infer", n_points=1 << 18, D=8), backward=True)
+
+
+def test_stress_sampler_reduced_hits_long_run_path():
+    rep = full_parity(make_workload("stress", n_points=1 << 20))
+    assert rep["stats"]["n_big_pixels"] > 0, "the reduced stress draw must exercise the long-run path"
+
+
+# ------------------------------------------------------------------------------ edge cases
+
+def test_empty_input_gives_zero_image():
+    cam = Camera(**TINY)
+    pos = torch.zeros((0, 3), device="cuda"); op = torch.zeros((0,), device="cuda"); feat = torch.zeros((0, 4), device="cuda")
+    img, alpha, ws = raster.inpc_raster_forward(pos, op, feat, cam)
+    torch.cuda.synchronize()
+    assert img.shape == (64, 64, 4) and float(img.abs().max()) == 0.0 and float(alpha.abs().max()) == 0.0
+    assert int(raster.inpc_raster_get_counts(ws, 64, 64).sum()) == 0
+    g = torch.ones((64, 64, 4), device="cuda")
+    d_feat, d_op, d_uv = raster.inpc_raster_backward(pos, op, feat, cam, g, None, ws)
+    torch.cuda.synchronize()
+    assert d_feat.numel() == 0 and d_op.numel() == 0 and d_uv.numel() == 0
+
+
+def test_all_points_culled():
+    cam = Camera(**TINY)
+    rng = np.random.Generator(np.random.PCG64(5))
+    pos = rng.uniform(-1, 1, (1000, 3)).astype(np.float32)
+    pos[:500, 2] = -3.0              # behind the camera
+    pos[500:800, 2] = 200.0          # beyond far
+    pos[800:900] = np.nan
+    pos[900:, 0] = 1e6; pos[900:, 2] = 1.0     # far outside the image
+    wl = _wl(pos, rng.uniform(0, 1, 1000), rng.uniform(0, 1, (1000, 4)), cam)
+    rep = full_parity(wl)
+    assert rep["stats"]["n_fragments"] == 0 and rep["stats"]["n_kept"] == 0
+
+
+def test_forced_depth_ties_and_duplicates():
+    cam = Camera(**TINY)
+    rng = np.random.Generator(np.random.PCG64(6))
+    base = np.stack([rng.uniform(-0.9, 0.9, 64), rng.uniform(-0.9, 0.9, 64), rng.uniform(2, 6, 64)], axis=1)
+    pos = np.repeat(base, 40, axis=0)            # 40 exact duplicates of each point: every key ties 40-fold
+    perm = rng.permutation(len(pos))
+    pos = pos[perm]
+    n = len(pos)
+    full_parity(_wl(pos, rng.uniform(0, 0.3, n), rng.uniform(0, 1, (n, 4)), cam))
+
+
+def test_points_on_pixel_centres_and_borders():
+    cam = Camera(**TINY)
+    rng = np.random.Generator(np.random.PCG64(7))
+    # pixel centres (u = i + 0.5): weights 1,0,0,0 with four counted fragments
+    i = rng.integers(0, 64, 500); j = rng.integers(0, 64, 500)
+    z = rng.uniform(2, 6, 500)
+    centres = np.stack([(i + 0.5 - 32.0) / 64.0 * z, (j + 0.5 - 32.0) / 64.0 * z, z], axis=1)
+    # image border: u in [-0.6, 0.6] and [63.4, 64.6] -> one or two in-image fragments
+    ub = np.concatenate([rng.uniform(-0.6, 0.6, 250), rng.uniform(63.4, 64.6, 250)])
+    vb = rng.uniform(-0.6, 64.6, 500)
+    zb = rng.uniform(2, 6, 500)
+    border = np.stack([(ub - 32.0) / 64.0 * zb, (vb - 32.0) / 64.0 * zb, zb], axis=1)
+    pos = np.concatenate([centres, border, border[:, [1, 0, 2]]], axis=0)
+    n = len(pos)
+    op = rng.uniform(0, 1, n)
+    op[:100] = 1.0                                # opaque points on pixel centres: a = 1 exactly
+    op[100:150] = 0.0
+    full_parity(_wl(pos, op, rng.uniform(0, 1, (n, 4)), cam))
+
+
+def test_one_very_deep_pixel_50k_fragments():
+    cam = Camera(**TINY)
+    rng = np.random.Generator(np.random.PCG64(8))
+    n = 50_000
+    z = rng.uniform(2, 6, n)
+    u = rng.uniform(20.0, 21.0, n); v = rng.uniform(30.0, 31.0, n)      # all inside one 2x2 pixel block
+    pos = np.stack([(u - 32.0) / 64.0 * z, (v - 32.0) / 64.0 * z, z], axis=1)
+    op = rng.uniform(0, 2e-4, n)                  # tiny opacities: nothing is cut off, every fragment is blended
+    rep = full_parity(_wl(pos, op, rng.uniform(0, 1, (n, 4)), cam))
+    assert rep["stats"]["n_big_pixels"] >= 4 and rep["stats"]["n_big_fragments"] > 100_000
+
+
+def test_deep_pixel_with_cutoff():
+    cam = Camera(**TINY)
+    rng = np.random.Generator(np.random.PCG64(9))
+    n = 30_000
+    z = rng.uniform(2, 6, n)
+    u = rng.uniform(10.0, 14.0, n); v = rng.uniform(40.0, 43.0, n)
+    pos = np.stack([(u - 32.0) / 64.0 * z, (v - 32.0) / 64.0 * z, z], axis=1)
+    full_parity(_wl(pos, rng.uniform(0, 0.2, n), rng.uniform(0, 1, (n, 4)), cam))
+
+
+def test_ragged_image_size_not_multiple_of_tile():
+    cam = Camera(fx=50.0, fy=50.0, cx=18.5, cy=11.5, width=37, height=23)
+    rng = np.random.Generator(np.random.PCG64(10))
+    n = 20_000
+    pos = np.stack([rng.uniform(-1.6, 1.6, n), rng.uniform(-1.0, 1.0, n), rng.uniform(1, 5, n)], axis=1)
+    full_parity(_wl(pos, rng.uniform(0, 1, n), rng.uniform(0, 1, (n, 4)), cam))
+
+
+def test_single_pixel_image():
+    cam = Camera(fx=2.0, fy=2.0, cx=0.5, cy=0.5, width=1, height=1)
+    rng = np.random.Generator(np.random.PCG64(11))
+    n = 300
+    pos = np.stack([rng.uniform(-1, 1, n), rng.uniform(-1, 1, n), rng.uniform(1, 5, n)], axis=1)
+    full_parity(_wl(pos, rng.uniform(0, 0.05, n), rng.uniform(0, 1, (n, 4)), cam))
+
+
+# ------------------------------------------------------------------------------ API behaviour
+
+def test_forward_is_repeatable_and_workspace_reusable():
+    wl = make_workload("tiny")
+    st = gpu_forward(wl)
+    img0, a0 = st["img"].clone(), st["alpha"].clone()
+    for _ in range(3):
+        raster.inpc_raster_forward(st["pos"], st["op"], st["feat"], wl.cam, out_feat=st["img"], out_alpha=st["alpha"],
+                                   workspace=st["ws"], flags=raster.SAVE_FOR_BACKWARD | raster.SAVE_SORTED)
+    torch.cuda.synchronize()
+    assert torch.equal(img0, st["img"]) or float((img0 - st["img"]).abs().max()) < 1e-6
+    assert float((a0 - st["alpha"]).abs().max()) < 1e-6
+    g1 = gpu_backward(wl, st)
+    g2 = gpu_backward(wl, st)
+    for a, b in zip(g1, g2):
+        assert float((a - b).abs().max()) < 1e-5
+
+
+def test_error_codes():
+    wl = make_workload("tiny")
+    st = gpu_forward(wl, flags=0)
+    g = torch.zeros((64, 64, 4), device="cuda")
+    with pytest.raises(raster.InpcError) as e:
+        raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g, None, st["ws"])
+    assert e.value.status == -4                    # forward did not save for backward
+    with pytest.raises(raster.InpcError) as e:
+        raster.inpc_raster_get_sorted(st["ws"], 64, 64)
+    assert e.value.status == -4
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(raster.InpcError) as e:
+        raster.inpc_raster_forward(st["pos"], st["op"], st["feat"], wl.cam, workspace=small)
+    assert e.value.status == -2
+    feat3 = torch.zeros((wl.N, 3), device="cuda")
+    with pytest.raises(ValueError):
+        raster.alloc_workspace(wl.N, 3, 64, 64)
+    with pytest.raises(raster.InpcError) as e:
+        raster.inpc_raster_forward(st["pos"], st["op"], feat3, wl.cam, workspace=st["ws"])
+    assert e.value.status == -5
+
+
+def test_launch_counter_counts_kernels():
+    wl = make_workload("tiny")
+    before = raster.inpc_raster_launch_count()
+    st = gpu_forward(wl, flags=raster.SAVE_FOR_BACKWARD)
+    mid = raster.inpc_raster_launch_count()
+    gpu_backward(wl, st)
+    after = raster.inpc_raster_launch_count()
+    assert mid - before >= 5 and after - mid >= 1
