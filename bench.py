@@ -1,0 +1,444 @@
+#!/usr/bin/env python
+"""bench.py -- measurement of the hot path (SURVEY.md section 8d / DESIGN.md section 7).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload train] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path -- inpc_raster_forward + inpc_raster_backward (rows a1..a5)
+-- over one seeded synthetic point cloud.  Default workload: BASELINE.json config 3 ("train":
+2^23 points, 1297x840, D = 4, octree sampler), the one north_star quotes its target on.
+
+One JSON line is printed by rank 0:
+  value            emitted fragments per second over the whole fwd+bwd step, inputs resident in HBM
+                   (all ranks' fragments / max-over-ranks device time of exactly K steps)
+  e2e              the same metric through the C-ABI binding with HOST (pinned) buffers: per step the
+                   inputs are copied host->device and every result device->host inside the timed region
+  roofline         the dominant kernel: algorithmic bytes per launch / its mean launch duration (CUDA
+                   events on the launching stream, recorded by the library around every stage)
+  roofline_step    the whole fwd+bwd step against the same peak (north_star's 50 % target)
+  cpu_baseline     the oracle, as it stands, on the host cores, on a bounded sample (rank 0, N = 1)
+  clocks           nvidia-smi samples taken while the timed regions ran
+
+Multi-GPU: the path does not shard in this build (north_star: one GPU, no collectives) -> REPLICAS ONLY:
+every rank rasterises its own seeded cloud (seed + rank); the only communication is the barrier and
+the max/sum of the timing scalars.  `--impl reference` times the oracle (oracle/, CPU) per step.
+"""
+from __future__ import annotations
+
+import argparse
+import datetime as _dt
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fragments/sec (fwd+bwd step; ms/frame fwd and fwd+bwd beside it)"
+UNIT = "fragments/s"
+L2_BYTES = 126 * 1024 * 1024
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/; the file named in NCU_TRAFFIC_SOURCE).  None until a capture exists for that kernel.
+NCU_TRAFFIC = {}
+NCU_TRAFFIC_SOURCE = None
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic bytes: per fragment / pixel / point figures
+def algorithmic_bytes(n_points: int, n_frag: int, n_pix: int, D: int) -> dict:
+    F = 4 * D
+    a12 = 24 * n_points + 8 * n_frag + 12 * n_pix                       # a1 + a2: project, count, scan, emit
+    a34 = (8 + 4 + F) * n_frag + 4 * (D + 1) * n_pix                    # a3 + a4: sort + blend
+    a5 = (8 + 4 + F + 8) * n_frag + (8 * (D + 1) + 8) * n_pix + (F + 12) * n_points   # a5: backward
+    return {"a1_a2": a12, "a3_a4": a34, "a5": a5, "fwd": a12 + a34, "bwd": a5, "fwd_bwd": a12 + a34 + a5}
+
+
+# which path rows each library stage belongs to (for the per-kernel roofline)
+STAGE_ROWS = {
+    "k_tile_fwd": "a3_a4", "k_big_fwd": "a3_a4",
+    "k_tile_bwd": "a5", "k_big_bwd": "a5", "zero_bwd": "a5",
+    "zero_fwd": "a1_a2", "k_project_count": "a1_a2", "k_scan_u32": "a1_a2", "k_scatter": "a1_a2",
+    "k_classify_pixels": "a1_a2", "k_build_items": "a1_a2",
+}
+
+
+def measured_peak_gbs() -> tuple[float, str]:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# ------------------------------------------------------------------------------------------------
+# aggregation over ranks: time = max, units = sum (tested with gloo, world_size 2, on CPU)
+def aggregate_over_ranks(local_ms: float, local_units: float, device="cpu") -> tuple[float, float]:
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(local_ms), float(local_units)
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def throughput(units: float, ms: float) -> float:
+    return units / (ms * 1e-3) if ms > 0 else 0.0
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks: the profiling recipe's nvidia-smi line, sampled while the timed regions run
+class ClockSampler:
+    FIELDS = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int, period_ms: int = 50):
+        self.path = os.path.join(tempfile.gettempdir(), f"inpc_clocks_{os.getpid()}.csv")
+        self.windows = []
+        self.proc = None
+        try:
+            self.out = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", str(period_ms)],
+                                         stdout=self.out, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def window(self):
+        sampler = self
+
+        class _W:
+            def __enter__(self_w):
+                self_w.t0 = _dt.datetime.now()
+
+            def __exit__(self_w, *exc):
+                sampler.windows.append((self_w.t0, _dt.datetime.now()))
+        return _W()
+
+    def finish(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "note": "nvidia-smi unavailable"}
+        time.sleep(0.12)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.out.close()
+        rows = []
+        with open(self.path) as f:
+            for line in f:
+                parts = [p.strip() for p in line.strip().split(",")]
+                if len(parts) < 9:
+                    continue
+                try:
+                    ts = _dt.datetime.strptime(parts[0], "%Y/%m/%d %H:%M:%S.%f")
+                    rows.append((ts, float(parts[1]), float(parts[2]), float(parts[3]), parts[4:]))
+                except ValueError:
+                    continue
+        try:
+            os.remove(self.path)
+        except OSError:
+            pass
+        inside = [r for r in rows if any(a <= r[0] <= b for a, b in self.windows)]
+        note = "samples inside the timed regions"
+        if not inside:
+            inside, note = rows, "no sample fell inside a timed region; all samples of the run"
+        if not inside:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "note": "no samples"}
+        sm = sorted(r[1] for r in inside)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[4][1 + k].lower().startswith("active") for r in inside)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(r[2] for r in inside), "reasons": reasons,
+                "power_w_max": max(r[3] for r in inside), "samples": len(inside), "note": note}
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle leg (cpu_baseline at N = 1, and --impl reference)
+def oracle_step(wl, n_sample: int) -> tuple[float, int]:
+    """One fwd+bwd of the oracle on the first n_sample points of the workload -> (seconds, fragments)."""
+    import oracle
+    t0 = time.perf_counter()
+    ref = oracle.Raster.from_points(wl.pos[:n_sample], wl.opacity[:n_sample], wl.feat[:n_sample], wl.cam)
+    ref.blend()
+    ref.backward(wl.g_img, wl.g_alpha)
+    dt = time.perf_counter() - t0
+    frags = ref.total
+    del ref
+    return dt, frags
+
+
+def oracle_sample_size(wl, seconds_per_step: float) -> int:
+    """Largest power-of-two prefix of the workload the oracle is expected to finish in the budget
+    (calibrated on a 2^17-point prefix)."""
+    n_cal = min(wl.N, 1 << 17)
+    dt, _ = oracle_step(wl, n_cal)
+    rate = n_cal / max(dt, 1e-6)
+    n = int(min(wl.N, rate * seconds_per_step))
+    p = 1 << 12
+    while p * 2 <= n:
+        p *= 2
+    return min(p, wl.N)
+
+
+def cpu_baseline(wl, budget_s: float = 15.0) -> dict:
+    n = oracle_sample_size(wl, budget_s)
+    dt, frags = oracle_step(wl, n)
+    return {"value": frags / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"first {n} of {wl.N} points of '{wl.name}' (same camera, full image), one fwd+bwd, "
+                      f"{frags} fragments in {dt:.2f} s; oracle/oracle.cpp is single-threaded fp64",
+            "seconds": dt}
+
+
+def run_reference(args) -> int:
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0                                     # under torchrun only rank 0 runs the oracle
+    from paper_2403_16862_b200.workloads import make_workload
+    wl = make_workload(args.workload)
+    total = max(1, args.steps + args.warmup)
+    n = oracle_sample_size(wl, min(15.0, 150.0 / total))
+    for _ in range(args.warmup):
+        oracle_step(wl, n)
+    secs, frags = 0.0, 0
+    for _ in range(args.steps):
+        dt, fr = oracle_step(wl, n)
+        secs += dt
+        frags += fr
+    value = frags / secs if secs > 0 else 0.0
+    sample = (f"each step = oracle fwd+bwd on the first {n} of {wl.N} points of '{wl.name}' "
+              f"(same camera, full image); single-threaded fp64 CPU")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, args.steps),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(wl, args),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_config(wl, args) -> dict:
+    return {"workload": f"{wl.name}: BASELINE.json config '{args.workload}', N={wl.N} points, "
+                        f"{wl.cam.width}x{wl.cam.height}, D={wl.D}, seed {wl.seed}",
+            "n_points": wl.N, "width": wl.cam.width, "height": wl.cam.height, "D": wl.D,
+            "pass": "forward + backward (grad_feat, grad_opacity, grad_uv)",
+            "parallelism": "replicas only (one cloud per GPU, no data-path collective)",
+            "l2_hygiene": "inputs + records larger than L2 (see l2 key)"}
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args) -> int:
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_2403_16862_b200 import raster           # raises when the CUDA library is missing
+    from paper_2403_16862_b200.workloads import CONFIGS, make_workload
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    raster.load()
+
+    wl = make_workload(args.workload, seed=CONFIGS[args.workload]["seed"] + rank)
+    W, H, D, N = wl.cam.width, wl.cam.height, wl.D, wl.N
+    cam = raster.camera_struct(wl.cam)
+    to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    pos, op, feat = to_dev(wl.pos), to_dev(wl.opacity), to_dev(wl.feat)
+    g_img, g_alpha = to_dev(wl.g_img), to_dev(wl.g_alpha)
+    flags = raster.SAVE_FOR_BACKWARD
+    ws = raster.alloc_workspace(N, D, W, H, flags, dev)
+    img = torch.empty((H, W, D), dtype=torch.float32, device=dev)
+    alpha = torch.empty((H, W), dtype=torch.float32, device=dev)
+    d_feat = torch.empty((N, D), dtype=torch.float32, device=dev)
+    d_op = torch.empty((N,), dtype=torch.float32, device=dev)
+    d_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def fwd(f=flags):
+        raster.inpc_raster_forward(pos, op, feat, cam, out_feat=img, out_alpha=alpha, workspace=ws, flags=f,
+                                   stream=stream)
+
+    def bwd():
+        raster.inpc_raster_backward(pos, op, feat, cam, g_img, g_alpha, ws, grad_feat=d_feat, grad_opacity=d_op,
+                                    grad_uv=d_uv, stream=stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        barrier()
+        return e0.elapsed_time(e1)
+
+    def step():
+        fwd()
+        bwd()
+
+    clocks = ClockSampler(local_rank) if rank == 0 else None
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    stats = raster.inpc_raster_get_stats(ws)
+    n_frag = stats["n_fragments"]
+
+    # ---- the headline: exactly K fwd+bwd steps, device-resident inputs -------------------------------
+    l0 = raster.inpc_raster_launch_count()
+    if clocks:
+        with clocks.window():
+            ms_total = timed(step, args.steps)
+    else:
+        ms_total = timed(step, args.steps)
+    launches = raster.inpc_raster_launch_count() - l0
+    ms_total, units = aggregate_over_ranks(ms_total, float(n_frag) * args.steps, dev)
+    ms_step = ms_total / args.steps
+    value = throughput(units, ms_total)
+
+    # ---- forward only (inference flags) ---------------------------------------------------------------
+    for _ in range(3):
+        fwd(0)
+    if clocks:
+        with clocks.window():
+            ms_fwd_total = timed(lambda: fwd(0), args.steps)
+    else:
+        ms_fwd_total = timed(lambda: fwd(0), args.steps)
+    ms_fwd_total, _ = aggregate_over_ranks(ms_fwd_total, 0.0, dev)
+    ms_fwd = ms_fwd_total / args.steps
+
+    # ---- per-stage device times (library-side CUDA events on the launching stream) --------------------
+    raster.inpc_raster_set_kernel_timing(True)
+    raster.inpc_raster_get_kernel_times(reset=True)
+    if clocks:
+        with clocks.window():
+            ms_staged = timed(step, args.steps)
+    else:
+        ms_staged = timed(step, args.steps)
+    stages = raster.inpc_raster_get_kernel_times(reset=True)
+    raster.inpc_raster_set_kernel_timing(False)
+
+    # ---- end to end: host buffers in, host buffers out, copies inside the timed region ----------------
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_in = [pin(wl.pos), pin(wl.opacity), pin(wl.feat), pin(wl.g_img), pin(wl.g_alpha)]
+    d_in = [pos, op, feat, g_img, g_alpha]
+    d_out = [img, alpha, d_feat, d_op, d_uv]
+    h_out = [torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in d_out]
+    h2d = sum(t.numel() * t.element_size() for t in h_in)
+    d2h = sum(t.numel() * t.element_size() for t in h_out)
+
+    def e2e_step():
+        for h, d in zip(h_in, d_in):
+            d.copy_(h, non_blocking=True)
+        fwd()
+        bwd()
+        for d, h in zip(d_out, h_out):
+            h.copy_(d, non_blocking=True)
+
+    e2e_steps = max(1, min(args.steps, 10))
+    e2e_step()
+    if clocks:
+        with clocks.window():
+            ms_e2e_total = timed(e2e_step, e2e_steps)
+    else:
+        ms_e2e_total = timed(e2e_step, e2e_steps)
+    ms_e2e_total, units_e2e = aggregate_over_ranks(ms_e2e_total, float(n_frag) * e2e_steps, dev)
+    clock_info = clocks.finish() if clocks else None
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline --------------------------------------------------------------------------------------
+    peak, peak_src = measured_peak_gbs()
+    P = W * H
+    alg = algorithmic_bytes(N, n_frag, P, D)
+    per_stage = {k: (ms / n if n else 0.0) for k, (ms, n) in stages.items()}
+    step_stage_ms = {k: ms / args.steps for k, (ms, n) in stages.items() if n}
+    kernels = {k: v for k, v in step_stage_ms.items() if k.startswith("k_")}
+    dom = max(kernels, key=kernels.get)
+    rows = STAGE_ROWS[dom]
+    achieved = alg[rows] / (per_stage[dom] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "rows": rows, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg[rows], "ms_per_launch": per_stage[dom],
+                "share_of_step": kernels[dom] / sum(step_stage_ms.values()),
+                "traffic": NCU_TRAFFIC.get(dom), "traffic_source": NCU_TRAFFIC_SOURCE}
+    ach_step = alg["fwd_bwd"] / (ms_step * 1e-3) / 1e9
+    ach_fwd = alg["fwd"] / (ms_fwd * 1e-3) / 1e9
+    roofline_step = {"bound": "hbm", "algorithmic_bytes_fwd_bwd": alg["fwd_bwd"], "achieved": ach_step,
+                     "peak": peak, "unit": "GB/s", "frac": ach_step / peak, "frac_of_8TBps_nominal": ach_step / 8000.0,
+                     "fwd_only": {"algorithmic_bytes": alg["fwd"], "achieved": ach_fwd, "frac": ach_fwd / peak}}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": workload_config(wl, args),
+        "ms_fwd": ms_fwd, "ms_fwd_bwd": ms_step, "fragments_per_sec_fwd": throughput(float(n_frag) * world, ms_fwd),
+        "fragments_per_step_per_gpu": n_frag, "stats": stats,
+        "e2e": {"value": throughput(units_e2e, ms_e2e_total), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e_total / e2e_steps, "steps": e2e_steps,
+                "how": "pinned host inputs (pos, opacity, feat, grad_out) copied H2D, forward, backward, and "
+                       "img/alpha/grad_feat/grad_opacity/grad_uv copied D2H, every step, on the launch stream"},
+        "gpu_launches": launches,
+        "roofline": roofline, "roofline_step": roofline_step,
+        "stage_ms_per_step": step_stage_ms, "stage_timed_ms_per_step": ms_staged / args.steps,
+        "l2": {"l2_bytes": L2_BYTES, "input_bytes": h2d, "record_bytes": stats["n_kept"] * (20 + 4 * D),
+               "policy": "inputs larger than L2" if h2d > L2_BYTES else "inputs fit L2: numbers are L2-warm"},
+        "clocks": clock_info,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(wl)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None) -> int:
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="train", choices=["tiny", "1m", "train", "infer", "stress"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle leg (profiling runs)")
+    args = ap.parse_args(argv)
+    if args.impl == "reference":
+        return run_reference(args)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and world == 1:
+        # convenience: relaunch under torchrun, one rank per GPU
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 2000), os.path.abspath(__file__)] + \
+              (argv if argv is not None else sys.argv[1:])
+        return subprocess.call(cmd)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
