@@ -48,7 +48,7 @@ typedef struct inpc_camera {
 
 typedef enum inpc_status {
     INPC_OK                      =  0,
-    INPC_ERR_INVALID_ARG         = -1,  /* NULL / misaligned pointer, N < 0, W/H <= 0, near >= far, N >= 2^30 */
+    INPC_ERR_INVALID_ARG         = -1,  /* NULL / misaligned pointer, N < 0, W/H <= 0, near >= far, near < 0, N >= 2^30 */
     INPC_ERR_WORKSPACE_TOO_SMALL = -2,
     INPC_ERR_CUDA                = -3,  /* launch failure or sticky error; see inpc_raster_last_cuda_error   */
     INPC_ERR_NO_SAVED_STATE      = -4,  /* backward / get_* on a workspace no matching forward has filled     */
@@ -64,8 +64,9 @@ typedef struct inpc_stats {          /* host struct filled by inpc_raster_get_st
     uint64_t n_kept;                 /* points that survived the cull (= records binned)                      */
     uint64_t n_fragments;            /* emitted fragments = sum over pixels of count[p]                       */
     uint64_t n_tile_items;           /* screen-tile work items built for the blend kernel                     */
-    uint64_t n_big_pixels;           /* pixels deeper than the in-tile limit, handled by the long-run path    */
+    uint64_t n_big_pixels;           /* pixels whose neighbourhood exceeds a tile, handled by the long-run path */
     uint64_t n_big_fragments;        /* fragments in those pixels                                             */
+    uint64_t n_big_cells;            /* cells too large for the counting sort (bitonic-sorted, one CTA each)  */
 } inpc_stats;
 
 /* Upper bound (for 4N fragments) of the workspace needed for N points; 0 on invalid arguments. */

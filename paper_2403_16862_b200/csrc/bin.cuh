@@ -1,10 +1,10 @@
 // bin.cuh -- steps a1/a2 of the hot path: projection, per-cell counting, device-wide scan, record
-// scatter, per-pixel classification and tile work-list construction.
+// emission, per-pixel counts and tile work-list construction.
 //
 // Path rows (SURVEY.md section 8a / DESIGN.md section 1):
 //   a1  k_project_count + k_scatter : Eq. 6 projection, cull, bilinear cell + fractions (Eq. 7 inputs)
 //   a2  k_project_count (count), k_scan_u32 (device-wide exclusive scan, decoupled look-back),
-//       k_classify_pixels (per-pixel fragment counts = 2x2 box sum of the cell counts)
+//       k_classify (per-pixel fragment counts = 2x2 box sum of the cell counts)
 #pragma once
 #include "common.cuh"
 
@@ -59,15 +59,14 @@ __global__ void __launch_bounds__(kBinThreads) k_project_count(const float* __re
     }
 }
 
-// a1 (emission): re-project (bit-identical), slot = celloff[cell] + rank, write the record once.
-template <int D>
+// a1 (emission): re-project (bit-identical), slot = celloff[cell] + rank, write ONE full 32-byte
+// sector per point: { depth_bits, idx, tx, ty | opacity, cell, 0, 0 }.  (Anything narrower than a
+// sector scattered by slot costs a DRAM read-modify-write: profiles/r01_v1_baseline.md.)
 __global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict__ pos,
-                                                          const float* __restrict__ opacity,
-                                                          const float* __restrict__ feat, long long N, Camera cam,
+                                                          const float* __restrict__ opacity, long long N, Camera cam,
                                                           const uint32_t* __restrict__ celloff,
                                                           const uint32_t* __restrict__ rank,
-                                                          float4* __restrict__ rec, float* __restrict__ rop) {
-    constexpr int RV = 1 + D / 4;                        // float4 per record
+                                                          float4* __restrict__ A) {
     __shared__ __align__(16) float s_pos[kBinChunk * 3];
     for (long long base = (long long)blockIdx.x * kBinChunk; base < N; base += (long long)gridDim.x * kBinChunk) {
         __syncthreads();
@@ -82,17 +81,16 @@ __global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict
             if (r == 0xFFFFFFFFu) continue;
             const Proj p = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]);
             const uint32_t slot = __ldg(&celloff[p.cell]) + r;
-            float4 key;
-            key.x = __uint_as_float(p.depth_bits);
-            key.y = __uint_as_float((uint32_t)i);
-            key.z = p.tx;
-            key.w = p.ty;
-            float4* dst = rec + (size_t)slot * RV;
-            dst[0] = key;
-#pragma unroll
-            for (int q = 0; q < D / 4; ++q)
-                dst[1 + q] = __ldcs(reinterpret_cast<const float4*>(feat + (size_t)i * D) + q);
-            rop[slot] = __ldcs(&opacity[i]);
+            float4 a0, a1;
+            a0.x = __uint_as_float(p.depth_bits);
+            a0.y = __uint_as_float((uint32_t)i);
+            a0.z = p.tx;
+            a0.w = p.ty;
+            a1.x = __ldcs(&opacity[i]);
+            a1.y = __uint_as_float((uint32_t)p.cell);
+            a1.z = 0.f; a1.w = 0.f;
+            A[2 * (size_t)slot] = a0;
+            A[2 * (size_t)slot + 1] = a1;
         }
     }
 }
@@ -199,25 +197,24 @@ __device__ __forceinline__ uint32_t pixel_count(const uint32_t* __restrict__ cel
     return (__ldg(&celloff[c0 + 2]) - __ldg(&celloff[c0])) + (__ldg(&celloff[c1 + 2]) - __ldg(&celloff[c1]));
 }
 
-// One thread per pixel: total fragment count, long-run ("big") pixel list, optional count image.
-__global__ void __launch_bounds__(256) k_classify_pixels(const uint32_t* __restrict__ celloff, int W, int H,
-                                                          Header* __restrict__ hdr, BigEntry* __restrict__ big,
-                                                          uint32_t* __restrict__ pixcnt) {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+// One thread per CELL index c = j (W+1) + i: the fragment count of pixel (i, j) when it is inside the
+// image (total, optional count image) and the list of cells too large for the counting sort.
+__global__ void __launch_bounds__(256) k_classify(const uint32_t* __restrict__ celloff, int W, int H,
+                                                   Header* __restrict__ hdr, BigCell* __restrict__ bigcells,
+                                                   uint32_t* __restrict__ pixcnt) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int C = (W + 1) * (H + 1);
     uint32_t n = 0;
-    if (p < W * H) {
-        const int y = p / W, x = p - y * W;
-        n = pixel_count(celloff, W, x, y);
-        if (pixcnt) pixcnt[p] = n;
-        if (n > (uint32_t)kPixMax) {
-            const unsigned long long old = atomicAdd(&hdr->big_packed, (1ull << 40) | (unsigned long long)n);
-            const uint32_t b = (uint32_t)(old >> 40);
-            const uint32_t start = (uint32_t)(old & ((1ull << 40) - 1));
-            BigEntry e;
-            e.pix = (uint32_t)p; e.n = n; e.start = start; e.nb = 0;
-            e.tin_base = (start >> 5) + b;               // disjoint per-chunk slots (see big.cuh)
-            e.pad[0] = e.pad[1] = e.pad[2] = 0;
-            big[b] = e;
+    if (c < C) {
+        const int j = c / (W + 1), i = c - j * (W + 1);
+        if (i < W && j < H) {
+            n = pixel_count(celloff, W, i, j);
+            if (pixcnt) pixcnt[j * W + i] = n;
+        }
+        const uint32_t a = __ldg(&celloff[c]), m = __ldg(&celloff[c + 1]) - a;
+        if (m > (uint32_t)kCellSmall) {
+            BigCell e; e.cell = (uint32_t)c; e.start = a; e.n = m; e.pad = 0;
+            bigcells[atomicAdd(&hdr->n_big_cells, 1u)] = e;
         }
     }
     // block reduction of n -> one 64-bit atomic per CTA
@@ -241,7 +238,7 @@ __global__ void __launch_bounds__(256) k_counts_out(const uint32_t* __restrict__
 }
 
 // Records a tile item of tw x th pixels at (X, Y) stages into shared memory: each of its th+1 cell
-// rows is one contiguous record range, widened to multiples of 4 records (16-byte bulk copies).
+// rows is one contiguous slot range, widened to multiples of 4 records (16-byte bulk copies of dk).
 __device__ __forceinline__ uint32_t tile_padded_records(const uint32_t* __restrict__ celloff, int W, int H, int X,
                                                         int Y, int tw, int th) {
     uint32_t tot = 0;
@@ -251,21 +248,22 @@ __device__ __forceinline__ uint32_t tile_padded_records(const uint32_t* __restri
         const uint32_t rowbase = (uint32_t)j * (W + 1);
         const uint32_t a = __ldg(&celloff[rowbase + min(X, W + 1)]);
         const uint32_t b = __ldg(&celloff[rowbase + min(X + tw + 1, W + 1)]);
-        tot += ((b + 3u) & ~3u) - (a & ~3u);
+        if (b > a) tot += ((b + 3u) & ~3u) - (a & ~3u);
     }
     return tot;
 }
 
-// One thread per base tile: emit it if its records fit the shared-memory capacity, otherwise split
-// (16x8 -> 8x4 -> 4x2 -> 2x1 -> 1x1).  A 1x1 leaf deeper than kPixMax belongs to the long-run path.
+// One thread per base tile: emit it if its records fit the shared-memory capacity, otherwise halve
+// its larger side and retry.  A sub-tile of kMinTilePix pixels or fewer that still does not fit sends
+// its pixels to the long-run list (they are merged straight from global memory, big.cuh).
 __global__ void __launch_bounds__(128) k_build_items(const uint32_t* __restrict__ celloff, int W, int H, int cap,
-                                                      Header* __restrict__ hdr, uint32_t* __restrict__ items) {
+                                                      Header* __restrict__ hdr, uint32_t* __restrict__ items,
+                                                      uint32_t* __restrict__ bigpix) {
     const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntx * nty) return;
     const int X0 = (t % ntx) * kTileW, Y0 = (t / ntx) * kTileH;
-    // explicit DFS stack: (X, Y, lw, lh); depth <= 5, at most 3 siblings pending per level
-    uint32_t stack[20];
+    uint32_t stack[12];                                  // binary DFS: depth <= 7, one sibling pending per level
     int sp = 0;
     stack[sp++] = encode_item(X0, Y0, kTileLW, kTileLH);
     while (sp > 0) {
@@ -274,20 +272,25 @@ __global__ void __launch_bounds__(128) k_build_items(const uint32_t* __restrict_
         if (X >= W || Y >= H) continue;
         const int tw = 1 << lw, th = 1 << lh;
         const uint32_t n = tile_padded_records(celloff, W, H, X, Y, tw, th);
-        if (lw == 0 && lh == 0) {
-            if (pixel_count(celloff, W, X, Y) <= (uint32_t)kPixMax) items[atomicAdd(&hdr->n_items, 1u)] = it;
-            continue;
-        }
         if (n <= (uint32_t)cap) {
-            items[atomicAdd(&hdr->n_items, 1u)] = it;
+            items[atomicAdd(&hdr->n_items, 1u)] = it;    // empty tiles too: their pixels must be zeroed
             continue;
         }
-        const int nlw = lw > 0 ? lw - 1 : 0, nlh = lh > 0 ? lh - 1 : 0;
-        const int hw = 1 << nlw, hh = 1 << nlh;
-        stack[sp++] = encode_item(X, Y, nlw, nlh);
-        if (lw > 0) stack[sp++] = encode_item(X + hw, Y, nlw, nlh);
-        if (lh > 0) stack[sp++] = encode_item(X, Y + hh, nlw, nlh);
-        if (lw > 0 && lh > 0) stack[sp++] = encode_item(X + hw, Y + hh, nlw, nlh);
+        if (tw * th <= kMinTilePix) {
+            for (int y = Y; y < min(Y + th, H); ++y)
+                for (int x = X; x < min(X + tw, W); ++x) {
+                    bigpix[atomicAdd(&hdr->n_big_pixels, 1u)] = (uint32_t)(y * W + x);
+                    atomicAdd(&hdr->n_big_fragments, (unsigned long long)pixel_count(celloff, W, x, y));
+                }
+            continue;
+        }
+        if (lw >= lh + 1 || lh == 0) {                   // split the wider side (tiles are kept ~2:1)
+            stack[sp++] = encode_item(X + (tw >> 1), Y, lw - 1, lh);
+            stack[sp++] = encode_item(X, Y, lw - 1, lh);
+        } else {
+            stack[sp++] = encode_item(X, Y + (th >> 1), lw, lh - 1);
+            stack[sp++] = encode_item(X, Y, lw, lh - 1);
+        }
     }
 }
 

@@ -3,12 +3,21 @@
 // Data layout in HBM (all inside the caller's workspace):
 //   cell grid   : (W+1) x (H+1) cells; cell (i, j) holds the kept points whose top-left pixel is
 //                 (x0, y0) = (i-1, j-1), x0 = floor(u-0.5).  Pixel (x, y) receives exactly the points of
-//                 cells (x, y), (x+1, y), (x, y+1), (x+1, y+1)  => its fragment run is two contiguous
-//                 record ranges of the cell-sorted record array (cell rows y and y+1).
+//                 cells (x, y), (x+1, y), (x, y+1), (x+1, y+1)  => its fragments are FOUR cell lists, two
+//                 contiguous slot ranges of the cell-ordered arrays (cell rows y and y+1).
 //   celloff[C+1]: exclusive sum of the per-cell point counts (device-wide scan), C = (W+1)(H+1).
-//   rec[nrec]   : cell-sorted point records, RB = 16 + 4*D bytes each:
-//                 { depth_bits, point_idx, tx, ty, feat[0..D) }  (tx = fu - x0, ty = fv - y0, exact)
-//   rop[nrec]   : opacity of each record (separate 4-byte array so that rec stays 16-byte granular).
+//   A[nrec]     : 32-byte emission records in arrival order inside each cell (written by k_scatter):
+//                 { depth_bits, point_idx, tx, ty | opacity, cell, 0, 0 }   (tx = fu - x0, ty = fv - y0, exact)
+//   dk[nrec]    : depth bits, every cell sorted ascending by (depth_bits, point_idx)   (k_cellsort)
+//   R[nrec]     : payload records in the same order, 16 + 4*D bytes: { tx, ty, opacity, point_idx | feat[D] }
+//   Because every cell list is sorted, a pixel's depth-ordered fragment run is the 4-way MERGE of its
+//   four cell lists; no per-pixel sort exists anywhere.
+//   gT[4*nrec]  : transmittance in front of fragment (slot, corner), written by the forward pass
+//   gD[4*nrec]  : dL/da of fragment (slot, corner), written by the backward pass   (gT|gD reuse A's bytes)
+//   pcur[P]     : per pixel, how many records of each of its four lists were blended before the cut-off
+//   gpt[N]      : per-point gradient records (8 or 16 floats), one or two full 32-byte sectors each
+// Corner c = 2*dy + dx is the pixel's offset from the record's top-left pixel; list j of a pixel
+// (0: cell (x,y), 1: (x+1,y), 2: (x,y+1), 3: (x+1,y+1)) holds its fragments of corner 3 - j.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -16,20 +25,21 @@
 namespace inpc {
 
 // ---- tunables -------------------------------------------------------------------------------------
-constexpr int kTileW      = 16;    // base screen tile (pixels); halved alternately down to 1x1
-constexpr int kTileH      = 8;
-constexpr int kTileLW     = 4;     // log2(kTileW)
-constexpr int kTileLH     = 3;     // log2(kTileH)
-constexpr int kTileThreads = 256;
-constexpr int kTileWarps  = kTileThreads / 32;
-constexpr int kPixMax     = 256;   // deepest pixel the tile kernel sorts itself (per-warp smem scratch)
-constexpr int kBigThreads = 512;
-constexpr int kBigChunk   = 8192;  // keys sorted in shared memory at a time by the long-run path
-constexpr float kTMin     = 1e-4f; // transmittance cut-off (BASELINE.json north_star)
+constexpr int kTileW       = 16;    // base screen tile (pixels); halved (larger side first) down to kMinTilePix
+constexpr int kTileH       = 8;
+constexpr int kTileLW      = 4;     // log2(kTileW)
+constexpr int kTileLH      = 3;     // log2(kTileH)
+constexpr int kTileThreads = kTileW * kTileH;   // one thread per pixel
+constexpr int kMinTilePix  = 8;     // a sub-tile this small that still does not fit goes to the long-run path
+constexpr int kCellSmall   = 128;   // cells up to this many points are ranked by counting; larger: bitonic
+constexpr int kBigThreads  = 512;
+constexpr int kBigChunk    = 8192;  // keys sorted in shared memory at a time by the large-cell sort
+constexpr float kTMin      = 1e-4f; // transmittance cut-off (BASELINE.json north_star)
+constexpr uint32_t kSentHi = 0xFFFFFFFFu;   // "list exhausted" for the ascending merge (depth bits < 0x7F800000)
 
 template <int D> struct TileCfg;
-template <> struct TileCfg<4> { static constexpr int kCap = 1600; };   // records per tile item
-template <> struct TileCfg<8> { static constexpr int kCap = 1280; };
+template <> struct TileCfg<4> { static constexpr int kCap = 1344; };   // records per tile item
+template <> struct TileCfg<8> { static constexpr int kCap = 1024; };
 
 struct Camera {
     float fx, fy, cx, cy;
@@ -51,19 +61,17 @@ struct Header {
     uint32_t scan_tile_counter;
     uint32_t pad0;
     unsigned long long n_fragments;
-    unsigned long long big_packed; // (n_big << 40) | n_big_fragments, bumped with one atomic
-    uint32_t pad[16];
+    uint32_t n_big_pixels;         // pixels routed to the long-run path
+    uint32_t n_big_cells;          // cells larger than kCellSmall (bitonic-sorted)
+    unsigned long long n_big_fragments;
+    uint32_t bigcell_cursor;
+    uint32_t bigcell_keys;         // running offset into the large-cell key scratch
+    uint32_t cellsort_cursor;
+    uint32_t pad[11];
 };
 static_assert(sizeof(Header) % 16 == 0, "header alignment");
 
-struct BigEntry {                  // one pixel deeper than kPixMax
-    uint32_t pix;                  // y * W + x
-    uint32_t n;                    // fragments
-    uint32_t start;                // offset of its run in bigkeys
-    uint32_t nb;                   // blended count (written by the forward)
-    uint32_t tin_base;             // offset of its per-chunk incoming transmittances in bigtin
-    uint32_t pad[3];
-};
+struct BigCell { uint32_t cell, start, n, pad; };   // a cell with more than kCellSmall points
 
 constexpr uint32_t kMagic = 0x494E5043u;  // "INPC"
 
@@ -101,16 +109,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
                      smem_u32(dst_smem)),
                  "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
-}
-__device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d)
-                 : "memory");
-}
-__device__ __forceinline__ void red_add_v2(float* addr, float a, float b) {
-    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(a), "f"(b) : "memory");
-}
-__device__ __forceinline__ void red_add(float* addr, float a) {
-    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
 }
 
 // ---- step a1: canonical fp32 projection (Eq. 6; reading R1) ------------

@@ -1,0 +1,112 @@
+// grad.cuh -- the last stage of step a5: "the per-point gradient [is computed] by combining its four splat
+// gradients in a weighted sum according to the ... bilinear interpolation weights".
+//
+//   k_combine  one thread per RECORD (slot order, coalesced): reads the record's four (T, dL/da) pairs
+//              from gT / gD, decides per corner whether that fragment was blended (its position in the
+//              cell list < the pixel's stop position pcur), and forms
+//                 dL/dfeat    = sum_c T_c a_c g_img[pixel_c]            (S5)
+//                 dL/dopacity = sum_c w_c dL/da_c                        (S6)
+//                 dL/d(u, v)  = opacity * sum_c (dw_c/du, dw_c/dv) dL/da_c
+//              and writes them as ONE (D = 4) or TWO (D = 8) full 32-byte sectors to gpt[point_idx]: the
+//              only scattered write of the backward pass, and never narrower than a sector.  No atomics:
+//              every fragment has exactly one writer, so gradients are bit-reproducible run to run.
+//   k_split    one thread per POINT: gpt -> grad_feat[N][D], grad_opacity[N], grad_uv[N][2] (coalesced);
+//              culled points (rank == ~0) get exact zeros.
+#pragma once
+#include "common.cuh"
+
+namespace inpc {
+
+constexpr int kGradThreads = 256;
+constexpr int kGradCells   = 1024;
+
+template <int D> __host__ __device__ constexpr int gpt_floats() { return D == 4 ? 8 : 16; }
+
+template <int D>
+__global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __restrict__ celloff, uint32_t C, int W,
+                                                           int H, const float4* __restrict__ R,
+                                                           const float4* __restrict__ gT, const float4* __restrict__ gD,
+                                                           const uint4* __restrict__ pcur,
+                                                           const float* __restrict__ g_feat, float* __restrict__ gpt) {
+    constexpr int RV = 1 + D / 4;
+    constexpr int GP = gpt_floats<D>();
+    __shared__ uint32_t s_off[kGradCells + 1];
+    const int tid = threadIdx.x;
+    const uint32_t n_units = (C + kGradCells - 1) / kGradCells;
+    for (uint32_t unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+        const uint32_t c0 = unit * kGradCells, nc = min((uint32_t)kGradCells, C - c0);
+        __syncthreads();
+        for (uint32_t c = tid; c <= nc; c += kGradThreads) s_off[c] = __ldg(&celloff[c0 + c]);
+        __syncthreads();
+        const uint32_t S = s_off[0], E = s_off[nc];
+        for (uint32_t slot = S + tid; slot < E; slot += kGradThreads) {
+            // cell of this slot: the last c with s_off[c] <= slot (empty cells repeat offsets)
+            uint32_t lo = 0, hi = nc - 1;
+            while (lo < hi) {
+                const uint32_t mid = (lo + hi + 1) >> 1;
+                if (s_off[mid] <= slot) lo = mid; else hi = mid - 1;
+            }
+            const uint32_t cell = c0 + lo, r = slot - s_off[lo];
+            const int j = cell / (W + 1), i = cell - j * (W + 1);
+            const int x0 = i - 1, y0 = j - 1;
+            const float4 r0 = __ldg(&R[(size_t)slot * RV]);       // tx, ty, opacity, idx
+            const float4 t4 = __ldcs(&gT[slot]), d4 = __ldcs(&gD[slot]);
+            const float tc[4] = {t4.x, t4.y, t4.z, t4.w}, dc[4] = {d4.x, d4.y, d4.z, d4.w};
+            float df[D];
+#pragma unroll
+            for (int d = 0; d < D; ++d) df[d] = 0.f;
+            float dop = 0.f, du = 0.f, dv = 0.f;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int dx = c & 1, dy = c >> 1;
+                const int px = x0 + dx, py = y0 + dy;
+                if (px < 0 || px >= W || py < 0 || py >= H) continue;      // fragment does not exist
+                const size_t pp = (size_t)py * W + px;
+                const uint4 cur = __ldg(&pcur[pp]);
+                const uint32_t lim = c == 3 ? cur.x : (c == 2 ? cur.y : (c == 1 ? cur.z : cur.w));   // list 3 - c
+                if (r >= lim) continue;                                    // behind the cut-off: exactly 0
+                const float wx = dx ? r0.x : 1.f - r0.x, wy = dy ? r0.y : 1.f - r0.y;
+                const float Ta = tc[c] * (r0.z * (wx * wy));
+                const float dl = dc[c];
+                dop += wx * wy * dl;
+                du += (dx ? wy : -wy) * dl;
+                dv += (dy ? wx : -wx) * dl;
+#pragma unroll
+                for (int v = 0; v < D / 4; ++v) {
+                    const float4 t = __ldg(reinterpret_cast<const float4*>(g_feat + pp * D) + v);
+                    df[4 * v] += Ta * t.x; df[4 * v + 1] += Ta * t.y; df[4 * v + 2] += Ta * t.z; df[4 * v + 3] += Ta * t.w;
+                }
+            }
+            du *= r0.z; dv *= r0.z;
+            float4* out = reinterpret_cast<float4*>(gpt + (size_t)__float_as_uint(r0.w) * GP);
+#pragma unroll
+            for (int v = 0; v < D / 4; ++v) out[v] = make_float4(df[4 * v], df[4 * v + 1], df[4 * v + 2], df[4 * v + 3]);
+            out[D / 4] = make_float4(dop, du, dv, 0.f);
+            if (D == 8) out[3] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    }
+}
+
+template <int D>
+__global__ void __launch_bounds__(256) k_split(const float* __restrict__ gpt, const uint32_t* __restrict__ rank,
+                                                long long N, float* __restrict__ d_feat, float* __restrict__ d_opacity,
+                                                float* __restrict__ d_uv) {
+    constexpr int GP = gpt_floats<D>();
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        float4 f[D / 4], o = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int v = 0; v < D / 4; ++v) f[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (__ldcs(&rank[i]) != 0xFFFFFFFFu) {
+            const float4* in = reinterpret_cast<const float4*>(gpt + (size_t)i * GP);
+#pragma unroll
+            for (int v = 0; v < D / 4; ++v) f[v] = __ldcs(&in[v]);
+            o = __ldcs(&in[D / 4]);
+        }
+#pragma unroll
+        for (int v = 0; v < D / 4; ++v) __stcs(reinterpret_cast<float4*>(d_feat + (size_t)i * D) + v, f[v]);
+        __stcs(&d_opacity[i], o.x);
+        __stcs(reinterpret_cast<float2*>(d_uv) + i, make_float2(o.y, o.z));
+    }
+}
+
+}  // namespace inpc

@@ -1,8 +1,8 @@
 // inpc_raster.cu -- C ABI (include/inpc_raster.h) over the sm_100a kernels in bin.cuh / tile.cuh / big.cuh.
 //
-// Forward  = memset | k_project_count | k_scan_u32 | k_scatter | k_classify_pixels | [k_scan_u32] |
-//            k_build_items | k_big<fwd> | k_tile<fwd>           (all on the caller's stream, no sync)
-// Backward = memset x3 | k_tile<bwd> | k_big<bwd>
+// Forward  = memset | k_project_count | k_scan_u32 | k_scatter | k_classify | k_cellsort | k_cellsort_big |
+//            [k_scan_u32] | k_build_items | k_tile<fwd> | k_big<fwd>     (all on the caller's stream, no sync)
+// Backward = k_tile<bwd> | k_big<bwd> | k_combine | k_split
 // No device memory is allocated here; there is no CPU fallback.
 #include "../../include/inpc_raster.h"
 
@@ -14,7 +14,9 @@
 
 #include "bin.cuh"
 #include "big.cuh"
+#include "cellsort.cuh"
 #include "common.cuh"
+#include "grad.cuh"
 #include "tile.cuh"
 
 namespace inpc {
@@ -25,11 +27,11 @@ static std::atomic<uint64_t> g_launches{0};
 // ---- optional per-stage device timing (inpc_raster_set_kernel_timing) ---------------------------------
 // Every stage the library enqueues is bracketed by two cudaEvents on the caller's stream; the
 // elapsed times are summed per stage when inpc_raster_get_kernel_times is called.  Off by default.
-enum Stage { kStZeroFwd = 0, kStProjectCount, kStScan, kStScatter, kStClassify, kStBuildItems, kStBigFwd, kStTileFwd,
-             kStZeroBwd, kStTileBwd, kStBigBwd, kStOther, kNumStages };
+enum Stage { kStZeroFwd = 0, kStProjectCount, kStScan, kStScatter, kStClassify, kStCellSort, kStCellSortBig, kStBuildItems,
+             kStTileFwd, kStBigFwd, kStZeroBwd, kStTileBwd, kStBigBwd, kStCombine, kStSplit, kStOther, kNumStages };
 static const char* const kStageNames[kNumStages] = {
-    "zero_fwd", "k_project_count", "k_scan_u32", "k_scatter", "k_classify_pixels", "k_build_items", "k_big_fwd", "k_tile_fwd",
-    "zero_bwd", "k_tile_bwd", "k_big_bwd", "other"};
+    "zero_fwd", "k_project_count", "k_scan_u32", "k_scatter", "k_classify", "k_cellsort", "k_cellsort_big", "k_build_items",
+    "k_tile_fwd", "k_big_fwd", "zero_bwd", "k_tile_bwd", "k_big_bwd", "k_combine", "k_split", "other"};
 struct Pending { int stage; cudaEvent_t a, b; };
 static std::mutex g_tmu;
 static bool g_timing = false;
@@ -60,10 +62,11 @@ struct StageTimer {                       // RAII: start event now, stop event a
 
 struct Layout {
     size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
-    size_t rank, rec, rop, items, big, bigkeys, bigtin;
+    size_t rank, A, gT, gD, dk, R, items, bigpix, bigcells, bigkeys;
+    size_t pcur, gpt;                                     // only with INPC_SAVE_FOR_BACKWARD
     size_t pixoff, sorted_idx, sorted_depth;              // only with INPC_SAVE_SORTED
     size_t total;
-    uint32_t C, P, max_big, n_status;
+    uint32_t C, P, max_big_cells, n_status;
 };
 
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
@@ -74,8 +77,7 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     L.C = (uint32_t)((W + 1) * (H + 1));
     L.P = (uint32_t)(W * H);
     L.n_status = (uint32_t)((std::max(L.C, L.P) + kScanTile - 1) / kScanTile + 1);
-    const size_t four_n = 4 * n;
-    L.max_big = (uint32_t)std::min<size_t>(L.P, four_n / (kPixMax + 1) + 1);
+    L.max_big_cells = (uint32_t)(n / (kCellSmall + 1) + 1);
     size_t o = 0;
     L.header = o;  o = align_up(o + sizeof(Header));
     L.status0 = o; o = align_up(o + (size_t)L.n_status * 8);
@@ -83,17 +85,23 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     L.cellcnt = o; o = align_up(o + ((size_t)L.C + 1) * 4);
     L.zero_end = o;
     L.rank = o;    o = align_up(o + n * 4 + 16);
-    L.rec = o;     o = align_up(o + (n + 8) * (size_t)(16 + 4 * D));
-    L.rop = o;     o = align_up(o + (n + 8) * 4);
+    L.A = o;       L.gT = o; L.gD = o + (n + 8) * 16;     // the emission records are dead once the cells are sorted:
+    o = align_up(o + (n + 8) * 32);                       // their bytes then hold gT | gD (16 B per record each)
+    L.dk = o;      o = align_up(o + (n + 16) * 4);
+    L.R = o;       o = align_up(o + (n + 8) * (size_t)(16 + 4 * D));
     const size_t nbase = (size_t)((W + kTileW - 1) / kTileW) * ((H + kTileH - 1) / kTileH);
     L.items = o;   o = align_up(o + ((size_t)L.P + nbase + 16) * 4);
-    L.big = o;     o = align_up(o + ((size_t)L.max_big + 1) * sizeof(BigEntry));
-    L.bigkeys = o; o = align_up(o + (four_n + 8) * 8);
-    L.bigtin = o;  o = align_up(o + (four_n / 32 + L.max_big + 8) * 8);
+    L.bigpix = o;  o = align_up(o + ((size_t)L.P + 16) * 4);
+    L.bigcells = o; o = align_up(o + ((size_t)L.max_big_cells + 1) * sizeof(BigCell));
+    L.bigkeys = o; o = align_up(o + (n + 8) * 8);
+    if (flags & INPC_SAVE_FOR_BACKWARD) {
+        L.pcur = o; o = align_up(o + (size_t)L.P * 16);
+        L.gpt = o;  o = align_up(o + n * (size_t)(D == 4 ? 32 : 64) + 64);
+    }
     if (flags & INPC_SAVE_SORTED) {
         L.pixoff = o;       o = align_up(o + ((size_t)L.P + 1) * 4);
-        L.sorted_idx = o;   o = align_up(o + (four_n + 8) * 4);
-        L.sorted_depth = o; o = align_up(o + (four_n + 8) * 4);
+        L.sorted_idx = o;   o = align_up(o + (4 * n + 8) * 4);
+        L.sorted_depth = o; o = align_up(o + (4 * n + 8) * 4);
     }
     L.total = o;
     return L;
@@ -130,6 +138,7 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 static int check_common(int64_t N, int D, const inpc_camera* cam) {
     if (!cam || N < 0 || N >= (1ll << 30)) return INPC_ERR_INVALID_ARG;
     if (cam->width <= 0 || cam->height <= 0 || !(cam->near_z < cam->far_z)) return INPC_ERR_INVALID_ARG;
+    if (!(cam->near_z >= 0.f)) return INPC_ERR_INVALID_ARG;   // depth keys are the raw bits of a positive z_c
     if (D != 4 && D != 8) return INPC_ERR_UNSUPPORTED;
     if (cam->width > 4095 || cam->height > 4095) return INPC_ERR_UNSUPPORTED;
     return INPC_OK;
@@ -172,20 +181,29 @@ static int launch_tile(const TileArgs& A, int sms, cudaStream_t st) {
 }
 
 template <int D, int MODE>
-static int launch_big(const BigArgs& A, int sms, uint32_t max_big, cudaStream_t st) {
-    constexpr size_t smem = MODE == kBwd ? 0 : (size_t)kBigChunk * 8;
+static int launch_big(const BigArgs& A, int sms, cudaStream_t st) {
+    { StageTimer tm(MODE == kBwd ? kStBigBwd : kStBigFwd, st);
+      k_big<D, MODE><<<sms * 8, kLongThreads, 0, st>>>(A); }
+    INPC_LAUNCHED();
+    return INPC_OK;
+}
+
+template <int D>
+static int launch_cellsort_big(const Header* hdr, uint32_t* cursor, const BigCell* bigcells, const float4* A,
+                               unsigned long long* keys, const float* feat, uint32_t* dk, float4* R, int sms,
+                               uint32_t max_big_cells, cudaStream_t st) {
+    constexpr size_t smem = (size_t)kBigChunk * 8;
     static bool configured = false;
     static int grid = 0;
     if (!configured) {
-        if (smem > 48 * 1024)
-            INPC_CUDA(cudaFuncSetAttribute(k_big<D, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int rc = persistent_grid(k_big<D, MODE>, kBigThreads, smem, sms, &grid);
+        INPC_CUDA(cudaFuncSetAttribute(k_cellsort_big<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int rc = persistent_grid(k_cellsort_big<D>, kBigThreads, smem, sms, &grid);
         if (rc != INPC_OK) return rc;
         configured = true;
     }
-    const int g = (int)std::min<uint32_t>((uint32_t)grid, std::max<uint32_t>(max_big, 1u));
-    { StageTimer tm(MODE == kBwd ? kStBigBwd : kStBigFwd, st);
-      k_big<D, MODE><<<g, kBigThreads, smem, st>>>(A); }
+    const int g = (int)std::min<uint32_t>((uint32_t)grid, std::max<uint32_t>(max_big_cells, 1u));
+    { StageTimer tm(kStCellSortBig, st);
+      k_cellsort_big<D><<<g, kBigThreads, smem, st>>>(hdr, cursor, bigcells, A, keys, feat, dk, R); }
     INPC_LAUNCHED();
     return INPC_OK;
 }
@@ -199,27 +217,30 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
                         float* out_feat, float* out_alpha, unsigned char* ws, const Layout& L, uint32_t flags,
                         cudaStream_t st) {
     const DeviceInfo di = device_info();
-    if (!di.ok) return cuda_fail(cudaGetLastError() == cudaSuccess ? cudaErrorNoDevice : cudaErrorNoDevice);
+    if (!di.ok) return cuda_fail(cudaErrorNoDevice);
     const Camera camk = to_camera(cam);
     const int W = cam->width, H = cam->height;
     Header* hdr = reinterpret_cast<Header*>(ws + L.header);
     uint32_t* cellcnt = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
     uint32_t* rank = reinterpret_cast<uint32_t*>(ws + L.rank);
-    float4* rec = reinterpret_cast<float4*>(ws + L.rec);
-    float* rop = reinterpret_cast<float*>(ws + L.rop);
+    float4* Arec = reinterpret_cast<float4*>(ws + L.A);
+    uint32_t* dk = reinterpret_cast<uint32_t*>(ws + L.dk);
+    float4* R = reinterpret_cast<float4*>(ws + L.R);
     uint32_t* items = reinterpret_cast<uint32_t*>(ws + L.items);
-    BigEntry* big = reinterpret_cast<BigEntry*>(ws + L.big);
+    uint32_t* bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix);
+    BigCell* bigcells = reinterpret_cast<BigCell*>(ws + L.bigcells);
     const bool dump = (flags & INPC_SAVE_SORTED) != 0;
+    const bool save = (flags & INPC_SAVE_FOR_BACKWARD) != 0;
     uint32_t* pixoff = dump ? reinterpret_cast<uint32_t*>(ws + L.pixoff) : nullptr;
 
     { StageTimer tm(kStZeroFwd, st);
       INPC_CUDA(cudaMemsetAsync(ws + L.header, 0, L.zero_end - L.header, st));
       k_write_header<<<1, 1, 0, st>>>(hdr, flags, W, H, D, (uint32_t)N); }
     INPC_LAUNCHED();
+    const int bin_grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
     if (N > 0) {
-        const int grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
         { StageTimer tm(kStProjectCount, st);
-          k_project_count<<<grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, rank); }
+          k_project_count<<<bin_grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, rank); }
         INPC_LAUNCHED();
     }
     { StageTimer tm(kStScan, st);
@@ -227,14 +248,24 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
           cellcnt, L.C, reinterpret_cast<unsigned long long*>(ws + L.status0), &hdr->scan_tile_counter, &hdr->nrec); }
     INPC_LAUNCHED();
     if (N > 0) {
-        const int grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
         { StageTimer tm(kStScatter, st);
-          k_scatter<D><<<grid, kBinThreads, 0, st>>>(pos, opacity, feat, (long long)N, camk, cellcnt, rank, rec, rop); }
+          k_scatter<<<bin_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cellcnt, rank, Arec); }
         INPC_LAUNCHED();
     }
     { StageTimer tm(kStClassify, st);
-      k_classify_pixels<<<(L.P + 255) / 256, 256, 0, st>>>(cellcnt, W, H, hdr, big, pixoff); }
+      k_classify<<<(L.C + 255) / 256, 256, 0, st>>>(cellcnt, W, H, hdr, bigcells, pixoff); }
     INPC_LAUNCHED();
+    if (N > 0) {
+        const uint32_t n_units = (L.C + kCsCells - 1) / kCsCells;
+        { StageTimer tm(kStCellSort, st);
+          k_cellsort<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 8), kCsThreads, 0, st>>>(
+              Arec, cellcnt, L.C, feat, dk, R); }
+        INPC_LAUNCHED();
+        int rc = launch_cellsort_big<D>(hdr, &hdr->bigcell_cursor, bigcells, Arec,
+                                        reinterpret_cast<unsigned long long*>(ws + L.bigkeys), feat, dk, R, di.sms,
+                                        L.max_big_cells, st);
+        if (rc != INPC_OK) return rc;
+    }
     if (dump) {
         { StageTimer tm(kStOther, st);
           k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
@@ -243,28 +274,27 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     }
     const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
     { StageTimer tm(kStBuildItems, st);
-      k_build_items<<<(ntx * nty + 127) / 128, 128, 0, st>>>(cellcnt, W, H, TileCfg<D>::kCap, hdr, items); }
+      k_build_items<<<(ntx * nty + 127) / 128, 128, 0, st>>>(cellcnt, W, H, TileCfg<D>::kCap, hdr, items, bigpix); }
     INPC_LAUNCHED();
 
-    BigArgs B{};
-    B.hdr = hdr; B.big_cursor = &hdr->big_cursor; B.big = big; B.celloff = cellcnt; B.rec = rec; B.rop = rop;
-    B.bigkeys = reinterpret_cast<unsigned long long*>(ws + L.bigkeys);
-    B.bigtin = reinterpret_cast<double*>(ws + L.bigtin);
-    B.W = W; B.H = H; B.out_feat = out_feat; B.out_alpha = out_alpha;
     TileArgs A{};
-    A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = items; A.celloff = cellcnt; A.rec = rec; A.rop = rop;
+    A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = items; A.celloff = cellcnt; A.dk = dk; A.R = R;
     A.W = W; A.H = H; A.out_feat = out_feat; A.out_alpha = out_alpha;
+    BigArgs B{};
+    B.hdr = hdr; B.bigpix = bigpix; B.celloff = cellcnt; B.dk = dk; B.R = R;
+    B.W = W; B.H = H; B.out_feat = out_feat; B.out_alpha = out_alpha;
+    if (save) {
+        A.gT = B.gT = reinterpret_cast<float*>(ws + L.gT);
+        A.pcur = B.pcur = reinterpret_cast<uint4*>(ws + L.pcur);
+    }
     if (dump) {
         B.pixoff = A.pixoff = pixoff;
         B.sorted_idx = A.sorted_idx = reinterpret_cast<uint32_t*>(ws + L.sorted_idx);
         B.sorted_depth = A.sorted_depth = reinterpret_cast<uint32_t*>(ws + L.sorted_depth);
     }
-    int rc;
-    if (N > 0) {
-        rc = dump ? launch_big<D, kFwdDump>(B, di.sms, L.max_big, st) : launch_big<D, kFwd>(B, di.sms, L.max_big, st);
-        if (rc != INPC_OK) return rc;
-    }
-    rc = dump ? launch_tile<D, kFwdDump>(A, di.sms, st) : launch_tile<D, kFwd>(A, di.sms, st);
+    int rc = dump ? launch_tile<D, kFwdDump>(A, di.sms, st) : launch_tile<D, kFwd>(A, di.sms, st);
+    if (rc != INPC_OK) return rc;
+    if (N > 0) rc = dump ? launch_big<D, kFwdDump>(B, di.sms, st) : launch_big<D, kFwd>(B, di.sms, st);
     return rc;
 }
 
@@ -277,30 +307,36 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     Header* hdr = reinterpret_cast<Header*>(ws + L.header);
     {
         StageTimer tm(kStZeroBwd, st);
-        if (N > 0) {
-            INPC_CUDA(cudaMemsetAsync(d_feat, 0, (size_t)N * D * 4, st));
-            INPC_CUDA(cudaMemsetAsync(d_opacity, 0, (size_t)N * 4, st));
-            INPC_CUDA(cudaMemsetAsync(d_uv, 0, (size_t)N * 8, st));
-        }
-        INPC_CUDA(cudaMemsetAsync(&hdr->item_cursor, 0, 8, st));     // item_cursor + big_cursor
+        INPC_CUDA(cudaMemsetAsync(&hdr->item_cursor, 0, 4, st));
     }
+    if (N == 0) return INPC_OK;
+    const uint32_t* celloff = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
+    const float4* R = reinterpret_cast<float4*>(ws + L.R);
+    float* gT = reinterpret_cast<float*>(ws + L.gT);
+    float* gD = reinterpret_cast<float*>(ws + L.gD);
+    uint4* pcur = reinterpret_cast<uint4*>(ws + L.pcur);
+    float* gpt = reinterpret_cast<float*>(ws + L.gpt);
     TileArgs A{};
     A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = reinterpret_cast<uint32_t*>(ws + L.items);
-    A.celloff = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
-    A.rec = reinterpret_cast<float4*>(ws + L.rec); A.rop = reinterpret_cast<float*>(ws + L.rop);
-    A.W = W; A.H = H; A.g_feat = g_feat; A.g_alpha = g_alpha; A.d_feat = d_feat; A.d_opacity = d_opacity; A.d_uv = d_uv;
+    A.celloff = celloff; A.dk = reinterpret_cast<uint32_t*>(ws + L.dk); A.R = R;
+    A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD;
     int rc = launch_tile<D, kBwd>(A, di.sms, st);
     if (rc != INPC_OK) return rc;
-    if (N > 0) {
-        BigArgs B{};
-        B.hdr = hdr; B.big_cursor = &hdr->big_cursor; B.big = reinterpret_cast<BigEntry*>(ws + L.big);
-        B.celloff = A.celloff; B.rec = A.rec; B.rop = A.rop;
-        B.bigkeys = reinterpret_cast<unsigned long long*>(ws + L.bigkeys);
-        B.bigtin = reinterpret_cast<double*>(ws + L.bigtin);
-        B.W = W; B.H = H; B.g_feat = g_feat; B.g_alpha = g_alpha; B.d_feat = d_feat; B.d_opacity = d_opacity; B.d_uv = d_uv;
-        rc = launch_big<D, kBwd>(B, di.sms, L.max_big, st);
-    }
-    return rc;
+    BigArgs B{};
+    B.hdr = hdr; B.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); B.celloff = celloff; B.dk = A.dk; B.R = R;
+    B.W = W; B.H = H; B.gT = gT; B.pcur = pcur; B.g_feat = g_feat; B.g_alpha = g_alpha; B.gD = gD;
+    rc = launch_big<D, kBwd>(B, di.sms, st);
+    if (rc != INPC_OK) return rc;
+    const uint32_t n_units = (L.C + kGradCells - 1) / kGradCells;
+    { StageTimer tm(kStCombine, st);
+      k_combine<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 8), kGradThreads, 0, st>>>(
+          celloff, L.C, W, H, R, reinterpret_cast<const float4*>(gT), reinterpret_cast<const float4*>(gD), pcur, g_feat, gpt); }
+    INPC_LAUNCHED();
+    { StageTimer tm(kStSplit, st);
+      k_split<D><<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16), 256, 0, st>>>(
+          gpt, reinterpret_cast<const uint32_t*>(ws + L.rank), (long long)N, d_feat, d_opacity, d_uv); }
+    INPC_LAUNCHED();
+    return INPC_OK;
 }
 
 }  // namespace inpc
@@ -406,8 +442,9 @@ int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_s
     stats->n_kept = h.nrec;
     stats->n_fragments = h.n_fragments;
     stats->n_tile_items = h.n_items;
-    stats->n_big_pixels = h.big_packed >> 40;
-    stats->n_big_fragments = h.big_packed & ((1ull << 40) - 1);
+    stats->n_big_pixels = h.n_big_pixels;
+    stats->n_big_fragments = h.n_big_fragments;
+    stats->n_big_cells = h.n_big_cells;
     return INPC_OK;
 }
 

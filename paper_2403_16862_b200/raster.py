@@ -35,7 +35,7 @@ class InpcCamera(C.Structure):
 
 class InpcStats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in ("n_points", "n_kept", "n_fragments", "n_tile_items",
-                                          "n_big_pixels", "n_big_fragments")]
+                                          "n_big_pixels", "n_big_fragments", "n_big_cells")]
 
 
 class InpcError(RuntimeError):

@@ -41,7 +41,7 @@ def test_every_declared_symbol_is_exported(lib):
 def test_camera_struct_layout_matches_header(lib):
     # 4 + 9 + 3 + 2 floats + 2 int32 = 80 bytes, no padding
     assert C.sizeof(raster.InpcCamera) == 80
-    assert C.sizeof(raster.InpcStats) == 48
+    assert C.sizeof(raster.InpcStats) == 56       # 7 x uint64
 
 
 def test_workspace_bytes_host_logic(lib):
