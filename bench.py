@@ -62,7 +62,9 @@ STAGE_ROWS = {
     "k_tile_fwd": "a3_a4", "k_big_fwd": "a3_a4",
     "k_tile_bwd": "a5", "k_big_bwd": "a5", "zero_bwd": "a5",
     "zero_fwd": "a1_a2", "k_project_count": "a1_a2", "k_scan_u32": "a1_a2", "k_scatter": "a1_a2",
-    "k_classify_pixels": "a1_a2", "k_build_items": "a1_a2",
+    "k_classify": "a1_a2", "k_build_items": "a1_a2",
+    "k_cellsort": "a3_a4", "k_cellsort_big": "a3_a4",
+    "k_combine": "a5", "k_split": "a5", "other": "a1_a2",
 }
 
 
