@@ -18,7 +18,8 @@ struct BigArgs {
     const uint32_t* bigpix;
     const uint32_t* celloff;
     const uint32_t* dk;
-    const float4* R;
+    const float4* Ra;
+    const float4* Rf;
     int W, H;
     float* out_feat;
     float* out_alpha;
@@ -47,7 +48,7 @@ __global__ void __launch_bounds__(kLongThreads) k_big(BigArgs A) {
             float acc[D]; float accA;
             uint4 consumed = make_uint4(0, 0, 0, 0);
             const uint32_t obase = (MODE == kFwdDump) ? A.pixoff[pix] : 0u;
-            blend_pixel<D, MODE == kFwdDump, double>(A.dk, A.R, L, 0u, 0u, A.gT, acc, accA, consumed, A.sorted_idx,
+            blend_pixel<D, MODE == kFwdDump, double>(A.dk, A.Ra, A.Rf, L, 0u, 0u, A.gT, acc, accA, consumed, A.sorted_idx,
                                                      A.sorted_depth, obase);
 #pragma unroll
             for (int v = 0; v < D / 4; ++v)
@@ -64,7 +65,7 @@ __global__ void __launch_bounds__(kLongThreads) k_big(BigArgs A) {
                 g[4 * v] = t.x; g[4 * v + 1] = t.y; g[4 * v + 2] = t.z; g[4 * v + 3] = t.w;
             }
             const float gA = A.g_alpha ? __ldg(A.g_alpha + pix) : 0.f;
-            backward_pixel<D, double>(A.dk, A.R, A.gT, L, 0u, 0u, g, gA, A.gD);
+            backward_pixel<D, double>(A.dk, A.Ra, A.Rf, A.gT, L, 0u, 0u, g, gA, A.gD);
         }
     }
 }

@@ -1,0 +1,235 @@
+// blend.cuh -- step a4 of the hot path: per-pixel 4-way merge of the sorted cell lists and front-to-back
+// compositing (Eq. 1; cut-off T < 1e-4 from BASELINE.json north_star).
+//
+// One persistent CTA per work item (a screen tile of tw x th <= 128 pixels whose records fit in shared
+// memory).  The tile's th+1 cell rows are contiguous slot ranges of the cell-sorted arrays dk / Ra / Rf
+// and are staged with cp.async.bulk (TMA, 1-D) onto one mbarrier.  Then
+//   1. one thread per staged record turns { tx, ty, opacity, idx } into the four per-corner alphas
+//      a_c = opacity * w_c (Eq. 7) in place, so the merge loop reads ONE float per fragment;
+//   2. the tile's pixels are handed to lanes in descending order of their fragment count (counting sort on
+//      count / 4), so that the 32 pixels of a warp run about equally long
+//      (profiles/r01_v2_cellsort_merge.md: neighbouring pixels gave 10 of 32 lanes active);
+//   3. ONE THREAD PER PIXEL merges its four lists.  The iteration is branch-free: every list's cursor and
+//      end are packed into one register (byte offset of the fragment's alpha | end << 16), the minimum
+//      head key selects the list with predicates, and only "two heads with equal depth bits" (ascending
+//      point index decides, read from global memory) and the two loop exits are branches.
+// With INPC_SAVE_FOR_BACKWARD the transmittance in front of every blended fragment goes to
+// gT[(slot, corner)] and the four list positions at the stop to pcur[pixel].
+#pragma once
+#include "common.cuh"
+
+namespace inpc {
+
+struct BlendArgs {
+    const Header* hdr;
+    uint32_t* item_cursor;
+    const uint32_t* items;
+    const uint32_t* celloff;
+    const uint32_t* dk;
+    const float4* Ra;
+    const float4* Rf;
+    int W, H;
+    float* out_feat;
+    float* out_alpha;
+    float* gT;               // NULL unless INPC_SAVE_FOR_BACKWARD
+    uint4* pcur;
+    // dump (INPC_SAVE_SORTED)
+    const uint32_t* pixoff;
+    uint32_t* sorted_idx;
+    uint32_t* sorted_depth;
+};
+
+template <int D> __host__ __device__ constexpr size_t blend_smem_bytes() {
+    return (size_t)TileCfg<D>::kCap * (4 + 16 + 4 * D);
+}
+
+// Packed list state: low 16 bits = byte offset of the head fragment's alpha inside s_a (record * 16 +
+// 4 * corner), high 16 bits = the same for the list's end.  One record further = + 16.
+__device__ __forceinline__ uint32_t pack_list(uint32_t start_rec, uint32_t end_rec, int corner) {
+    return (start_rec * 16u + 4u * corner) | ((end_rec * 16u + 4u * corner) << 16);
+}
+
+template <int D, bool DUMP>
+__global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
+    constexpr int FV  = D / 4;                     // float4 of features per record
+    constexpr int CAP = TileCfg<D>::kCap;
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint32_t* s_dk = reinterpret_cast<uint32_t*>(smem);
+    float4*   s_a4 = reinterpret_cast<float4*>(smem + (size_t)CAP * 4);
+    float4*   s_f  = reinterpret_cast<float4*>(smem + (size_t)CAP * 20);
+    const unsigned char* s_ab = smem + (size_t)CAP * 4;
+
+    __shared__ uint32_t s_off[kTileH + 1][kTileW + 2];
+    __shared__ uint32_t s_sbase[kTileH + 1], s_a4row[kTileH + 1];
+    __shared__ uint32_t s_hist[64];
+    __shared__ uint8_t  s_perm[kTileThreads];
+    __shared__ uint32_t s_item, s_tot;
+    __shared__ __align__(8) uint64_t s_bar;
+
+    const int tid = threadIdx.x;
+    const int W = A.W, H = A.H;
+    const uint32_t n_items = A.hdr->n_items;
+
+    if (tid == 0) { mbar_init(&s_bar, 1); fence_mbar_init(); }
+    uint32_t parity = 0;
+
+    while (true) {
+        __syncthreads();                                  // everyone is done with the previous item's smem
+        if (tid == 0) s_item = atomicAdd(A.item_cursor, 1u);
+        if (tid < 64) s_hist[tid] = 0;
+        __syncthreads();
+        const uint32_t item_i = s_item;
+        if (item_i >= n_items) break;
+        const uint32_t it = A.items[item_i];
+        const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
+        const int tw = 1 << lw, th = 1 << lh;
+
+        // cell offsets of the tile's (th+1) x (tw+2) window
+        for (int e = tid; e < (th + 1) * (tw + 2); e += kTileThreads) {
+            const int r = e / (tw + 2), c = e - r * (tw + 2);
+            const int j = Y + r;
+            uint32_t v = 0;
+            if (j <= H) v = __ldg(&A.celloff[(uint32_t)j * (W + 1) + min(X + c, W + 1)]);
+            s_off[r][c] = v;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            uint32_t tot = 0;
+            for (int r = 0; r <= th; ++r) {
+                const uint32_t a = s_off[r][0], b = s_off[r][tw + 1];
+                const uint32_t a4 = a & ~3u, b4 = (b + 3u) & ~3u;
+                s_a4row[r] = a4; s_sbase[r] = tot;
+                tot += (b > a) ? (b4 - a4) : 0u;
+            }
+            s_tot = tot;
+            if (tot > 0) {
+                fence_proxy_async();
+                mbar_arrive_expect_tx(&s_bar, tot * (uint32_t)(4 + 16 + 16 * FV));
+                for (int r = 0; r <= th; ++r) {
+                    const uint32_t a = s_off[r][0], b = s_off[r][tw + 1];
+                    if (b <= a) continue;
+                    const uint32_t a4 = s_a4row[r], len = ((b + 3u) & ~3u) - a4, sb = s_sbase[r];
+                    bulk_g2s(s_dk + sb, A.dk + a4, len * 4, &s_bar);
+                    bulk_g2s(s_a4 + sb, A.Ra + a4, len * 16, &s_bar);
+                    bulk_g2s(s_f + (size_t)sb * FV, A.Rf + (size_t)a4 * FV, len * FV * 16, &s_bar);
+                }
+            }
+        }
+        // while the copies fly: this thread's pixel, its fragment count, and the count histogram
+        const int ly0 = tid >> lw, lx0 = tid & (tw - 1);
+        uint32_t n_mine = 0;
+        const bool live0 = tid < tw * th && X + lx0 < W && Y + ly0 < H;
+        if (live0)
+            n_mine = (s_off[ly0][lx0 + 2] - s_off[ly0][lx0]) + (s_off[ly0 + 1][lx0 + 2] - s_off[ly0 + 1][lx0]);
+        const uint32_t bucket = 63u - min(n_mine >> 2, 63u);          // descending count
+        const uint32_t rank_in_bucket = atomicAdd(&s_hist[bucket], 1u);
+        __syncthreads();
+        if (tid < 32) {                                                // exclusive scan of the 64 buckets
+            const uint32_t h0 = s_hist[2 * tid], h1 = s_hist[2 * tid + 1];
+            uint32_t inc = h0 + h1;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d); if (tid >= d) inc += t; }
+            s_hist[2 * tid] = inc - h0 - h1;
+            s_hist[2 * tid + 1] = inc - h1;
+        }
+        __syncthreads();
+        s_perm[s_hist[bucket] + rank_in_bucket] = (uint8_t)tid;
+        const uint32_t tot = s_tot;
+        if (tot > 0) { mbar_wait(&s_bar, parity); parity ^= 1u; }
+        // 1. per-corner alphas in place: { tx, ty, opacity, idx } -> { a_0, a_1, a_2, a_3 }, corner c = 2 dy + dx
+        for (uint32_t r = tid; r < tot; r += kTileThreads) {
+            const float4 q = s_a4[r];
+            const float wx0 = 1.f - q.x, wy0 = 1.f - q.y;
+            s_a4[r] = make_float4(q.z * (wx0 * wy0), q.z * (q.x * wy0), q.z * (wx0 * q.y), q.z * (q.x * q.y));
+        }
+        __syncthreads();
+
+        // ---------------------------------------------------------------- 3. one thread per pixel
+        const int q = s_perm[tid];
+        const int ly = q >> lw, lx = q & (tw - 1);
+        const int x = X + lx, y = Y + ly;
+        if (q >= tw * th || x >= W || y >= H) continue;
+        const size_t pix = (size_t)y * W + x;
+        // smem record of global slot g in cell row r: g + (s_sbase[r] - s_a4row[r])
+        const uint32_t bt = s_sbase[ly] - s_a4row[ly], bb = s_sbase[ly + 1] - s_a4row[ly + 1];
+        const uint32_t st0 = s_off[ly][lx] + bt, st1 = s_off[ly][lx + 1] + bt, en1 = s_off[ly][lx + 2] + bt;
+        const uint32_t st2 = s_off[ly + 1][lx] + bb, st3 = s_off[ly + 1][lx + 1] + bb, en3 = s_off[ly + 1][lx + 2] + bb;
+        // list j holds the pixel's fragments of corner 3 - j
+        uint32_t ce0 = pack_list(st0, st1, 3), ce1 = pack_list(st1, en1, 2);
+        uint32_t ce2 = pack_list(st2, st3, 1), ce3 = pack_list(st3, en3, 0);
+        uint32_t h0 = st0 < st1 ? s_dk[st0] : kSentHi, h1 = st1 < en1 ? s_dk[st1] : kSentHi;
+        uint32_t h2 = st2 < st3 ? s_dk[st2] : kSentHi, h3 = st3 < en3 ? s_dk[st3] : kSentHi;
+        // global float index of (slot, corner) = (cursor >> 2) + 4 * (slot - smem record)
+        float* gTtop = A.gT ? A.gT + 4 * ((ptrdiff_t)(int32_t)(0u - bt)) : nullptr;
+        float* gTbot = A.gT ? A.gT + 4 * ((ptrdiff_t)(int32_t)(0u - bb)) : nullptr;
+
+        float acc[D];
+#pragma unroll
+        for (int d = 0; d < D; ++d) acc[d] = 0.f;
+        float accA = 0.f, T = 1.f;
+        uint4 consumed = make_uint4(0, 0, 0, 0);
+        bool blending = true;
+        uint32_t k = 0;
+        const uint32_t obase = DUMP ? A.pixoff[pix] : 0u;
+        while (true) {
+            const uint32_t m = min(min(h0, h1), min(h2, h3));
+            if (m == kSentHi) break;
+            if (DUMP) {
+                if (blending && T < kTMin) {
+                    blending = false;
+                    consumed = make_uint4(((ce0 & 0xffffu) >> 4) - st0, ((ce1 & 0xffffu) >> 4) - st1,
+                                          ((ce2 & 0xffffu) >> 4) - st2, ((ce3 & 0xffffu) >> 4) - st3);
+                }
+            } else {
+                if (T < kTMin) break;                     // fragment k is blended iff T_k >= 1e-4
+            }
+            bool p0 = h0 == m, p1 = h1 == m, p2 = h2 == m, p3 = h3 == m;
+            if ((p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3)) {
+                uint32_t best = 0xFFFFFFFFu;              // equal depth bits: ascending point index
+                int jb = 0;
+                if (p0) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce0 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 0; } }
+                if (p1) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce1 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 1; } }
+                if (p2) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce2 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 2; } }
+                if (p3) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce3 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 3; } }
+                p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;
+            }
+            const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
+            const uint32_t cur = ce & 0xffffu;
+            if (!DUMP || blending) {
+                const float a = *reinterpret_cast<const float*>(s_ab + cur);
+                const float c = T * a;
+                accA += c;
+#pragma unroll
+                for (int v = 0; v < FV; ++v) {
+                    const float4 f = s_f[(cur >> 4) * FV + v];
+                    acc[4 * v] += c * f.x; acc[4 * v + 1] += c * f.y; acc[4 * v + 2] += c * f.z; acc[4 * v + 3] += c * f.w;
+                }
+                if (A.gT) ((p0 | p1) ? gTtop : gTbot)[cur >> 2] = T;
+                T *= (1.f - a);
+            }
+            if (DUMP) {
+                const uint32_t slot = (cur >> 4) - ((p0 | p1) ? bt : bb);
+                A.sorted_idx[obase + k] = __float_as_uint(__ldg(&A.Ra[slot]).w);
+                A.sorted_depth[obase + k] = m;
+                ++k;
+            }
+            const uint32_t nx = ce + 16u;
+            const uint32_t nc = nx & 0xffffu;
+            const uint32_t nh = nc < (nx >> 16) ? s_dk[nc >> 4] : kSentHi;
+            h0 = p0 ? nh : h0; ce0 = p0 ? nx : ce0;
+            h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;
+            h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
+            h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
+        }
+        if (!DUMP || blending)
+            consumed = make_uint4(((ce0 & 0xffffu) >> 4) - st0, ((ce1 & 0xffffu) >> 4) - st1,
+                                  ((ce2 & 0xffffu) >> 4) - st2, ((ce3 & 0xffffu) >> 4) - st3);
+#pragma unroll
+        for (int v = 0; v < FV; ++v)
+            reinterpret_cast<float4*>(A.out_feat + pix * D)[v] = make_float4(acc[4 * v], acc[4 * v + 1], acc[4 * v + 2], acc[4 * v + 3]);
+        A.out_alpha[pix] = accA;
+        if (A.gT) A.pcur[pix] = consumed;
+    }
+}
+
+}  // namespace inpc

@@ -26,24 +26,23 @@ constexpr int kCsCells   = 1024;                         // cells per CTA work u
 template <int D>
 __device__ __forceinline__ void emit_sorted(const float4 a0, const float4 a1, uint32_t dst,
                                             const float* __restrict__ feat, uint32_t* __restrict__ dk,
-                                            float4* __restrict__ R) {
-    constexpr int RV = 1 + D / 4;
+                                            float4* __restrict__ Ra, float4* __restrict__ Rf) {
+    constexpr int FV = D / 4;
     const uint32_t idx = __float_as_uint(a0.y);
     float4 f[D / 4];
 #pragma unroll
     for (int q = 0; q < D / 4; ++q) f[q] = __ldg(reinterpret_cast<const float4*>(feat + (size_t)idx * D) + q);
     dk[dst] = __float_as_uint(a0.x);
-    float4* out = R + (size_t)dst * RV;
-    out[0] = make_float4(a0.z, a0.w, a1.x, a0.y);        // tx, ty, opacity, idx
+    Ra[dst] = make_float4(a0.z, a0.w, a1.x, a0.y);       // tx, ty, opacity, idx
 #pragma unroll
-    for (int q = 0; q < D / 4; ++q) out[1 + q] = f[q];
+    for (int q = 0; q < FV; ++q) Rf[(size_t)dst * FV + q] = f[q];
 }
 
 template <int D>
 __global__ void __launch_bounds__(kCsThreads) k_cellsort(const float4* __restrict__ A,
                                                           const uint32_t* __restrict__ celloff, uint32_t C,
                                                           const float* __restrict__ feat,
-                                                          uint32_t* __restrict__ dk, float4* __restrict__ R) {
+                                                          uint32_t* __restrict__ dk, float4* __restrict__ Ra, float4* __restrict__ Rf) {
     __shared__ uint32_t s_off[kCsCells + 1];
     __shared__ unsigned long long s_key[kCsWindow];
     const int tid = threadIdx.x;
@@ -86,7 +85,7 @@ __global__ void __launch_bounds__(kCsThreads) k_cellsort(const float4* __restric
                             const unsigned long long me = s_key[l];
                             uint32_t r = 0;
                             for (uint32_t j = cs; j < ce; ++j) r += s_key[j] < me ? 1u : 0u;
-                            emit_sorted<D>(a0[q], a1[q], s0 + cs + r, feat, dk, R);
+                            emit_sorted<D>(a0[q], a1[q], s0 + cs + r, feat, dk, Ra, Rf);
                         }
                     }
                 }
@@ -146,7 +145,7 @@ __global__ void __launch_bounds__(kBigThreads) k_cellsort_big(const Header* __re
                                                                const float4* __restrict__ A,
                                                                unsigned long long* __restrict__ keys_all,
                                                                const float* __restrict__ feat,
-                                                               uint32_t* __restrict__ dk, float4* __restrict__ R) {
+                                                               uint32_t* __restrict__ dk, float4* __restrict__ Ra, float4* __restrict__ Rf) {
     extern __shared__ __align__(16) unsigned char smem_big[];
     unsigned long long* s_keys = reinterpret_cast<unsigned long long*>(smem_big);
     __shared__ uint32_t s_b;
@@ -217,7 +216,7 @@ __global__ void __launch_bounds__(kBigThreads) k_cellsort_big(const Header* __re
         for (uint32_t l = tid; l < n; l += kBigThreads) {
             const uint32_t src = (uint32_t)__ldcg(&keys[l]);
             const float4 a0 = __ldg(&A[2 * (size_t)src]), a1 = __ldg(&A[2 * (size_t)src + 1]);
-            emit_sorted<D>(a0, a1, start + l, feat, dk, R);
+            emit_sorted<D>(a0, a1, start + l, feat, dk, Ra, Rf);
         }
     }
 }

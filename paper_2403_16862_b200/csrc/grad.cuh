@@ -24,11 +24,10 @@ template <int D> __host__ __device__ constexpr int gpt_floats() { return D == 4 
 
 template <int D>
 __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __restrict__ celloff, uint32_t C, int W,
-                                                           int H, const float4* __restrict__ R,
+                                                           int H, const float4* __restrict__ Ra,
                                                            const float4* __restrict__ gT, const float4* __restrict__ gD,
                                                            const uint4* __restrict__ pcur,
                                                            const float* __restrict__ g_feat, float* __restrict__ gpt) {
-    constexpr int RV = 1 + D / 4;
     constexpr int GP = gpt_floats<D>();
     __shared__ uint32_t s_off[kGradCells + 1];
     const int tid = threadIdx.x;
@@ -49,7 +48,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
             const uint32_t cell = c0 + lo, r = slot - s_off[lo];
             const int j = cell / (W + 1), i = cell - j * (W + 1);
             const int x0 = i - 1, y0 = j - 1;
-            const float4 r0 = __ldg(&R[(size_t)slot * RV]);       // tx, ty, opacity, idx
+            const float4 r0 = __ldg(&Ra[slot]);       // tx, ty, opacity, idx
             const float4 t4 = __ldcs(&gT[slot]), d4 = __ldcs(&gD[slot]);
             const float tc[4] = {t4.x, t4.y, t4.z, t4.w}, dc[4] = {d4.x, d4.y, d4.z, d4.w};
             float df[D];

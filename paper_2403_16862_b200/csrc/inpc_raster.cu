@@ -14,6 +14,7 @@
 
 #include "bin.cuh"
 #include "big.cuh"
+#include "blend.cuh"
 #include "cellsort.cuh"
 #include "common.cuh"
 #include "grad.cuh"
@@ -62,7 +63,7 @@ struct StageTimer {                       // RAII: start event now, stop event a
 
 struct Layout {
     size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
-    size_t rank, A, gT, gD, dk, R, items, bigpix, bigcells, bigkeys;
+    size_t rank, A, gT, gD, dk, Ra, Rf, items, bigpix, bigcells, bigkeys;
     size_t pcur, gpt;                                     // only with INPC_SAVE_FOR_BACKWARD
     size_t pixoff, sorted_idx, sorted_depth;              // only with INPC_SAVE_SORTED
     size_t total;
@@ -88,7 +89,8 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     L.A = o;       L.gT = o; L.gD = o + (n + 8) * 16;     // the emission records are dead once the cells are sorted:
     o = align_up(o + (n + 8) * 32);                       // their bytes then hold gT | gD (16 B per record each)
     L.dk = o;      o = align_up(o + (n + 16) * 4);
-    L.R = o;       o = align_up(o + (n + 8) * (size_t)(16 + 4 * D));
+    L.Ra = o;      o = align_up(o + (n + 8) * 16);
+    L.Rf = o;      o = align_up(o + (n + 8) * (size_t)(4 * D));
     const size_t nbase = (size_t)((W + kTileW - 1) / kTileW) * ((H + kTileH - 1) / kTileH);
     L.items = o;   o = align_up(o + ((size_t)L.P + nbase + 16) * 4);
     L.bigpix = o;  o = align_up(o + ((size_t)L.P + 16) * 4);
@@ -180,6 +182,23 @@ static int launch_tile(const TileArgs& A, int sms, cudaStream_t st) {
     return INPC_OK;
 }
 
+template <int D, bool DUMP>
+static int launch_blend(const BlendArgs& A, int sms, cudaStream_t st) {
+    constexpr size_t smem = blend_smem_bytes<D>();
+    static bool configured = false;
+    static int grid = 0;
+    if (!configured) {
+        INPC_CUDA(cudaFuncSetAttribute(k_blend<D, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int rc = persistent_grid(k_blend<D, DUMP>, kTileThreads, smem, sms, &grid);
+        if (rc != INPC_OK) return rc;
+        configured = true;
+    }
+    { StageTimer tm(kStTileFwd, st);
+      k_blend<D, DUMP><<<grid, kTileThreads, smem, st>>>(A); }
+    INPC_LAUNCHED();
+    return INPC_OK;
+}
+
 template <int D, int MODE>
 static int launch_big(const BigArgs& A, int sms, cudaStream_t st) {
     { StageTimer tm(MODE == kBwd ? kStBigBwd : kStBigFwd, st);
@@ -190,7 +209,7 @@ static int launch_big(const BigArgs& A, int sms, cudaStream_t st) {
 
 template <int D>
 static int launch_cellsort_big(const Header* hdr, uint32_t* cursor, const BigCell* bigcells, const float4* A,
-                               unsigned long long* keys, const float* feat, uint32_t* dk, float4* R, int sms,
+                               unsigned long long* keys, const float* feat, uint32_t* dk, float4* Ra, float4* Rf, int sms,
                                uint32_t max_big_cells, cudaStream_t st) {
     constexpr size_t smem = (size_t)kBigChunk * 8;
     static bool configured = false;
@@ -203,7 +222,7 @@ static int launch_cellsort_big(const Header* hdr, uint32_t* cursor, const BigCel
     }
     const int g = (int)std::min<uint32_t>((uint32_t)grid, std::max<uint32_t>(max_big_cells, 1u));
     { StageTimer tm(kStCellSortBig, st);
-      k_cellsort_big<D><<<g, kBigThreads, smem, st>>>(hdr, cursor, bigcells, A, keys, feat, dk, R); }
+      k_cellsort_big<D><<<g, kBigThreads, smem, st>>>(hdr, cursor, bigcells, A, keys, feat, dk, Ra, Rf); }
     INPC_LAUNCHED();
     return INPC_OK;
 }
@@ -225,7 +244,8 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     uint32_t* rank = reinterpret_cast<uint32_t*>(ws + L.rank);
     float4* Arec = reinterpret_cast<float4*>(ws + L.A);
     uint32_t* dk = reinterpret_cast<uint32_t*>(ws + L.dk);
-    float4* R = reinterpret_cast<float4*>(ws + L.R);
+    float4* Ra = reinterpret_cast<float4*>(ws + L.Ra);
+    float4* Rf = reinterpret_cast<float4*>(ws + L.Rf);
     uint32_t* items = reinterpret_cast<uint32_t*>(ws + L.items);
     uint32_t* bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix);
     BigCell* bigcells = reinterpret_cast<BigCell*>(ws + L.bigcells);
@@ -259,10 +279,10 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
         const uint32_t n_units = (L.C + kCsCells - 1) / kCsCells;
         { StageTimer tm(kStCellSort, st);
           k_cellsort<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 8), kCsThreads, 0, st>>>(
-              Arec, cellcnt, L.C, feat, dk, R); }
+              Arec, cellcnt, L.C, feat, dk, Ra, Rf); }
         INPC_LAUNCHED();
         int rc = launch_cellsort_big<D>(hdr, &hdr->bigcell_cursor, bigcells, Arec,
-                                        reinterpret_cast<unsigned long long*>(ws + L.bigkeys), feat, dk, R, di.sms,
+                                        reinterpret_cast<unsigned long long*>(ws + L.bigkeys), feat, dk, Ra, Rf, di.sms,
                                         L.max_big_cells, st);
         if (rc != INPC_OK) return rc;
     }
@@ -277,11 +297,11 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
       k_build_items<<<(ntx * nty + 127) / 128, 128, 0, st>>>(cellcnt, W, H, TileCfg<D>::kCap, hdr, items, bigpix); }
     INPC_LAUNCHED();
 
-    TileArgs A{};
-    A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = items; A.celloff = cellcnt; A.dk = dk; A.R = R;
+    BlendArgs A{};
+    A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = items; A.celloff = cellcnt; A.dk = dk; A.Ra = Ra; A.Rf = Rf;
     A.W = W; A.H = H; A.out_feat = out_feat; A.out_alpha = out_alpha;
     BigArgs B{};
-    B.hdr = hdr; B.bigpix = bigpix; B.celloff = cellcnt; B.dk = dk; B.R = R;
+    B.hdr = hdr; B.bigpix = bigpix; B.celloff = cellcnt; B.dk = dk; B.Ra = Ra; B.Rf = Rf;
     B.W = W; B.H = H; B.out_feat = out_feat; B.out_alpha = out_alpha;
     if (save) {
         A.gT = B.gT = reinterpret_cast<float*>(ws + L.gT);
@@ -292,7 +312,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
         B.sorted_idx = A.sorted_idx = reinterpret_cast<uint32_t*>(ws + L.sorted_idx);
         B.sorted_depth = A.sorted_depth = reinterpret_cast<uint32_t*>(ws + L.sorted_depth);
     }
-    int rc = dump ? launch_tile<D, kFwdDump>(A, di.sms, st) : launch_tile<D, kFwd>(A, di.sms, st);
+    int rc = dump ? launch_blend<D, true>(A, di.sms, st) : launch_blend<D, false>(A, di.sms, st);
     if (rc != INPC_OK) return rc;
     if (N > 0) rc = dump ? launch_big<D, kFwdDump>(B, di.sms, st) : launch_big<D, kFwd>(B, di.sms, st);
     return rc;
@@ -311,26 +331,27 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     }
     if (N == 0) return INPC_OK;
     const uint32_t* celloff = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
-    const float4* R = reinterpret_cast<float4*>(ws + L.R);
+    const float4* Ra = reinterpret_cast<float4*>(ws + L.Ra);
+    const float4* Rf = reinterpret_cast<float4*>(ws + L.Rf);
     float* gT = reinterpret_cast<float*>(ws + L.gT);
     float* gD = reinterpret_cast<float*>(ws + L.gD);
     uint4* pcur = reinterpret_cast<uint4*>(ws + L.pcur);
     float* gpt = reinterpret_cast<float*>(ws + L.gpt);
     TileArgs A{};
     A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = reinterpret_cast<uint32_t*>(ws + L.items);
-    A.celloff = celloff; A.dk = reinterpret_cast<uint32_t*>(ws + L.dk); A.R = R;
+    A.celloff = celloff; A.dk = reinterpret_cast<uint32_t*>(ws + L.dk); A.Ra = Ra; A.Rf = Rf;
     A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD;
     int rc = launch_tile<D, kBwd>(A, di.sms, st);
     if (rc != INPC_OK) return rc;
     BigArgs B{};
-    B.hdr = hdr; B.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); B.celloff = celloff; B.dk = A.dk; B.R = R;
+    B.hdr = hdr; B.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); B.celloff = celloff; B.dk = A.dk; B.Ra = Ra; B.Rf = Rf;
     B.W = W; B.H = H; B.gT = gT; B.pcur = pcur; B.g_feat = g_feat; B.g_alpha = g_alpha; B.gD = gD;
     rc = launch_big<D, kBwd>(B, di.sms, st);
     if (rc != INPC_OK) return rc;
     const uint32_t n_units = (L.C + kGradCells - 1) / kGradCells;
     { StageTimer tm(kStCombine, st);
       k_combine<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 8), kGradThreads, 0, st>>>(
-          celloff, L.C, W, H, R, reinterpret_cast<const float4*>(gT), reinterpret_cast<const float4*>(gD), pcur, g_feat, gpt); }
+          celloff, L.C, W, H, Ra, reinterpret_cast<const float4*>(gT), reinterpret_cast<const float4*>(gD), pcur, g_feat, gpt); }
     INPC_LAUNCHED();
     { StageTimer tm(kStSplit, st);
       k_split<D><<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16), 256, 0, st>>>(

@@ -29,7 +29,8 @@ struct TileArgs {
     const uint32_t* items;
     const uint32_t* celloff;
     const uint32_t* dk;
-    const float4* R;
+    const float4* Ra;
+    const float4* Rf;
     int W, H;
     // forward
     float* out_feat;
@@ -46,11 +47,8 @@ struct TileArgs {
     float* gD;
 };
 
-template <int D> __host__ __device__ constexpr int rec_bytes() { return 16 + 4 * D; }
 template <int D, int MODE> __host__ __device__ constexpr size_t tile_smem_bytes() {
-    size_t b = (size_t)TileCfg<D>::kCap * (4 + rec_bytes<D>());
-    if (MODE == kBwd) b += (size_t)TileCfg<D>::kCap * 16;            // staged gT
-    return b;
+    return (size_t)TileCfg<D>::kCap * (4 + 16 + 4 * D + 16);       // dk, Ra, Rf, staged gT
 }
 
 // The four lists of one pixel as cursors into dk / R (shared-memory indices in the tile kernel, global
@@ -60,11 +58,11 @@ struct PixLists { uint32_t c0, e0, c1, e1, c2, e2, c3, e3; };
 // Forward merge + blend of one pixel.  gofs_top / gofs_bot: global slot = cursor + gofs (per cell row).
 // TT = float in the tile kernel, double in the long-run path (thousands of factors).
 template <int D, bool DUMP, typename TT>
-__device__ __forceinline__ void blend_pixel(const uint32_t* dk, const float4* R, PixLists L, uint32_t gofs_top,
+__device__ __forceinline__ void blend_pixel(const uint32_t* dk, const float4* Ra, const float4* Rf, PixLists L, uint32_t gofs_top,
                                             uint32_t gofs_bot, float* __restrict__ gT, float (&acc)[D], float& accA,
                                             uint4& consumed, uint32_t* __restrict__ sorted_idx,
                                             uint32_t* __restrict__ sorted_depth, uint32_t obase) {
-    constexpr int RV = 1 + D / 4;
+    constexpr int FV = D / 4;
     const uint32_t s0 = L.c0, s1 = L.c1, s2 = L.c2, s3 = L.c3;
     uint32_t c0 = L.c0, c1 = L.c1, c2 = L.c2, c3 = L.c3;
     uint32_t h0 = c0 < L.e0 ? dk[c0] : kSentHi, h1 = c1 < L.e1 ? dk[c1] : kSentHi;
@@ -86,14 +84,14 @@ __device__ __forceinline__ void blend_pixel(const uint32_t* dk, const float4* R,
         int j = h0 == m ? 0 : (h1 == m ? 1 : (h2 == m ? 2 : 3));
         if ((int)(h0 == m) + (int)(h1 == m) + (int)(h2 == m) + (int)(h3 == m) > 1) {
             uint32_t best = 0xFFFFFFFFu;                 // equal depth bits: ascending point index
-            if (h0 == m) { const uint32_t i = __float_as_uint(R[c0 * RV].w); if (i < best) { best = i; j = 0; } }
-            if (h1 == m) { const uint32_t i = __float_as_uint(R[c1 * RV].w); if (i < best) { best = i; j = 1; } }
-            if (h2 == m) { const uint32_t i = __float_as_uint(R[c2 * RV].w); if (i < best) { best = i; j = 2; } }
-            if (h3 == m) { const uint32_t i = __float_as_uint(R[c3 * RV].w); if (i < best) { best = i; j = 3; } }
+            if (h0 == m) { const uint32_t i = __float_as_uint(Ra[c0].w); if (i < best) { best = i; j = 0; } }
+            if (h1 == m) { const uint32_t i = __float_as_uint(Ra[c1].w); if (i < best) { best = i; j = 1; } }
+            if (h2 == m) { const uint32_t i = __float_as_uint(Ra[c2].w); if (i < best) { best = i; j = 2; } }
+            if (h3 == m) { const uint32_t i = __float_as_uint(Ra[c3].w); if (i < best) { best = i; j = 3; } }
         }
         const uint32_t ref = j == 0 ? c0 : (j == 1 ? c1 : (j == 2 ? c2 : c3));
         const uint32_t end = j == 0 ? L.e0 : (j == 1 ? L.e1 : (j == 2 ? L.e2 : L.e3));
-        const float4 r0 = R[ref * RV];                   // tx, ty, opacity, idx
+        const float4 r0 = Ra[ref];                   // tx, ty, opacity, idx
         if (blending) {
             const float wx = (j & 1) ? 1.f - r0.x : r0.x;       // lists 0, 2: corner dx = 1 (weight tx)
             const float wy = (j & 2) ? 1.f - r0.y : r0.y;       // lists 0, 1: corner dy = 1 (weight ty)
@@ -102,7 +100,7 @@ __device__ __forceinline__ void blend_pixel(const uint32_t* dk, const float4* R,
             accA += c;
 #pragma unroll
             for (int v = 0; v < D / 4; ++v) {
-                const float4 f = R[ref * RV + 1 + v];
+                const float4 f = Rf[ref * FV + v];
                 acc[4 * v] += c * f.x; acc[4 * v + 1] += c * f.y; acc[4 * v + 2] += c * f.z; acc[4 * v + 3] += c * f.w;
             }
             if (gT) gT[(size_t)(ref + ((j & 2) ? gofs_bot : gofs_top)) * 4 + (3 - j)] = (float)T;
@@ -123,10 +121,10 @@ __device__ __forceinline__ void blend_pixel(const uint32_t* dk, const float4* R,
 
 // Backward of one pixel: lists hold [start, start + consumed); gTa is indexed like dk (cursor * 4 + corner).
 template <int D, typename TT>
-__device__ __forceinline__ void backward_pixel(const uint32_t* dk, const float4* R, const float* gTa, PixLists L,
+__device__ __forceinline__ void backward_pixel(const uint32_t* dk, const float4* Ra, const float4* Rf, const float* gTa, PixLists L,
                                                uint32_t gofs_top, uint32_t gofs_bot, const float (&g)[D], float gA,
                                                float* __restrict__ gD) {
-    constexpr int RV = 1 + D / 4;
+    constexpr int FV = D / 4;
     // c_j = one past the last blended record of list j; L.c_j = its start
     uint32_t c0 = L.e0, c1 = L.e1, c2 = L.e2, c3 = L.e3;
     uint32_t t0 = c0 > L.c0 ? dk[c0 - 1] : 0u, t1 = c1 > L.c1 ? dk[c1 - 1] : 0u;
@@ -138,14 +136,14 @@ __device__ __forceinline__ void backward_pixel(const uint32_t* dk, const float4*
         int j = t0 == m ? 0 : (t1 == m ? 1 : (t2 == m ? 2 : 3));
         if ((int)(t0 == m) + (int)(t1 == m) + (int)(t2 == m) + (int)(t3 == m) > 1) {
             uint32_t best = 0u;                          // reverse order: descending point index
-            if (t0 == m) { const uint32_t i = __float_as_uint(R[(c0 - 1) * RV].w); if (i >= best) { best = i; j = 0; } }
-            if (t1 == m) { const uint32_t i = __float_as_uint(R[(c1 - 1) * RV].w); if (i >= best) { best = i; j = 1; } }
-            if (t2 == m) { const uint32_t i = __float_as_uint(R[(c2 - 1) * RV].w); if (i >= best) { best = i; j = 2; } }
-            if (t3 == m) { const uint32_t i = __float_as_uint(R[(c3 - 1) * RV].w); if (i >= best) { best = i; j = 3; } }
+            if (t0 == m) { const uint32_t i = __float_as_uint(Ra[c0 - 1].w); if (i >= best) { best = i; j = 0; } }
+            if (t1 == m) { const uint32_t i = __float_as_uint(Ra[c1 - 1].w); if (i >= best) { best = i; j = 1; } }
+            if (t2 == m) { const uint32_t i = __float_as_uint(Ra[c2 - 1].w); if (i >= best) { best = i; j = 2; } }
+            if (t3 == m) { const uint32_t i = __float_as_uint(Ra[c3 - 1].w); if (i >= best) { best = i; j = 3; } }
         }
         const uint32_t ref = (j == 0 ? c0 : (j == 1 ? c1 : (j == 2 ? c2 : c3))) - 1u;
         const uint32_t start = j == 0 ? L.c0 : (j == 1 ? L.c1 : (j == 2 ? L.c2 : L.c3));
-        const float4 r0 = R[ref * RV];
+        const float4 r0 = Ra[ref];
         const float T = gTa[(size_t)ref * 4 + (3 - j)];
         const float wx = (j & 1) ? 1.f - r0.x : r0.x;
         const float wy = (j & 2) ? 1.f - r0.y : r0.y;
@@ -153,7 +151,7 @@ __device__ __forceinline__ void backward_pixel(const uint32_t* dk, const float4*
         float G = gA;
 #pragma unroll
         for (int v = 0; v < D / 4; ++v) {
-            const float4 f = R[ref * RV + 1 + v];
+            const float4 f = Rf[ref * FV + v];
             G += f.x * g[4 * v] + f.y * g[4 * v + 1] + f.z * g[4 * v + 2] + f.w * g[4 * v + 3];
         }
         gD[(size_t)(ref + ((j & 2) ? gofs_bot : gofs_top)) * 4 + (3 - j)] = (float)((TT)T * ((TT)G - B));
@@ -166,12 +164,14 @@ __device__ __forceinline__ void backward_pixel(const uint32_t* dk, const float4*
 
 template <int D, int MODE>
 __global__ void __launch_bounds__(kTileThreads) k_tile(TileArgs A) {
-    constexpr int RV  = 1 + D / 4;                 // float4 per record
+    static_assert(MODE == kBwd, "the forward pass lives in blend.cuh");
+    constexpr int FV  = D / 4;                     // float4 of features per record
     constexpr int CAP = TileCfg<D>::kCap;
     extern __shared__ __align__(128) unsigned char smem[];
     uint32_t* s_dk = reinterpret_cast<uint32_t*>(smem);
-    float4*   s_r  = reinterpret_cast<float4*>(smem + (size_t)CAP * 4);
-    float*    s_gt = reinterpret_cast<float*>(smem + (size_t)CAP * 4 + (size_t)CAP * RV * 16);
+    float4*   s_a  = reinterpret_cast<float4*>(smem + (size_t)CAP * 4);
+    float4*   s_f  = reinterpret_cast<float4*>(smem + (size_t)CAP * 20);
+    float*    s_gt = reinterpret_cast<float*>(smem + (size_t)CAP * (20 + 16 * FV));
 
     __shared__ uint32_t s_off[kTileH + 1][kTileW + 2];
     __shared__ uint32_t s_sbase[kTileH + 1], s_a4[kTileH + 1];
@@ -195,7 +195,6 @@ __global__ void __launch_bounds__(kTileThreads) k_tile(TileArgs A) {
         const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
         const int tw = 1 << lw, th = 1 << lh;
 
-        // cell offsets of the tile's (th+1) x (tw+2) window
         for (int e = tid; e < (th + 1) * (tw + 2); e += kTileThreads) {
             const int r = e / (tw + 2), c = e - r * (tw + 2);
             const int j = Y + r;
@@ -215,27 +214,26 @@ __global__ void __launch_bounds__(kTileThreads) k_tile(TileArgs A) {
             s_tot = tot;
             if (tot > 0) {
                 fence_proxy_async();
-                mbar_arrive_expect_tx(&s_bar, tot * (uint32_t)(4 + RV * 16 + (MODE == kBwd ? 16 : 0)));
+                mbar_arrive_expect_tx(&s_bar, tot * (uint32_t)(4 + 16 + 16 * FV + 16));
                 for (int r = 0; r <= th; ++r) {
                     const uint32_t a = s_off[r][0], b = s_off[r][tw + 1];
                     if (b <= a) continue;
                     const uint32_t a4 = s_a4[r], len = ((b + 3u) & ~3u) - a4, sb = s_sbase[r];
                     bulk_g2s(s_dk + sb, A.dk + a4, len * 4, &s_bar);
-                    bulk_g2s(s_r + (size_t)sb * RV, A.R + (size_t)a4 * RV, len * RV * 16, &s_bar);
-                    if (MODE == kBwd) bulk_g2s(s_gt + (size_t)sb * 4, A.gT + (size_t)a4 * 4, len * 16, &s_bar);
+                    bulk_g2s(s_a + sb, A.Ra + a4, len * 16, &s_bar);
+                    bulk_g2s(s_f + (size_t)sb * FV, A.Rf + (size_t)a4 * FV, len * FV * 16, &s_bar);
+                    bulk_g2s(s_gt + (size_t)sb * 4, A.gT + (size_t)a4 * 4, len * 16, &s_bar);
                 }
             }
         }
         __syncthreads();
         if (s_tot > 0) { mbar_wait(&s_bar, parity); parity ^= 1u; }
 
-        // ---------------------------------------------------------------- one thread per pixel
         const int q = tid;
         const int ly = q >> lw, lx = q & (tw - 1);
         const int x = X + lx, y = Y + ly;
         if (q >= tw * th || x >= W || y >= H) continue;
         const size_t pix = (size_t)y * W + x;
-        // smem index of global slot g in cell row r: g + (s_sbase[r] - s_a4[r])
         const uint32_t bt = s_sbase[ly] - s_a4[ly], bb = s_sbase[ly + 1] - s_a4[ly + 1];
         PixLists L;
         L.c0 = s_off[ly][lx] + bt;         L.e0 = s_off[ly][lx + 1] + bt;
@@ -243,29 +241,16 @@ __global__ void __launch_bounds__(kTileThreads) k_tile(TileArgs A) {
         L.c2 = s_off[ly + 1][lx] + bb;     L.e2 = s_off[ly + 1][lx + 1] + bb;
         L.c3 = L.e2;                       L.e3 = s_off[ly + 1][lx + 2] + bb;
 
-        if (MODE != kBwd) {
-            float acc[D]; float accA;
-            uint4 consumed = make_uint4(0, 0, 0, 0);
-            const uint32_t obase = (MODE == kFwdDump) ? A.pixoff[pix] : 0u;
-            blend_pixel<D, MODE == kFwdDump, float>(s_dk, s_r, L, 0u - bt, 0u - bb, A.gT, acc, accA, consumed,
-                                                    A.sorted_idx, A.sorted_depth, obase);
+        const uint4 consumed = A.pcur[pix];
+        L.e0 = L.c0 + consumed.x; L.e1 = L.c1 + consumed.y; L.e2 = L.c2 + consumed.z; L.e3 = L.c3 + consumed.w;
+        float g[D];
 #pragma unroll
-            for (int v = 0; v < D / 4; ++v)
-                reinterpret_cast<float4*>(A.out_feat + pix * D)[v] = make_float4(acc[4 * v], acc[4 * v + 1], acc[4 * v + 2], acc[4 * v + 3]);
-            A.out_alpha[pix] = accA;
-            if (A.gT) A.pcur[pix] = consumed;
-        } else {
-            const uint4 consumed = A.pcur[pix];
-            L.e0 = L.c0 + consumed.x; L.e1 = L.c1 + consumed.y; L.e2 = L.c2 + consumed.z; L.e3 = L.c3 + consumed.w;
-            float g[D];
-#pragma unroll
-            for (int v = 0; v < D / 4; ++v) {
-                const float4 t = __ldg(reinterpret_cast<const float4*>(A.g_feat + pix * D) + v);
-                g[4 * v] = t.x; g[4 * v + 1] = t.y; g[4 * v + 2] = t.z; g[4 * v + 3] = t.w;
-            }
-            const float gA = A.g_alpha ? __ldg(A.g_alpha + pix) : 0.f;
-            backward_pixel<D, float>(s_dk, s_r, s_gt, L, 0u - bt, 0u - bb, g, gA, A.gD);
+        for (int v = 0; v < D / 4; ++v) {
+            const float4 t = __ldg(reinterpret_cast<const float4*>(A.g_feat + pix * D) + v);
+            g[4 * v] = t.x; g[4 * v + 1] = t.y; g[4 * v + 2] = t.z; g[4 * v + 3] = t.w;
         }
+        const float gA = A.g_alpha ? __ldg(A.g_alpha + pix) : 0.f;
+        backward_pixel<D, float>(s_dk, s_a, s_f, s_gt, L, 0u - bt, 0u - bb, g, gA, A.gD);
     }
 }
 
