@@ -14,6 +14,7 @@
 
 #include "bin.cuh"
 #include "big.cuh"
+#include "back.cuh"
 #include "blend.cuh"
 #include "cellsort.cuh"
 #include "common.cuh"
@@ -165,19 +166,19 @@ static int persistent_grid(K kernel, int threads, size_t smem, int sms, int* out
     return INPC_OK;
 }
 
-template <int D, int MODE>
-static int launch_tile(const TileArgs& A, int sms, cudaStream_t st) {
-    constexpr size_t smem = tile_smem_bytes<D, MODE>();
+template <int D>
+static int launch_back(const BackArgs& A, int sms, cudaStream_t st) {
+    constexpr size_t smem = back_smem_bytes<D>();
     static bool configured = false;
     static int grid = 0;
     if (!configured) {
-        INPC_CUDA(cudaFuncSetAttribute(k_tile<D, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int rc = persistent_grid(k_tile<D, MODE>, kTileThreads, smem, sms, &grid);
+        INPC_CUDA(cudaFuncSetAttribute(k_back<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int rc = persistent_grid(k_back<D>, kTileThreads, smem, sms, &grid);
         if (rc != INPC_OK) return rc;
         configured = true;
     }
-    { StageTimer tm(MODE == kBwd ? kStTileBwd : kStTileFwd, st);
-      k_tile<D, MODE><<<grid, kTileThreads, smem, st>>>(A); }
+    { StageTimer tm(kStTileBwd, st);
+      k_back<D><<<grid, kTileThreads, smem, st>>>(A); }
     INPC_LAUNCHED();
     return INPC_OK;
 }
@@ -337,11 +338,11 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     float* gD = reinterpret_cast<float*>(ws + L.gD);
     uint4* pcur = reinterpret_cast<uint4*>(ws + L.pcur);
     float* gpt = reinterpret_cast<float*>(ws + L.gpt);
-    TileArgs A{};
+    BackArgs A{};
     A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = reinterpret_cast<uint32_t*>(ws + L.items);
     A.celloff = celloff; A.dk = reinterpret_cast<uint32_t*>(ws + L.dk); A.Ra = Ra; A.Rf = Rf;
     A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD;
-    int rc = launch_tile<D, kBwd>(A, di.sms, st);
+    int rc = launch_back<D>(A, di.sms, st);
     if (rc != INPC_OK) return rc;
     BigArgs B{};
     B.hdr = hdr; B.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); B.celloff = celloff; B.dk = A.dk; B.Ra = Ra; B.Rf = Rf;

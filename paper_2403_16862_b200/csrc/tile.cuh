@@ -47,9 +47,6 @@ struct TileArgs {
     float* gD;
 };
 
-template <int D, int MODE> __host__ __device__ constexpr size_t tile_smem_bytes() {
-    return (size_t)TileCfg<D>::kCap * (4 + 16 + 4 * D + 16);       // dk, Ra, Rf, staged gT
-}
 
 // The four lists of one pixel as cursors into dk / R (shared-memory indices in the tile kernel, global
 // slots in the long-run path).  Lists 0, 1 lie in cell row y, lists 2, 3 in cell row y+1.
@@ -159,98 +156,6 @@ __device__ __forceinline__ void backward_pixel(const uint32_t* dk, const float4*
         const uint32_t nt = ref > start ? dk[ref - 1] : 0u;
         if (j == 0) { c0 = ref; t0 = nt; } else if (j == 1) { c1 = ref; t1 = nt; }
         else if (j == 2) { c2 = ref; t2 = nt; } else { c3 = ref; t3 = nt; }
-    }
-}
-
-template <int D, int MODE>
-__global__ void __launch_bounds__(kTileThreads) k_tile(TileArgs A) {
-    static_assert(MODE == kBwd, "the forward pass lives in blend.cuh");
-    constexpr int FV  = D / 4;                     // float4 of features per record
-    constexpr int CAP = TileCfg<D>::kCap;
-    extern __shared__ __align__(128) unsigned char smem[];
-    uint32_t* s_dk = reinterpret_cast<uint32_t*>(smem);
-    float4*   s_a  = reinterpret_cast<float4*>(smem + (size_t)CAP * 4);
-    float4*   s_f  = reinterpret_cast<float4*>(smem + (size_t)CAP * 20);
-    float*    s_gt = reinterpret_cast<float*>(smem + (size_t)CAP * (20 + 16 * FV));
-
-    __shared__ uint32_t s_off[kTileH + 1][kTileW + 2];
-    __shared__ uint32_t s_sbase[kTileH + 1], s_a4[kTileH + 1];
-    __shared__ uint32_t s_item, s_tot;
-    __shared__ __align__(8) uint64_t s_bar;
-
-    const int tid = threadIdx.x;
-    const int W = A.W, H = A.H;
-    const uint32_t n_items = A.hdr->n_items;
-
-    if (tid == 0) { mbar_init(&s_bar, 1); fence_mbar_init(); }
-    uint32_t parity = 0;
-
-    while (true) {
-        __syncthreads();                                  // everyone is done with the previous item's smem
-        if (tid == 0) s_item = atomicAdd(A.item_cursor, 1u);
-        __syncthreads();
-        const uint32_t item_i = s_item;
-        if (item_i >= n_items) break;
-        const uint32_t it = A.items[item_i];
-        const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
-        const int tw = 1 << lw, th = 1 << lh;
-
-        for (int e = tid; e < (th + 1) * (tw + 2); e += kTileThreads) {
-            const int r = e / (tw + 2), c = e - r * (tw + 2);
-            const int j = Y + r;
-            uint32_t v = 0;
-            if (j <= H) v = __ldg(&A.celloff[(uint32_t)j * (W + 1) + min(X + c, W + 1)]);
-            s_off[r][c] = v;
-        }
-        __syncthreads();
-        if (tid == 0) {
-            uint32_t tot = 0;
-            for (int r = 0; r <= th; ++r) {
-                const uint32_t a = s_off[r][0], b = s_off[r][tw + 1];
-                const uint32_t a4 = a & ~3u, b4 = (b + 3u) & ~3u;
-                s_a4[r] = a4; s_sbase[r] = tot;
-                tot += (b > a) ? (b4 - a4) : 0u;
-            }
-            s_tot = tot;
-            if (tot > 0) {
-                fence_proxy_async();
-                mbar_arrive_expect_tx(&s_bar, tot * (uint32_t)(4 + 16 + 16 * FV + 16));
-                for (int r = 0; r <= th; ++r) {
-                    const uint32_t a = s_off[r][0], b = s_off[r][tw + 1];
-                    if (b <= a) continue;
-                    const uint32_t a4 = s_a4[r], len = ((b + 3u) & ~3u) - a4, sb = s_sbase[r];
-                    bulk_g2s(s_dk + sb, A.dk + a4, len * 4, &s_bar);
-                    bulk_g2s(s_a + sb, A.Ra + a4, len * 16, &s_bar);
-                    bulk_g2s(s_f + (size_t)sb * FV, A.Rf + (size_t)a4 * FV, len * FV * 16, &s_bar);
-                    bulk_g2s(s_gt + (size_t)sb * 4, A.gT + (size_t)a4 * 4, len * 16, &s_bar);
-                }
-            }
-        }
-        __syncthreads();
-        if (s_tot > 0) { mbar_wait(&s_bar, parity); parity ^= 1u; }
-
-        const int q = tid;
-        const int ly = q >> lw, lx = q & (tw - 1);
-        const int x = X + lx, y = Y + ly;
-        if (q >= tw * th || x >= W || y >= H) continue;
-        const size_t pix = (size_t)y * W + x;
-        const uint32_t bt = s_sbase[ly] - s_a4[ly], bb = s_sbase[ly + 1] - s_a4[ly + 1];
-        PixLists L;
-        L.c0 = s_off[ly][lx] + bt;         L.e0 = s_off[ly][lx + 1] + bt;
-        L.c1 = L.e0;                       L.e1 = s_off[ly][lx + 2] + bt;
-        L.c2 = s_off[ly + 1][lx] + bb;     L.e2 = s_off[ly + 1][lx + 1] + bb;
-        L.c3 = L.e2;                       L.e3 = s_off[ly + 1][lx + 2] + bb;
-
-        const uint4 consumed = A.pcur[pix];
-        L.e0 = L.c0 + consumed.x; L.e1 = L.c1 + consumed.y; L.e2 = L.c2 + consumed.z; L.e3 = L.c3 + consumed.w;
-        float g[D];
-#pragma unroll
-        for (int v = 0; v < D / 4; ++v) {
-            const float4 t = __ldg(reinterpret_cast<const float4*>(A.g_feat + pix * D) + v);
-            g[4 * v] = t.x; g[4 * v + 1] = t.y; g[4 * v + 2] = t.z; g[4 * v + 3] = t.w;
-        }
-        const float gA = A.g_alpha ? __ldg(A.g_alpha + pix) : 0.f;
-        backward_pixel<D, float>(s_dk, s_a, s_f, s_gt, L, 0u - bt, 0u - bb, g, gA, A.gD);
     }
 }
 
