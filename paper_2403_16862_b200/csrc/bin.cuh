@@ -45,16 +45,24 @@ __global__ void __launch_bounds__(kBinThreads) k_project_count(const float* __re
         __syncthreads();
         stage_positions(pos, base, N, s_pos);
         __syncthreads();
+        // all projections, then all atomics, then all stores: kBinPPT atomics in flight per thread
+        int cell[kBinPPT];
+        uint32_t r[kBinPPT];
 #pragma unroll
         for (int k = 0; k < kBinPPT; ++k) {
             const int l = k * kBinThreads + threadIdx.x;
-            const long long i = base + l;
-            if (i < N) {
-                const Proj p = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]);
-                uint32_t r = 0xFFFFFFFFu;
-                if (p.cell >= 0) r = atomicAdd(&cellcnt[p.cell], 1u);
-                __stcs(&rank[i], r);
-            }
+            cell[k] = -1;
+            if (base + l < N) cell[k] = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]).cell;
+        }
+#pragma unroll
+        for (int k = 0; k < kBinPPT; ++k) {
+            r[k] = 0xFFFFFFFFu;
+            if (cell[k] >= 0) r[k] = atomicAdd(&cellcnt[cell[k]], 1u);
+        }
+#pragma unroll
+        for (int k = 0; k < kBinPPT; ++k) {
+            const long long i = base + k * kBinThreads + threadIdx.x;
+            if (i < N) __stcs(&rank[i], r[k]);
         }
     }
 }
@@ -72,25 +80,41 @@ __global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict
         __syncthreads();
         stage_positions(pos, base, N, s_pos);
         __syncthreads();
+        // ranks (coalesced), projections, then all celloff gathers and opacity loads in flight, then the stores
+        uint32_t r[kBinPPT], off[kBinPPT];
+        float op[kBinPPT];
+        Proj p[kBinPPT];
+#pragma unroll
+        for (int k = 0; k < kBinPPT; ++k) {
+            const long long i = base + k * kBinThreads + threadIdx.x;
+            r[k] = i < N ? __ldcs(&rank[i]) : 0xFFFFFFFFu;
+        }
 #pragma unroll
         for (int k = 0; k < kBinPPT; ++k) {
             const int l = k * kBinThreads + threadIdx.x;
-            const long long i = base + l;
-            if (i >= N) continue;
-            const uint32_t r = __ldcs(&rank[i]);
-            if (r == 0xFFFFFFFFu) continue;
-            const Proj p = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]);
-            const uint32_t slot = __ldg(&celloff[p.cell]) + r;
+            p[k] = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]);
+        }
+#pragma unroll
+        for (int k = 0; k < kBinPPT; ++k) {
+            const bool live = r[k] != 0xFFFFFFFFu;
+            off[k] = live ? __ldg(&celloff[p[k].cell]) : 0u;
+            op[k] = live ? __ldcs(&opacity[base + k * kBinThreads + threadIdx.x]) : 0.f;
+        }
+#pragma unroll
+        for (int k = 0; k < kBinPPT; ++k) {
+            if (r[k] == 0xFFFFFFFFu) continue;
+            const long long i = base + k * kBinThreads + threadIdx.x;
+            const size_t slot = (size_t)off[k] + r[k];
             float4 a0, a1;
-            a0.x = __uint_as_float(p.depth_bits);
+            a0.x = __uint_as_float(p[k].depth_bits);
             a0.y = __uint_as_float((uint32_t)i);
-            a0.z = p.tx;
-            a0.w = p.ty;
-            a1.x = __ldcs(&opacity[i]);
-            a1.y = __uint_as_float((uint32_t)p.cell);
+            a0.z = p[k].tx;
+            a0.w = p[k].ty;
+            a1.x = op[k];
+            a1.y = __uint_as_float((uint32_t)p[k].cell);
             a1.z = 0.f; a1.w = 0.f;
-            A[2 * (size_t)slot] = a0;
-            A[2 * (size_t)slot + 1] = a1;
+            A[2 * slot] = a0;
+            A[2 * slot + 1] = a1;
         }
     }
 }

@@ -48,8 +48,22 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
             const uint32_t cell = c0 + lo, r = slot - s_off[lo];
             const int j = cell / (W + 1), i = cell - j * (W + 1);
             const int x0 = i - 1, y0 = j - 1;
-            const float4 r0 = __ldg(&Ra[slot]);       // tx, ty, opacity, idx
+            const float4 r0 = __ldg(&Ra[slot]);                   // tx, ty, opacity, idx
             const float4 t4 = __ldcs(&gT[slot]), d4 = __ldcs(&gD[slot]);
+            // every gather of the four corner pixels is issued before any of them is used
+            uint4 cur[4];
+            float4 gp[4][D / 4];
+            bool in[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int px = x0 + (c & 1), py = y0 + (c >> 1);
+                in[c] = px >= 0 && px < W && py >= 0 && py < H;               // else: fragment does not exist
+                const size_t pp = in[c] ? (size_t)py * W + px : 0;
+                cur[c] = in[c] ? __ldg(&pcur[pp]) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+                for (int v = 0; v < D / 4; ++v)
+                    gp[c][v] = in[c] ? __ldg(reinterpret_cast<const float4*>(g_feat + pp * D) + v) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
             const float tc[4] = {t4.x, t4.y, t4.z, t4.w}, dc[4] = {d4.x, d4.y, d4.z, d4.w};
             float df[D];
 #pragma unroll
@@ -58,12 +72,8 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const int dx = c & 1, dy = c >> 1;
-                const int px = x0 + dx, py = y0 + dy;
-                if (px < 0 || px >= W || py < 0 || py >= H) continue;      // fragment does not exist
-                const size_t pp = (size_t)py * W + px;
-                const uint4 cur = __ldg(&pcur[pp]);
-                const uint32_t lim = c == 3 ? cur.x : (c == 2 ? cur.y : (c == 1 ? cur.z : cur.w));   // list 3 - c
-                if (r >= lim) continue;                                    // behind the cut-off: exactly 0
+                const uint32_t lim = c == 3 ? cur[c].x : (c == 2 ? cur[c].y : (c == 1 ? cur[c].z : cur[c].w));   // list 3 - c
+                if (!in[c] || r >= lim) continue;                          // behind the cut-off: exactly 0
                 const float wx = dx ? r0.x : 1.f - r0.x, wy = dy ? r0.y : 1.f - r0.y;
                 const float Ta = tc[c] * (r0.z * (wx * wy));
                 const float dl = dc[c];
@@ -72,7 +82,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
                 dv += (dy ? wx : -wx) * dl;
 #pragma unroll
                 for (int v = 0; v < D / 4; ++v) {
-                    const float4 t = __ldg(reinterpret_cast<const float4*>(g_feat + pp * D) + v);
+                    const float4 t = gp[c][v];
                     df[4 * v] += Ta * t.x; df[4 * v + 1] += Ta * t.y; df[4 * v + 2] += Ta * t.z; df[4 * v + 3] += Ta * t.w;
                 }
             }
