@@ -63,24 +63,25 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
     __shared__ uint32_t s_sbase[kTileH + 1], s_a4row[kTileH + 1];
     __shared__ uint32_t s_hist[64];
     __shared__ uint8_t  s_perm[kTileThreads];
-    __shared__ uint32_t s_item, s_tot;
+    __shared__ uint32_t s_next, s_next_code, s_tot;
     __shared__ __align__(8) uint64_t s_bar;
 
     const int tid = threadIdx.x;
     const int W = A.W, H = A.H;
     const uint32_t n_items = A.hdr->n_items;
 
-    if (tid == 0) { mbar_init(&s_bar, 1); fence_mbar_init(); }
+    if (tid == 0) {
+        mbar_init(&s_bar, 1); fence_mbar_init();
+        const uint32_t nx = atomicAdd(A.item_cursor, 1u);
+        s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
+    }
     uint32_t parity = 0;
 
     while (true) {
         __syncthreads();                                  // everyone is done with the previous item's smem
-        if (tid == 0) s_item = atomicAdd(A.item_cursor, 1u);
-        if (tid < 64) s_hist[tid] = 0;
-        __syncthreads();
-        const uint32_t item_i = s_item;
+        const uint32_t item_i = s_next;
         if (item_i >= n_items) break;
-        const uint32_t it = A.items[item_i];
+        const uint32_t it = s_next_code;
         const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
         const int tw = 1 << lw, th = 1 << lh;
 
@@ -92,27 +93,36 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
             if (j <= H) v = __ldg(&A.celloff[(uint32_t)j * (W + 1) + min(X + c, W + 1)]);
             s_off[r][c] = v;
         }
+        if (tid < 64) s_hist[tid] = 0;
         __syncthreads();
-        if (tid == 0) {
-            uint32_t tot = 0;
-            for (int r = 0; r <= th; ++r) {
-                const uint32_t a = s_off[r][0], b = s_off[r][tw + 1];
-                const uint32_t a4 = a & ~3u, b4 = (b + 3u) & ~3u;
-                s_a4row[r] = a4; s_sbase[r] = tot;
-                tot += (b > a) ? (b4 - a4) : 0u;
+        if (tid == 32) {                                  // fetch the next work item while this one is processed
+            const uint32_t nx = atomicAdd(A.item_cursor, 1u);
+            s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
+        }
+        if (tid < 32) {                                   // warp 0: one lane per cell row issues that row's copies
+            const bool row = tid <= th;
+            uint32_t a4 = 0, len = 0;
+            if (row) {
+                const uint32_t a = s_off[tid][0], b = s_off[tid][tw + 1];
+                a4 = a & ~3u;
+                len = b > a ? ((b + 3u) & ~3u) - a4 : 0u;
             }
-            s_tot = tot;
-            if (tot > 0) {
-                fence_proxy_async();
-                mbar_arrive_expect_tx(&s_bar, tot * (uint32_t)(4 + 16 + 16 * FV));
-                for (int r = 0; r <= th; ++r) {
-                    const uint32_t a = s_off[r][0], b = s_off[r][tw + 1];
-                    if (b <= a) continue;
-                    const uint32_t a4 = s_a4row[r], len = ((b + 3u) & ~3u) - a4, sb = s_sbase[r];
-                    bulk_g2s(s_dk + sb, A.dk + a4, len * 4, &s_bar);
-                    bulk_g2s(s_a4 + sb, A.Ra + a4, len * 16, &s_bar);
-                    bulk_g2s(s_f + (size_t)sb * FV, A.Rf + (size_t)a4 * FV, len * FV * 16, &s_bar);
-                }
+            uint32_t inc = len;
+#pragma unroll
+            for (int d = 1; d < 16; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d); if (tid >= d) inc += t; }
+            const uint32_t sb = inc - len;
+            const uint32_t tot = __shfl_sync(0xffffffffu, inc, 15);
+            if (row) { s_a4row[tid] = a4; s_sbase[tid] = sb; }
+            fence_proxy_async();
+            if (tid == 0) {
+                s_tot = tot;
+                if (tot > 0) mbar_arrive_expect_tx(&s_bar, tot * (uint32_t)(4 + 16 + 16 * FV));
+            }
+            __syncwarp();
+            if (len) {
+                bulk_g2s(s_dk + sb, A.dk + a4, len * 4, &s_bar);
+                bulk_g2s(s_a4 + sb, A.Ra + a4, len * 16, &s_bar);
+                bulk_g2s(s_f + (size_t)sb * FV, A.Rf + (size_t)a4 * FV, len * FV * 16, &s_bar);
             }
         }
         // while the copies fly: this thread's pixel, its fragment count, and the count histogram
