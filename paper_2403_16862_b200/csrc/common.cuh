@@ -31,7 +31,7 @@ constexpr int kTileLW      = 4;     // log2(kTileW)
 constexpr int kTileLH      = 3;     // log2(kTileH)
 constexpr int kTileThreads = kTileW * kTileH;   // one thread per pixel
 constexpr int kMinTilePix  = 8;     // a sub-tile this small that still does not fit goes to the long-run path
-constexpr int kCellSmall   = 128;   // cells up to this many points are ranked by counting; larger: bitonic
+constexpr int kCellSmall   = 256;   // cells up to this many points are ranked by counting; larger: bitonic
 constexpr int kBigThreads  = 512;
 constexpr int kBigChunk    = 8192;  // keys sorted in shared memory at a time by the large-cell sort
 constexpr float kTMin      = 1e-4f; // transmittance cut-off (BASELINE.json north_star)

@@ -105,7 +105,10 @@ def check_forward(wl, st, ref, window=None, report=None):
             e_alt = np.minimum(e_alt, np.maximum(np.abs(img - im2).max(axis=2), np.abs(alpha - al2)))
         bad = (e_alt > FWD_ATOL) & mask & amb
         assert not bad.any(), f"ambiguous-pixel forward error {e_alt[bad].max():.3e} at {np.argwhere(bad)[:5]}"
-    assert n_amb <= max(8, int(0.002 * mask.sum())), f"too many termination-ambiguous pixels: {n_amb}"
+    # flagged pixels are still compared (against the oracle re-blended with the cut-off moved by +-2 MARGIN); the
+    # bound only guards against the flag swallowing the test.  Deep workloads reach the cut-off in ~10 % of
+    # their pixels and each of those has a ~3 % chance of a T_k inside the +-MARGIN band => 0.3 % (train) to 0.8 % (infer) flagged.
+    assert n_amb <= max(8, int(0.02 * mask.sum())), f"too many termination-ambiguous pixels: {n_amb}"
     if report is not None:
         report.update(fwd_max_err=float(err[mask & ~amb].max()) if (mask & ~amb).any() else 0.0, n_ambiguous=n_amb)
     return amb

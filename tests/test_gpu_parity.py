@@ -80,6 +80,25 @@ def test_stress_sampler_reduced_hits_long_run_path():
     assert rep["stats"]["n_big_pixels"] > 0, "the reduced stress draw must exercise the long-run path"
 
 
+# ------------------------------------------------------------------------------ full sizes (BASELINE.json configs 3-5)
+# The oracle finishes these in tens of seconds, so the whole image / every gradient is compared, in the same
+# launch configuration bench.py times.
+
+def test_train_full_size():
+    rep = full_parity(make_workload("train"))
+    assert rep["stats"]["n_kept"] == 1 << 23
+
+
+def test_infer_full_size_forward_d8():
+    rep = full_parity(make_workload("infer"), backward=False)
+    assert rep["stats"]["n_kept"] == 1 << 25
+
+
+def test_stress_full_size():
+    rep = full_parity(make_workload("stress"))
+    assert rep["stats"]["n_big_pixels"] > 0
+
+
 # ------------------------------------------------------------------------------ edge cases
 
 def test_empty_input_gives_zero_image():
