@@ -43,8 +43,11 @@ L2_BYTES = 126 * 1024 * 1024
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/; the file named in NCU_TRAFFIC_SOURCE).  None until a capture exists for that kernel.
-NCU_TRAFFIC = {}
-NCU_TRAFFIC_SOURCE = None
+NCU_TRAFFIC = {   # bytes per launch, train workload
+    "k_project_count": 115.2e6, "k_scatter": 424.7e6, "k_cellsort": 1203.3e6, "k_blend": 632.0e6,
+    "k_back": 809.7e6, "k_combine": 746.8e6, "k_split": 492.9e6,
+}
+NCU_TRAFFIC_SOURCE = "profiles/r01_v3_blend_back.md (ncu --set full, train workload; k_cellsort from r01_v2_cellsort_merge.md)"
 
 
 # ------------------------------------------------------------------------------------------------
@@ -54,17 +57,20 @@ def algorithmic_bytes(n_points: int, n_frag: int, n_pix: int, D: int) -> dict:
     a12 = 24 * n_points + 8 * n_frag + 12 * n_pix                       # a1 + a2: project, count, scan, emit
     a34 = (8 + 4 + F) * n_frag + 4 * (D + 1) * n_pix                    # a3 + a4: sort + blend
     a5 = (8 + 4 + F + 8) * n_frag + (8 * (D + 1) + 8) * n_pix + (F + 12) * n_points   # a5: backward
-    return {"a1_a2": a12, "a3_a4": a34, "a5": a5, "fwd": a12 + a34, "bwd": a5, "fwd_bwd": a12 + a34 + a5}
+    a5_walk = (8 + 4 + F + 8) * n_frag + (8 * (D + 1) + 8) * n_pix       # reverse traversal (k_back, k_big<bwd>)
+    a5_out = (F + 12) * n_points                                         # per-point gradients (k_combine, k_split)
+    return {"a1_a2": a12, "a3_a4": a34, "a5": a5, "a5_walk": a5_walk, "a5_out": a5_out,
+            "fwd": a12 + a34, "bwd": a5, "fwd_bwd": a12 + a34 + a5}
 
 
 # which path rows each library stage belongs to (for the per-kernel roofline)
 STAGE_ROWS = {
-    "k_tile_fwd": "a3_a4", "k_big_fwd": "a3_a4",
-    "k_tile_bwd": "a5", "k_big_bwd": "a5", "zero_bwd": "a5",
+    "k_blend": "a3_a4", "k_big_fwd": "a3_a4",
+    "k_back": "a5_walk", "k_big_bwd": "a5_walk", "zero_bwd": "a5_walk",
     "zero_fwd": "a1_a2", "k_project_count": "a1_a2", "k_scan_u32": "a1_a2", "k_scatter": "a1_a2",
     "k_classify": "a1_a2", "k_build_items": "a1_a2",
     "k_cellsort": "a3_a4", "k_cellsort_big": "a3_a4",
-    "k_combine": "a5", "k_split": "a5", "other": "a1_a2",
+    "k_combine": "a5_out", "k_split": "a5_out", "other": "a1_a2",
 }
 
 
@@ -383,10 +389,12 @@ def run_ours(args) -> int:
     kernels = {k: v for k, v in step_stage_ms.items() if k.startswith("k_")}
     dom = max(kernels, key=kernels.get)
     rows = STAGE_ROWS[dom]
-    achieved = alg[rows] / (per_stage[dom] * 1e-3) / 1e9
+    group_ms = sum(v for k, v in per_stage.items() if STAGE_ROWS.get(k) == rows)    # every kernel sharing these rows
+    achieved = alg[rows] / (group_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "rows": rows, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg[rows], "ms_per_launch": per_stage[dom],
+                "ms_rows": group_ms, "kernels_of_rows": sorted(k for k in per_stage if STAGE_ROWS.get(k) == rows and per_stage[k] > 0),
                 "share_of_step": kernels[dom] / sum(step_stage_ms.values()),
                 "traffic": NCU_TRAFFIC.get(dom), "traffic_source": NCU_TRAFFIC_SOURCE}
     ach_step = alg["fwd_bwd"] / (ms_step * 1e-3) / 1e9

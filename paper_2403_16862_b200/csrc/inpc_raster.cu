@@ -33,7 +33,7 @@ enum Stage { kStZeroFwd = 0, kStProjectCount, kStScan, kStScatter, kStClassify, 
              kStTileFwd, kStBigFwd, kStZeroBwd, kStTileBwd, kStBigBwd, kStCombine, kStSplit, kStOther, kNumStages };
 static const char* const kStageNames[kNumStages] = {
     "zero_fwd", "k_project_count", "k_scan_u32", "k_scatter", "k_classify", "k_cellsort", "k_cellsort_big", "k_build_items",
-    "k_tile_fwd", "k_big_fwd", "zero_bwd", "k_tile_bwd", "k_big_bwd", "k_combine", "k_split", "other"};
+    "k_blend", "k_big_fwd", "zero_bwd", "k_back", "k_big_bwd", "k_combine", "k_split", "other"};
 struct Pending { int stage; cudaEvent_t a, b; };
 static std::mutex g_tmu;
 static bool g_timing = false;
