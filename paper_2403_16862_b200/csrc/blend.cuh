@@ -179,11 +179,14 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
         float accA = 0.f, T = 1.f;
         uint4 consumed = make_uint4(0, 0, 0, 0);
         if constexpr (!DUMP) {
-            // Software-pipelined: iteration k SELECTS fragment k and issues its shared-memory loads (alpha,
-            // features, the list's next head key), then BLENDS fragment k-1 while those loads are in flight.
-            // Fragment k is blended iff T_k >= 1e-4, T_k being the transmittance after fragment k-1: the
-            // check sits between the blend of k-1 and the advance of k's list, so the cursors count exactly
-            // the blended fragments.
+            // Software-pipelined, ONE basic block and ONE backward branch per fragment: iteration k selects
+            // fragment k (predicates from the minimum head key), issues its shared-memory loads (alpha, features,
+            // the list's next head key), blends fragment k-1 while they are in flight, advances the list and
+            // recomputes minimum / list predicates / tie flag; the three exit conditions are tested together:
+            // lists exhausted, two heads with equal depth bits (resolved by point index in the outer loop), and
+            // the cut-off -- fragment k+1 is blended iff T_{k+1} = T_k (1 - a_k) >= 1e-4, known as soon as a_k
+            // has arrived.  Entering the body therefore means "fragment k will be blended": the cursors count
+            // exactly the blended fragments.
             float pa = 0.f;                               // pending fragment: alpha, features, gT address
             float4 pf[FV];
 #pragma unroll
@@ -191,9 +194,10 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
             float* pg = nullptr;
             bool have = false;
             uint32_t m = min(min(h0, h1), min(h2, h3));
-            while (m != kSentHi) {
-                bool p0 = h0 == m, p1 = h1 == m, p2 = h2 == m, p3 = h3 == m;
-                if ((p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3)) {
+            bool p0 = h0 == m, p1 = h1 == m, p2 = h2 == m, p3 = h3 == m;
+            bool tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
+            while (m != kSentHi && !(T * (1.f - pa) < kTMin)) {
+                if (tie) {
                     uint32_t best = 0xFFFFFFFFu;          // equal depth bits: ascending point index
                     int jb = 0;
                     if (p0) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce0 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 0; } }
@@ -202,35 +206,38 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
                     if (p3) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce3 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 3; } }
                     p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;
                 }
-                const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
-                const uint32_t cur = ce & 0xffffu;
-                const uint32_t nx = ce + 16u;
-                const uint32_t nc = nx & 0xffffu;
-                // issue the loads of fragment k
-                const float na = *reinterpret_cast<const float*>(s_ab + cur);
-                float4 nf[FV];
+                do {
+                    const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
+                    const uint32_t cur = ce & 0xffffu;
+                    const uint32_t nx = ce + 16u;
+                    const uint32_t nc = nx & 0xffffu;
+                    // issue the loads of fragment k
+                    const float na = *reinterpret_cast<const float*>(s_ab + cur);
+                    float4 nf[FV];
 #pragma unroll
-                for (int v = 0; v < FV; ++v) nf[v] = s_f[(cur >> 4) * FV + v];
-                const uint32_t nh = nc < (nx >> 16) ? s_dk[nc >> 4] : kSentHi;
-                float* ng = ((p0 | p1) ? gTtop : gTbot) + (cur >> 2);
-                // blend fragment k-1
-                const float c = T * pa;
-                accA += c;
+                    for (int v = 0; v < FV; ++v) nf[v] = s_f[(cur >> 4) * FV + v];
+                    const uint32_t nh = nc < (nx >> 16) ? s_dk[nc >> 4] : kSentHi;
+                    float* ng = ((p0 | p1) ? gTtop : gTbot) + (cur >> 2);
+                    // blend fragment k-1
+                    const float c = T * pa;
+                    accA += c;
 #pragma unroll
-                for (int v = 0; v < FV; ++v) {
-                    acc[4 * v] += c * pf[v].x; acc[4 * v + 1] += c * pf[v].y; acc[4 * v + 2] += c * pf[v].z; acc[4 * v + 3] += c * pf[v].w;
-                }
-                if (A.gT && have) *pg = T;
-                T *= (1.f - pa);
-                if (T < kTMin) { have = false; break; }   // fragment k is not blended: its list does not advance
-                h0 = p0 ? nh : h0; ce0 = p0 ? nx : ce0;
-                h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;
-                h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
-                h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
-                pa = na; pg = ng; have = true;
+                    for (int v = 0; v < FV; ++v) {
+                        acc[4 * v] += c * pf[v].x; acc[4 * v + 1] += c * pf[v].y; acc[4 * v + 2] += c * pf[v].z; acc[4 * v + 3] += c * pf[v].w;
+                    }
+                    if (A.gT && have) *pg = T;
+                    T *= (1.f - pa);
+                    h0 = p0 ? nh : h0; ce0 = p0 ? nx : ce0;
+                    h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;
+                    h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
+                    h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
+                    pa = na; pg = ng; have = true;
 #pragma unroll
-                for (int v = 0; v < FV; ++v) pf[v] = nf[v];
-                m = min(min(h0, h1), min(h2, h3));
+                    for (int v = 0; v < FV; ++v) pf[v] = nf[v];
+                    m = min(min(h0, h1), min(h2, h3));
+                    p0 = h0 == m; p1 = h1 == m; p2 = h2 == m; p3 = h3 == m;
+                    tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
+                } while ((m != kSentHi) & !tie & !(T * (1.f - pa) < kTMin));
             }
             if (have) {                                   // the last selected fragment
                 const float c = T * pa;
