@@ -34,77 +34,63 @@ __device__ __forceinline__ void stage_positions(const float* __restrict__ pos, l
     }
 }
 
-// a1 + a2: project every point, bump its cell counter; the returned old value is the point's rank
-// inside its cell (its slot in the counting sort), stored so that the scatter pass needs no second
-// atomic.  One global atomic per POINT (not per fragment): the 2x2 footprint is implied by the cell.
+// a1 + a2: project every point and bump its cell counter with a fire-and-forget reduction (RED: no return
+// value, so the pass is bound by reading the positions, not by atomic latency).  One global atomic per
+// POINT (not per fragment): the 2x2 footprint is implied by the cell.  kept[i / 32] bit i % 32 = point i
+// survived the cull (read by k_split).
 __global__ void __launch_bounds__(kBinThreads) k_project_count(const float* __restrict__ pos, long long N,
                                                                 Camera cam, uint32_t* __restrict__ cellcnt,
-                                                                uint32_t* __restrict__ rank) {
+                                                                uint32_t* __restrict__ kept) {
     __shared__ __align__(16) float s_pos[kBinChunk * 3];
     for (long long base = (long long)blockIdx.x * kBinChunk; base < N; base += (long long)gridDim.x * kBinChunk) {
         __syncthreads();
         stage_positions(pos, base, N, s_pos);
         __syncthreads();
-        // all projections, then all atomics, then all stores: kBinPPT atomics in flight per thread
-        int cell[kBinPPT];
-        uint32_t r[kBinPPT];
 #pragma unroll
         for (int k = 0; k < kBinPPT; ++k) {
             const int l = k * kBinThreads + threadIdx.x;
-            cell[k] = -1;
-            if (base + l < N) cell[k] = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]).cell;
-        }
-#pragma unroll
-        for (int k = 0; k < kBinPPT; ++k) {
-            r[k] = 0xFFFFFFFFu;
-            if (cell[k] >= 0) r[k] = atomicAdd(&cellcnt[cell[k]], 1u);
-        }
-#pragma unroll
-        for (int k = 0; k < kBinPPT; ++k) {
-            const long long i = base + k * kBinThreads + threadIdx.x;
-            if (i < N) __stcs(&rank[i], r[k]);
+            const long long i = base + l;                // a warp's lanes hold 32 consecutive, 32-aligned points
+            int cell = -1;
+            if (i < N) cell = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]).cell;
+            if (cell >= 0) atomicAdd(&cellcnt[cell], 1u);
+            const uint32_t mask = __ballot_sync(0xffffffffu, cell >= 0);
+            if ((threadIdx.x & 31) == 0 && i < N) kept[i >> 5] = mask;
         }
     }
 }
 
-// a1 (emission): re-project (bit-identical), slot = celloff[cell] + rank, write ONE full 32-byte
-// sector per point: { depth_bits, idx, tx, ty | opacity, cell, 0, 0 }.  (Anything narrower than a
-// sector scattered by slot costs a DRAM read-modify-write: profiles/r01_v1_baseline.md.)
+// a1 (emission): re-project (bit-identical to the count pass), take the point's slot from a returning atomic
+// on cursor[cell] (a copy of the exclusive cell offsets, so slots of a cell are handed out in arrival order;
+// afterwards cursor[c] == celloff[c + 1]) and write ONE full 32-byte sector per point:
+// { depth_bits, idx, tx, ty | opacity, cell, 0, 0 }.  (Anything narrower than a sector scattered by slot costs a
+// DRAM read-modify-write: profiles/r01_v1_baseline.md.)  All of a thread's atomics and opacity loads are
+// issued before the first store.
 __global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict__ pos,
                                                           const float* __restrict__ opacity, long long N, Camera cam,
-                                                          const uint32_t* __restrict__ celloff,
-                                                          const uint32_t* __restrict__ rank,
-                                                          float4* __restrict__ A) {
+                                                          uint32_t* __restrict__ cursor, float4* __restrict__ A) {
     __shared__ __align__(16) float s_pos[kBinChunk * 3];
     for (long long base = (long long)blockIdx.x * kBinChunk; base < N; base += (long long)gridDim.x * kBinChunk) {
         __syncthreads();
         stage_positions(pos, base, N, s_pos);
         __syncthreads();
-        // ranks (coalesced), projections, then all celloff gathers and opacity loads in flight, then the stores
-        uint32_t r[kBinPPT], off[kBinPPT];
+        uint32_t slot[kBinPPT];
         float op[kBinPPT];
         Proj p[kBinPPT];
 #pragma unroll
         for (int k = 0; k < kBinPPT; ++k) {
-            const long long i = base + k * kBinThreads + threadIdx.x;
-            r[k] = i < N ? __ldcs(&rank[i]) : 0xFFFFFFFFu;
-        }
-#pragma unroll
-        for (int k = 0; k < kBinPPT; ++k) {
             const int l = k * kBinThreads + threadIdx.x;
-            p[k] = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]);
+            p[k] = project_point(cam, s_pos[3 * l], s_pos[3 * l + 1], s_pos[3 * l + 2]);   // padding -> culled
         }
 #pragma unroll
         for (int k = 0; k < kBinPPT; ++k) {
-            const bool live = r[k] != 0xFFFFFFFFu;
-            off[k] = live ? __ldg(&celloff[p[k].cell]) : 0u;
+            const bool live = p[k].cell >= 0;
+            slot[k] = live ? atomicAdd(&cursor[p[k].cell], 1u) : 0u;
             op[k] = live ? __ldcs(&opacity[base + k * kBinThreads + threadIdx.x]) : 0.f;
         }
 #pragma unroll
         for (int k = 0; k < kBinPPT; ++k) {
-            if (r[k] == 0xFFFFFFFFu) continue;
+            if (p[k].cell < 0) continue;
             const long long i = base + k * kBinThreads + threadIdx.x;
-            const size_t slot = (size_t)off[k] + r[k];
             float4 a0, a1;
             a0.x = __uint_as_float(p[k].depth_bits);
             a0.y = __uint_as_float((uint32_t)i);
@@ -113,8 +99,8 @@ __global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict
             a1.x = op[k];
             a1.y = __uint_as_float((uint32_t)p[k].cell);
             a1.z = 0.f; a1.w = 0.f;
-            A[2 * slot] = a0;
-            A[2 * slot + 1] = a1;
+            A[2 * (size_t)slot[k]] = a0;
+            A[2 * (size_t)slot[k] + 1] = a1;
         }
     }
 }
@@ -130,7 +116,8 @@ constexpr int kScanTile    = kScanThreads * kScanItems;
 __global__ void __launch_bounds__(kScanThreads) k_scan_u32(uint32_t* __restrict__ data, uint32_t n,
                                                             unsigned long long* __restrict__ status,
                                                             uint32_t* __restrict__ tile_counter,
-                                                            uint32_t* __restrict__ total_out) {
+                                                            uint32_t* __restrict__ total_out,
+                                                            uint32_t* __restrict__ copy_out) {
     __shared__ uint32_t s_tile;
     __shared__ uint32_t s_warp[kScanThreads / 32];
     __shared__ uint32_t s_prefix;
@@ -206,12 +193,15 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_u32(uint32_t* __restrict_
     if (base + kScanItems <= n) {
 #pragma unroll
         for (int q = 0; q < kScanItems / 4; ++q)
-            reinterpret_cast<uint4*>(data + base)[q] =
-                make_uint4(v[4 * q] + off, v[4 * q + 1] + off, v[4 * q + 2] + off, v[4 * q + 3] + off);
+        {
+            const uint4 o4 = make_uint4(v[4 * q] + off, v[4 * q + 1] + off, v[4 * q + 2] + off, v[4 * q + 3] + off);
+            reinterpret_cast<uint4*>(data + base)[q] = o4;
+            if (copy_out) reinterpret_cast<uint4*>(copy_out + base)[q] = o4;     // second copy (the scatter's slot cursors)
+        }
     } else {
 #pragma unroll
         for (int q = 0; q < kScanItems; ++q)
-            if (base + q < n) data[base + q] = v[q] + off;
+            if (base + q < n) { data[base + q] = v[q] + off; if (copy_out) copy_out[base + q] = v[q] + off; }
     }
 }
 

@@ -11,7 +11,7 @@
 //              only scattered write of the backward pass, and never narrower than a sector.  No atomics:
 //              every fragment has exactly one writer, so gradients are bit-reproducible run to run.
 //   k_split    one thread per POINT: gpt -> grad_feat[N][D], grad_opacity[N], grad_uv[N][2] (coalesced);
-//              culled points (rank == ~0) get exact zeros.
+//              culled points (their bit of the kept mask is 0) get exact zeros.
 #pragma once
 #include "common.cuh"
 
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
 }
 
 template <int D>
-__global__ void __launch_bounds__(256) k_split(const float* __restrict__ gpt, const uint32_t* __restrict__ rank,
+__global__ void __launch_bounds__(256) k_split(const float* __restrict__ gpt, const uint32_t* __restrict__ kept,
                                                 long long N, float* __restrict__ d_feat, float* __restrict__ d_opacity,
                                                 float* __restrict__ d_uv) {
     constexpr int GP = gpt_floats<D>();
@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(256) k_split(const float* __restrict__ gpt, co
         float4 f[D / 4], o = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
         for (int v = 0; v < D / 4; ++v) f[v] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (__ldcs(&rank[i]) != 0xFFFFFFFFu) {
+        if ((__ldg(&kept[i >> 5]) >> (i & 31)) & 1u) {
             const float4* in = reinterpret_cast<const float4*>(gpt + (size_t)i * GP);
 #pragma unroll
             for (int v = 0; v < D / 4; ++v) f[v] = __ldcs(&in[v]);

@@ -64,7 +64,7 @@ struct StageTimer {                       // RAII: start event now, stop event a
 
 struct Layout {
     size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
-    size_t rank, A, gT, gD, dk, Ra, Rf, items, bigpix, bigcells, bigkeys;
+    size_t kept, cursor, A, gT, gD, dk, Ra, Rf, items, bigpix, bigcells, bigkeys;
     size_t pcur, gpt;                                     // only with INPC_SAVE_FOR_BACKWARD
     size_t pixoff, sorted_idx, sorted_depth;              // only with INPC_SAVE_SORTED
     size_t total;
@@ -86,7 +86,8 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     L.status1 = o; o = align_up(o + (size_t)L.n_status * 8);
     L.cellcnt = o; o = align_up(o + ((size_t)L.C + 1) * 4);
     L.zero_end = o;
-    L.rank = o;    o = align_up(o + n * 4 + 16);
+    L.kept = o;    o = align_up(o + (n / 32 + 2) * 4);
+    L.cursor = o;  o = align_up(o + ((size_t)L.C + 16) * 4);
     L.A = o;       L.gT = o; L.gD = o + (n + 8) * 16;     // the emission records are dead once the cells are sorted:
     o = align_up(o + (n + 8) * 32);                       // their bytes then hold gT | gD (16 B per record each)
     L.dk = o;      o = align_up(o + (n + 16) * 4);
@@ -242,7 +243,8 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     const int W = cam->width, H = cam->height;
     Header* hdr = reinterpret_cast<Header*>(ws + L.header);
     uint32_t* cellcnt = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
-    uint32_t* rank = reinterpret_cast<uint32_t*>(ws + L.rank);
+    uint32_t* kept = reinterpret_cast<uint32_t*>(ws + L.kept);
+    uint32_t* cursor = reinterpret_cast<uint32_t*>(ws + L.cursor);
     float4* Arec = reinterpret_cast<float4*>(ws + L.A);
     uint32_t* dk = reinterpret_cast<uint32_t*>(ws + L.dk);
     float4* Ra = reinterpret_cast<float4*>(ws + L.Ra);
@@ -261,16 +263,16 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     const int bin_grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
     if (N > 0) {
         { StageTimer tm(kStProjectCount, st);
-          k_project_count<<<bin_grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, rank); }
+          k_project_count<<<bin_grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, kept); }
         INPC_LAUNCHED();
     }
     { StageTimer tm(kStScan, st);
       k_scan_u32<<<(L.C + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
-          cellcnt, L.C, reinterpret_cast<unsigned long long*>(ws + L.status0), &hdr->scan_tile_counter, &hdr->nrec); }
+          cellcnt, L.C, reinterpret_cast<unsigned long long*>(ws + L.status0), &hdr->scan_tile_counter, &hdr->nrec, cursor); }
     INPC_LAUNCHED();
     if (N > 0) {
         { StageTimer tm(kStScatter, st);
-          k_scatter<<<bin_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cellcnt, rank, Arec); }
+          k_scatter<<<bin_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cursor, Arec); }
         INPC_LAUNCHED();
     }
     { StageTimer tm(kStClassify, st);
@@ -290,7 +292,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     if (dump) {
         { StageTimer tm(kStOther, st);
           k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
-              pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr); }
+              pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr, nullptr); }
         INPC_LAUNCHED();
     }
     const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
@@ -356,7 +358,7 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     INPC_LAUNCHED();
     { StageTimer tm(kStSplit, st);
       k_split<D><<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16), 256, 0, st>>>(
-          gpt, reinterpret_cast<const uint32_t*>(ws + L.rank), (long long)N, d_feat, d_opacity, d_uv); }
+          gpt, reinterpret_cast<const uint32_t*>(ws + L.kept), (long long)N, d_feat, d_opacity, d_uv); }
     INPC_LAUNCHED();
     return INPC_OK;
 }
