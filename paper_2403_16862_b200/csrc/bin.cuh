@@ -99,8 +99,7 @@ __global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict
             a1.x = op[k];
             a1.y = __uint_as_float((uint32_t)p[k].cell);
             a1.z = 0.f; a1.w = 0.f;
-            A[2 * (size_t)slot[k]] = a0;
-            A[2 * (size_t)slot[k] + 1] = a1;
+            st_sector(A + 2 * (size_t)slot[k], a0, a1);         // one 256-bit store = the whole 32-byte sector
         }
     }
 }

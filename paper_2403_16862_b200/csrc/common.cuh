@@ -103,6 +103,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "r"(parity)
         : "memory");
 }
+// One 256-bit store: a whole 32-byte sector in ONE instruction.  A lane-divergent store costs L1 wavefronts
+// per instruction, so two 128-bit stores to the same sector cost twice (k_scatter 222 -> 173 us).
+__device__ __forceinline__ void st_sector(void* p, float4 lo, float4 hi) {
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(lo.x), "f"(lo.y), "f"(lo.z),
+                 "f"(lo.w), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w)
+                 : "memory");
+}
 // TMA bulk copy global -> shared (1-D, no tensor map): 16-byte aligned src/dst, size multiple of 16.
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(

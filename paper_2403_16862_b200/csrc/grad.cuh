@@ -88,10 +88,12 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
             }
             du *= r0.z; dv *= r0.z;
             float4* out = reinterpret_cast<float4*>(gpt + (size_t)__float_as_uint(r0.w) * GP);
-#pragma unroll
-            for (int v = 0; v < D / 4; ++v) out[v] = make_float4(df[4 * v], df[4 * v + 1], df[4 * v + 2], df[4 * v + 3]);
-            out[D / 4] = make_float4(dop, du, dv, 0.f);
-            if (D == 8) out[3] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (D == 4) {
+                st_sector(out, make_float4(df[0], df[1], df[2], df[3]), make_float4(dop, du, dv, 0.f));
+            } else {
+                st_sector(out, make_float4(df[0], df[1], df[2], df[3]), make_float4(df[4], df[5], df[6], df[7]));
+                st_sector(out + 2, make_float4(dop, du, dv, 0.f), make_float4(0.f, 0.f, 0.f, 0.f));
+            }
         }
     }
 }
