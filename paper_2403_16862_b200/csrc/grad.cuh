@@ -38,9 +38,13 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
         for (uint32_t c = tid; c <= nc; c += kGradThreads) s_off[c] = __ldg(&celloff[c0 + c]);
         __syncthreads();
         const uint32_t S = s_off[0], E = s_off[nc];
+        uint32_t lo = 0;                                         // a thread's slots ascend: the search resumes at its last cell
         for (uint32_t slot = S + tid; slot < E; slot += kGradThreads) {
+            // the record's own (coalesced) loads first: they do not depend on the cell search
+            const float4 r0 = __ldg(&Ra[slot]);                   // tx, ty, opacity, idx
+            const float4 t4 = __ldcs(&gT[slot]), d4 = __ldcs(&gD[slot]);
             // cell of this slot: the last c with s_off[c] <= slot (empty cells repeat offsets)
-            uint32_t lo = 0, hi = nc - 1;
+            uint32_t hi = nc - 1;
             while (lo < hi) {
                 const uint32_t mid = (lo + hi + 1) >> 1;
                 if (s_off[mid] <= slot) lo = mid; else hi = mid - 1;
@@ -48,8 +52,6 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
             const uint32_t cell = c0 + lo, r = slot - s_off[lo];
             const int j = cell / (W + 1), i = cell - j * (W + 1);
             const int x0 = i - 1, y0 = j - 1;
-            const float4 r0 = __ldg(&Ra[slot]);                   // tx, ty, opacity, idx
-            const float4 t4 = __ldcs(&gT[slot]), d4 = __ldcs(&gD[slot]);
             // every gather of the four corner pixels is issued before any of them is used
             uint4 cur[4];
             float4 gp[4][D / 4];
