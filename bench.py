@@ -44,10 +44,10 @@ L2_BYTES = 126 * 1024 * 1024
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/; the file named in NCU_TRAFFIC_SOURCE).  None until a capture exists for that kernel.
 NCU_TRAFFIC = {   # bytes per launch, train workload
-    "k_project_count": 115.2e6, "k_scatter": 424.7e6, "k_cellsort": 1203.3e6, "k_blend": 632.0e6,
-    "k_back": 809.7e6, "k_combine": 746.8e6, "k_split": 492.9e6,
+    "k_project_count": 108.4e6, "k_scatter": 390.4e6, "k_cellsort": 1203.3e6, "k_blend": 632.3e6,
+    "k_back": 804.6e6, "k_combine": 750.6e6, "k_split": 457.4e6,
 }
-NCU_TRAFFIC_SOURCE = "profiles/r01_v3_blend_back.md (ncu --set full, train workload; k_cellsort from r01_v2_cellsort_merge.md)"
+NCU_TRAFFIC_SOURCE = "profiles/r01_v3b_sector_stores.md (ncu --set full, train workload; k_cellsort from r01_v2_cellsort_merge.md)"
 
 
 # ------------------------------------------------------------------------------------------------
