@@ -9,7 +9,9 @@
 //   A[nrec]     : 32-byte emission records in arrival order inside each cell (written by k_scatter):
 //                 { depth_bits, point_idx, tx, ty | opacity, cell, 0, 0 }   (tx = fu - x0, ty = fv - y0, exact)
 //   dk[nrec]    : depth bits, every cell sorted ascending by (depth_bits, point_idx)   (k_cellsort)
-//   R[nrec]     : payload records in the same order, 16 + 4*D bytes: { tx, ty, opacity, point_idx | feat[D] }
+//   Ra[nrec]    : { tx, ty, opacity, point_idx } in the same order (16 B; staged by the tile kernels and turned
+//                 into the four per-corner alphas in shared memory), Rf[nrec] : feat[D] in the same order
+//   kept[N/32]  : 1 bit per point = survived the cull; cursor[C] : copy of celloff the scatter hands slots out of
 //   Because every cell list is sorted, a pixel's depth-ordered fragment run is the 4-way MERGE of its
 //   four cell lists; no per-pixel sort exists anywhere.
 //   gT[4*nrec]  : transmittance in front of fragment (slot, corner), written by the forward pass
