@@ -260,7 +260,10 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
       INPC_CUDA(cudaMemsetAsync(ws + L.header, 0, L.zero_end - L.header, st));
       k_write_header<<<1, 1, 0, st>>>(hdr, flags, W, H, D, (uint32_t)N); }
     INPC_LAUNCHED();
+    // grid sizes in CTAs per SM are measured optima (profiles/r01_v3b_sector_stores.md): the passes that scatter
+    // (k_scatter, k_cellsort) are fastest with ONE resident wave of 4 CTAs per SM, the streaming count pass with 8
     const int bin_grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
+    const int scatter_grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 4);
     if (N > 0) {
         { StageTimer tm(kStProjectCount, st);
           k_project_count<<<bin_grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, kept); }
@@ -272,7 +275,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     INPC_LAUNCHED();
     if (N > 0) {
         { StageTimer tm(kStScatter, st);
-          k_scatter<<<bin_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cursor, Arec); }
+          k_scatter<<<scatter_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cursor, Arec); }
         INPC_LAUNCHED();
     }
     { StageTimer tm(kStClassify, st);
@@ -281,7 +284,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     if (N > 0) {
         const uint32_t n_units = (L.C + kCsCells - 1) / kCsCells;
         { StageTimer tm(kStCellSort, st);
-          k_cellsort<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 8), kCsThreads, 0, st>>>(
+          k_cellsort<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 4), kCsThreads, 0, st>>>(
               Arec, cellcnt, L.C, feat, dk, Ra, Rf); }
         INPC_LAUNCHED();
         int rc = launch_cellsort_big<D>(hdr, &hdr->bigcell_cursor, bigcells, Arec,
