@@ -356,7 +356,53 @@ def run_ours(args) -> int:
     h2d = sum(t.numel() * t.element_size() for t in h_in)
     d2h = sum(t.numel() * t.element_size() for t in h_out)
 
-    def e2e_step():
+    # Three streams, two buffer sets: step i's host->device copy, step i-1's forward + backward and step i-2's
+    # device->host copy overlap (PCIe is full duplex); every step still copies ITS inputs in and ITS results out
+    # inside the timed region.
+    s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+    sets = []
+    for b in range(2):
+        di = d_in if b == 0 else [torch.empty_like(t) for t in d_in]
+        do = d_out if b == 0 else [torch.empty_like(t) for t in d_out]
+        wsb = ws if b == 0 else raster.alloc_workspace(N, D, W, H, flags, dev)
+        ho = h_out if b == 0 else [torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in d_out]
+        sets.append({"d_in": di, "d_out": do, "ws": wsb, "h_out": ho,
+                     "in_ready": torch.cuda.Event(), "done": torch.cuda.Event(), "out_free": torch.cuda.Event()})
+
+    def e2e_pipeline(steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        s_in.wait_stream(stream); s_out.wait_stream(stream)
+        e0.record(s_in)
+        for i in range(steps):
+            S = sets[i % 2]
+            if i >= 2:
+                s_in.wait_event(S["done"])               # step i-2 has finished reading these inputs
+            with torch.cuda.stream(s_in):
+                for h, d in zip(h_in, S["d_in"]):
+                    d.copy_(h, non_blocking=True)
+                S["in_ready"].record(s_in)
+            stream.wait_event(S["in_ready"])
+            if i >= 2:
+                stream.wait_event(S["out_free"])         # step i-2's results have left the device
+            p_, o_, f_, gi_, ga_ = S["d_in"]
+            im_, al_, df_, dop_, du_ = S["d_out"]
+            raster.inpc_raster_forward(p_, o_, f_, cam, out_feat=im_, out_alpha=al_, workspace=S["ws"], flags=flags,
+                                       stream=stream)
+            raster.inpc_raster_backward(p_, o_, f_, cam, gi_, ga_, S["ws"], grad_feat=df_, grad_opacity=dop_,
+                                        grad_uv=du_, stream=stream)
+            S["done"].record(stream)
+            s_out.wait_event(S["done"])
+            with torch.cuda.stream(s_out):
+                for d, h in zip(S["d_out"], S["h_out"]):
+                    h.copy_(d, non_blocking=True)
+                S["out_free"].record(s_out)
+        e1.record(s_out)
+        stream.wait_stream(s_out)
+        barrier()
+        return e0.elapsed_time(e1)
+
+    def e2e_step():                                       # the same, one stream, nothing overlapped
         for h, d in zip(h_in, d_in):
             d.copy_(h, non_blocking=True)
         fwd()
@@ -364,13 +410,15 @@ def run_ours(args) -> int:
         for d, h in zip(d_out, h_out):
             h.copy_(d, non_blocking=True)
 
-    e2e_steps = max(1, min(args.steps, 10))
+    e2e_steps = max(2, min(args.steps, 10))
     e2e_step()
+    ms_e2e_serial = timed(e2e_step, e2e_steps) / e2e_steps
+    e2e_pipeline(2)
     if clocks:
         with clocks.window():
-            ms_e2e_total = timed(e2e_step, e2e_steps)
+            ms_e2e_total = e2e_pipeline(e2e_steps)
     else:
-        ms_e2e_total = timed(e2e_step, e2e_steps)
+        ms_e2e_total = e2e_pipeline(e2e_steps)
     ms_e2e_total, units_e2e = aggregate_over_ranks(ms_e2e_total, float(n_frag) * e2e_steps, dev)
     clock_info = clocks.finish() if clocks else None
 
@@ -411,8 +459,11 @@ def run_ours(args) -> int:
         "fragments_per_step_per_gpu": n_frag, "stats": stats,
         "e2e": {"value": throughput(units_e2e, ms_e2e_total), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e_total / e2e_steps, "steps": e2e_steps,
-                "how": "pinned host inputs (pos, opacity, feat, grad_out) copied H2D, forward, backward, and "
-                       "img/alpha/grad_feat/grad_opacity/grad_uv copied D2H, every step, on the launch stream"},
+                "ms_per_step_one_stream": ms_e2e_serial,
+                "how": "every step copies its pinned host inputs (pos, opacity, feat, grad_out) H2D, runs forward + "
+                       "backward and copies img/alpha/grad_feat/grad_opacity/grad_uv D2H; three streams and two buffer "
+                       "sets overlap step i's H2D, step i-1's kernels and step i-2's D2H (ms_per_step_one_stream: "
+                       "the same without overlap)"},
         "gpu_launches": launches,
         "roofline": roofline, "roofline_step": roofline_step,
         "stage_ms_per_step": step_stage_ms, "stage_timed_ms_per_step": ms_staged / args.steps,
