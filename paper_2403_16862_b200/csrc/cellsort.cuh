@@ -107,16 +107,23 @@ __device__ __forceinline__ bool bigcell_less(unsigned long long a, unsigned long
     return ia < ib;
 }
 
-// merge stages j = j0, j0/2, ..., 1 of the all-ascending network on s[0..m) (m <= kBigChunk)
+// One compare-exchange of the all-ascending network on shared-memory keys (equal depth bits: rare).
+__device__ __forceinline__ void cex(unsigned long long* s, uint32_t i, uint32_t l, const float4* A) {
+    const unsigned long long a = s[i], b = s[l];
+    const uint32_t da = (uint32_t)(a >> 32), db = (uint32_t)(b >> 32);
+    bool sw = db < da;
+    if (da == db) sw = bigcell_less(b, a, A);
+    if (sw) { s[i] = b; s[l] = a; }
+}
+
+// merge stages j = j0, j0/2, ..., 1 of the all-ascending network on s[0..m) (m <= kBigChunk); j0 a power of two.
+// All index arithmetic is shifts: span, j are powers of two (lj = log2 j).
 __device__ __forceinline__ void smem_merge_stages(unsigned long long* s, uint32_t m, uint32_t j0, const float4* A) {
     uint32_t span = 2; while (span < m) span <<= 1;
-    for (uint32_t j = j0; j > 0; j >>= 1) {
+    for (uint32_t j = j0, lj = 31u - __clz(j0); j > 0; j >>= 1, --lj) {
         for (uint32_t c = threadIdx.x; c < (span >> 1); c += blockDim.x) {
-            const uint32_t i = ((c / j) * (j << 1)) + (c & (j - 1)), l = i + j;
-            if (l < m) {
-                const unsigned long long a = s[i], b = s[l];
-                if (bigcell_less(b, a, A)) { s[i] = b; s[l] = a; }
-            }
+            const uint32_t i = ((c >> lj) << (lj + 1)) + (c & (j - 1)), l = i + j;
+            if (l < m) cex(s, i, l, A);
         }
         __syncthreads();
     }
@@ -124,14 +131,11 @@ __device__ __forceinline__ void smem_merge_stages(unsigned long long* s, uint32_
 
 __device__ __forceinline__ void smem_sort_full(unsigned long long* s, uint32_t m, const float4* A) {
     uint32_t span = 2; while (span < m) span <<= 1;
-    for (uint32_t k = 2; k <= span; k <<= 1) {
+    for (uint32_t k = 2, lhk = 0; k <= span; k <<= 1, ++lhk) {          // hk = k / 2 = 1 << lhk
         const uint32_t hk = k >> 1;
         for (uint32_t c = threadIdx.x; c < (span >> 1); c += blockDim.x) {
-            const uint32_t i = ((c / hk) * k) + (c & (hk - 1)), l = i ^ (k - 1);
-            if (l < m) {
-                const unsigned long long a = s[i], b = s[l];
-                if (bigcell_less(b, a, A)) { s[i] = b; s[l] = a; }
-            }
+            const uint32_t i = ((c >> lhk) << (lhk + 1)) + (c & (hk - 1)), l = i ^ (k - 1);
+            if (l < m) cex(s, i, l, A);
         }
         __syncthreads();
         if (k >= 4) smem_merge_stages(s, m, k >> 2, A);
