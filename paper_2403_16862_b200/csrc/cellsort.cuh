@@ -142,8 +142,12 @@ __device__ __forceinline__ void smem_sort_full(unsigned long long* s, uint32_t m
     }
 }
 
-template <int D>
-__global__ void __launch_bounds__(kBigThreads) k_cellsort_big(const Header* __restrict__ hdr,
+// THREADS / CHUNK: CTA size and keys sorted in shared memory at a time.  Two instances run back to back: cells of
+// up to 1024 points on 128-thread CTAs with 8 KB of shared memory (16 CTAs per SM: what bounds this kernel is the
+// number of cells in flight, every bitonic stage being a CTA barrier), larger cells on 512-thread CTAs with 64 KB.
+// A CTA takes every cell of the list in turn and skips those outside [n_lo, n_hi].
+template <int D, int THREADS, int CHUNK>
+__global__ void __launch_bounds__(THREADS) k_cellsort_big(const Header* __restrict__ hdr, uint32_t n_lo, uint32_t n_hi,
                                                                uint32_t* __restrict__ cursor,
                                                                const BigCell* __restrict__ bigcells,
                                                                const float4* __restrict__ A,
@@ -163,30 +167,31 @@ __global__ void __launch_bounds__(kBigThreads) k_cellsort_big(const Header* __re
         if (b >= n_big) break;
         const BigCell e = bigcells[b];
         const uint32_t n = e.n, start = e.start;
+        if (n < n_lo || n > n_hi) continue;               // the other instance's (uniform across the CTA)
         unsigned long long* keys = keys_all + start;     // scratch slice, indexed like the slots
         auto make_key = [&](uint32_t l) -> unsigned long long {
             const uint32_t depth = __float_as_uint(__ldg(&A[2 * (size_t)(start + l)]).x);
             return ((unsigned long long)depth << 32) | (unsigned long long)(start + l);
         };
-        if (n <= (uint32_t)kBigChunk) {
-            for (uint32_t l = tid; l < n; l += kBigThreads) s_keys[l] = make_key(l);
+        if (n <= (uint32_t)CHUNK) {
+            for (uint32_t l = tid; l < n; l += THREADS) s_keys[l] = make_key(l);
             __syncthreads();
             smem_sort_full(s_keys, n, A);
-            for (uint32_t l = tid; l < n; l += kBigThreads) __stcg(&keys[l], s_keys[l]);
+            for (uint32_t l = tid; l < n; l += THREADS) __stcg(&keys[l], s_keys[l]);
         } else {
-            for (uint32_t cb = 0; cb < n; cb += kBigChunk) {
-                const uint32_t m = min((uint32_t)kBigChunk, n - cb);
+            for (uint32_t cb = 0; cb < n; cb += CHUNK) {
+                const uint32_t m = min((uint32_t)CHUNK, n - cb);
                 __syncthreads();
-                for (uint32_t l = tid; l < m; l += kBigThreads) s_keys[l] = make_key(cb + l);
+                for (uint32_t l = tid; l < m; l += THREADS) s_keys[l] = make_key(cb + l);
                 __syncthreads();
                 smem_sort_full(s_keys, m, A);
-                for (uint32_t l = tid; l < m; l += kBigThreads) __stcg(&keys[cb + l], s_keys[l]);
+                for (uint32_t l = tid; l < m; l += THREADS) __stcg(&keys[cb + l], s_keys[l]);
             }
             __syncthreads();
-            uint32_t np2 = kBigChunk; while (np2 < n) np2 <<= 1;
-            for (uint32_t k = 2u * kBigChunk; k <= np2; k <<= 1) {
+            uint32_t np2 = CHUNK; while (np2 < n) np2 <<= 1;
+            for (uint32_t k = 2u * CHUNK; k <= np2; k <<= 1) {
                 const uint32_t hk = k >> 1;
-                for (uint32_t c = tid; c < (np2 >> 1); c += kBigThreads) {          // flip stage, global
+                for (uint32_t c = tid; c < (np2 >> 1); c += THREADS) {          // flip stage, global
                     const uint32_t i = ((c / hk) * k) + (c & (hk - 1)), l = i ^ (k - 1);
                     if (l < n) {
                         const unsigned long long a = __ldcg(&keys[i]), bb = __ldcg(&keys[l]);
@@ -195,8 +200,8 @@ __global__ void __launch_bounds__(kBigThreads) k_cellsort_big(const Header* __re
                 }
                 __syncthreads();
                 uint32_t j = k >> 2;
-                for (; j >= (uint32_t)kBigChunk; j >>= 1) {                          // long-distance stages, global
-                    for (uint32_t c = tid; c < (np2 >> 1); c += kBigThreads) {
+                for (; j >= (uint32_t)CHUNK; j >>= 1) {                          // long-distance stages, global
+                    for (uint32_t c = tid; c < (np2 >> 1); c += THREADS) {
                         const uint32_t i = ((c / j) * (j << 1)) + (c & (j - 1)), l = i + j;
                         if (l < n) {
                             const unsigned long long a = __ldcg(&keys[i]), bb = __ldcg(&keys[l]);
@@ -205,19 +210,19 @@ __global__ void __launch_bounds__(kBigThreads) k_cellsort_big(const Header* __re
                     }
                     __syncthreads();
                 }
-                for (uint32_t cb = 0; cb < n; cb += kBigChunk) {                     // j < chunk: in shared memory
-                    const uint32_t m = min((uint32_t)kBigChunk, n - cb);
-                    for (uint32_t l = tid; l < m; l += kBigThreads) s_keys[l] = __ldcg(&keys[cb + l]);
+                for (uint32_t cb = 0; cb < n; cb += CHUNK) {                     // j < chunk: in shared memory
+                    const uint32_t m = min((uint32_t)CHUNK, n - cb);
+                    for (uint32_t l = tid; l < m; l += THREADS) s_keys[l] = __ldcg(&keys[cb + l]);
                     __syncthreads();
-                    smem_merge_stages(s_keys, m, kBigChunk >> 1, A);
-                    for (uint32_t l = tid; l < m; l += kBigThreads) __stcg(&keys[cb + l], s_keys[l]);
+                    smem_merge_stages(s_keys, m, CHUNK >> 1, A);
+                    for (uint32_t l = tid; l < m; l += THREADS) __stcg(&keys[cb + l], s_keys[l]);
                     __syncthreads();
                 }
             }
         }
         __syncthreads();
         // permute: sorted position l takes the record of source slot low32(keys[l])
-        for (uint32_t l = tid; l < n; l += kBigThreads) {
+        for (uint32_t l = tid; l < n; l += THREADS) {
             const uint32_t src = (uint32_t)__ldcg(&keys[l]);
             const float4 a0 = __ldg(&A[2 * (size_t)src]), a1 = __ldg(&A[2 * (size_t)src + 1]);
             emit_sorted<D>(a0, a1, start + l, feat, dk, Ra, Rf);

@@ -209,24 +209,36 @@ static int launch_big(const BigArgs& A, int sms, cudaStream_t st) {
     return INPC_OK;
 }
 
-template <int D>
-static int launch_cellsort_big(const Header* hdr, uint32_t* cursor, const BigCell* bigcells, const float4* A,
-                               unsigned long long* keys, const float* feat, uint32_t* dk, float4* Ra, float4* Rf, int sms,
-                               uint32_t max_big_cells, cudaStream_t st) {
-    constexpr size_t smem = (size_t)kBigChunk * 8;
+template <int D, int THREADS, int CHUNK>
+static int launch_cellsort_big_class(const Header* hdr, uint32_t n_lo, uint32_t n_hi, uint32_t* cursor,
+                                     const BigCell* bigcells, const float4* A, unsigned long long* keys, const float* feat,
+                                     uint32_t* dk, float4* Ra, float4* Rf, int sms, uint32_t max_big_cells, cudaStream_t st) {
+    constexpr size_t smem = (size_t)CHUNK * 8;
     static bool configured = false;
     static int grid = 0;
     if (!configured) {
-        INPC_CUDA(cudaFuncSetAttribute(k_cellsort_big<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int rc = persistent_grid(k_cellsort_big<D>, kBigThreads, smem, sms, &grid);
+        INPC_CUDA(cudaFuncSetAttribute(k_cellsort_big<D, THREADS, CHUNK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int rc = persistent_grid(k_cellsort_big<D, THREADS, CHUNK>, THREADS, smem, sms, &grid);
         if (rc != INPC_OK) return rc;
         configured = true;
     }
     const int g = (int)std::min<uint32_t>((uint32_t)grid, std::max<uint32_t>(max_big_cells, 1u));
-    { StageTimer tm(kStCellSortBig, st);
-      k_cellsort_big<D><<<g, kBigThreads, smem, st>>>(hdr, cursor, bigcells, A, keys, feat, dk, Ra, Rf); }
+    k_cellsort_big<D, THREADS, CHUNK><<<g, THREADS, smem, st>>>(hdr, n_lo, n_hi, cursor, bigcells, A, keys, feat, dk, Ra, Rf);
     INPC_LAUNCHED();
     return INPC_OK;
+}
+
+// cells of kCellSmall+1 .. 1024 points, then the larger ones (two work cursors in the header)
+template <int D>
+static int launch_cellsort_big(Header* hdr, const BigCell* bigcells, const float4* A, unsigned long long* keys,
+                               const float* feat, uint32_t* dk, float4* Ra, float4* Rf, int sms, uint32_t max_big_cells,
+                               cudaStream_t st) {
+    StageTimer tm(kStCellSortBig, st);
+    int rc = launch_cellsort_big_class<D, 128, 1024>(hdr, 0u, 1024u, &hdr->bigcell_cursor, bigcells, A, keys, feat, dk, Ra,
+                                                     Rf, sms, max_big_cells, st);
+    if (rc != INPC_OK) return rc;
+    return launch_cellsort_big_class<D, kBigThreads, kBigChunk>(hdr, 1025u, 0xFFFFFFFFu, &hdr->cellsort_cursor, bigcells, A,
+                                                                keys, feat, dk, Ra, Rf, sms, max_big_cells, st);
 }
 
 __global__ void k_write_header(Header* h, uint32_t flags, int W, int H, int D, uint32_t N) {
@@ -287,7 +299,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
           k_cellsort<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 4), kCsThreads, 0, st>>>(
               Arec, cellcnt, L.C, feat, dk, Ra, Rf); }
         INPC_LAUNCHED();
-        int rc = launch_cellsort_big<D>(hdr, &hdr->bigcell_cursor, bigcells, Arec,
+        int rc = launch_cellsort_big<D>(hdr, bigcells, Arec,
                                         reinterpret_cast<unsigned long long*>(ws + L.bigkeys), feat, dk, Ra, Rf, di.sms,
                                         L.max_big_cells, st);
         if (rc != INPC_OK) return rc;
