@@ -37,6 +37,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+# flags of the two timed launch configurations (tests/harness.py runs its parity comparison with exactly these)
+FLAGS_STEP = 1      # INPC_SAVE_FOR_BACKWARD: the forward of the fwd+bwd step
+FLAGS_FWD = 0       # forward only (inference)
+
 METRIC = "fragments/sec (fwd+bwd step; ms/frame fwd and fwd+bwd beside it)"
 UNIT = "fragments/s"
 L2_BYTES = 126 * 1024 * 1024
@@ -244,6 +248,37 @@ def workload_config(wl, args) -> dict:
             "l2_hygiene": "inputs + records larger than L2 (see l2 key)"}
 
 
+def make_step_functions(raster, wl, dev, stream=None):
+    """Device-resident buffers of one workload and the two calls a step is made of.
+    -> fwd(flags), bwd(), dict of the tensors.  tests/test_gpu_parity.py launches these to check that what is
+    timed here is what the parity tests compared with the oracle."""
+    import numpy as np
+    import torch
+    W, H, D, N = wl.cam.width, wl.cam.height, wl.D, wl.N
+    cam = raster.camera_struct(wl.cam)
+    to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    t = dict(pos=to_dev(wl.pos), op=to_dev(wl.opacity), feat=to_dev(wl.feat), g_img=to_dev(wl.g_img),
+             g_alpha=to_dev(wl.g_alpha), cam=cam)
+    t["ws"] = raster.alloc_workspace(N, D, W, H, FLAGS_STEP, dev)
+    t["img"] = torch.empty((H, W, D), dtype=torch.float32, device=dev)
+    t["alpha"] = torch.empty((H, W), dtype=torch.float32, device=dev)
+    t["d_feat"] = torch.empty((N, D), dtype=torch.float32, device=dev)
+    t["d_op"] = torch.empty((N,), dtype=torch.float32, device=dev)
+    t["d_uv"] = torch.empty((N, 2), dtype=torch.float32, device=dev)
+    if stream is None:
+        stream = torch.cuda.current_stream()
+
+    def fwd(f=FLAGS_STEP):
+        raster.inpc_raster_forward(t["pos"], t["op"], t["feat"], cam, out_feat=t["img"], out_alpha=t["alpha"],
+                                   workspace=t["ws"], flags=f, stream=stream)
+
+    def bwd():
+        raster.inpc_raster_backward(t["pos"], t["op"], t["feat"], cam, t["g_img"], t["g_alpha"], t["ws"],
+                                    grad_feat=t["d_feat"], grad_opacity=t["d_op"], grad_uv=t["d_uv"], stream=stream)
+
+    return fwd, bwd, t
+
+
 # ------------------------------------------------------------------------------------------------
 def run_ours(args) -> int:
     import numpy as np
@@ -266,26 +301,13 @@ def run_ours(args) -> int:
 
     wl = make_workload(args.workload, seed=CONFIGS[args.workload]["seed"] + rank)
     W, H, D, N = wl.cam.width, wl.cam.height, wl.D, wl.N
-    cam = raster.camera_struct(wl.cam)
-    to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
-    pos, op, feat = to_dev(wl.pos), to_dev(wl.opacity), to_dev(wl.feat)
-    g_img, g_alpha = to_dev(wl.g_img), to_dev(wl.g_alpha)
-    flags = raster.SAVE_FOR_BACKWARD
-    ws = raster.alloc_workspace(N, D, W, H, flags, dev)
-    img = torch.empty((H, W, D), dtype=torch.float32, device=dev)
-    alpha = torch.empty((H, W), dtype=torch.float32, device=dev)
-    d_feat = torch.empty((N, D), dtype=torch.float32, device=dev)
-    d_op = torch.empty((N,), dtype=torch.float32, device=dev)
-    d_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
+    assert FLAGS_STEP == raster.SAVE_FOR_BACKWARD
+    flags = FLAGS_STEP
     stream = torch.cuda.current_stream()
-
-    def fwd(f=flags):
-        raster.inpc_raster_forward(pos, op, feat, cam, out_feat=img, out_alpha=alpha, workspace=ws, flags=f,
-                                   stream=stream)
-
-    def bwd():
-        raster.inpc_raster_backward(pos, op, feat, cam, g_img, g_alpha, ws, grad_feat=d_feat, grad_opacity=d_op,
-                                    grad_uv=d_uv, stream=stream)
+    fwd, bwd, T = make_step_functions(raster, wl, dev, stream)
+    cam, ws = T["cam"], T["ws"]
+    pos, op, feat, g_img, g_alpha = T["pos"], T["op"], T["feat"], T["g_img"], T["g_alpha"]
+    img, alpha, d_feat, d_op, d_uv = T["img"], T["alpha"], T["d_feat"], T["d_op"], T["d_uv"]
 
     def barrier():
         if world > 1:
@@ -327,12 +349,12 @@ def run_ours(args) -> int:
 
     # ---- forward only (inference flags) ---------------------------------------------------------------
     for _ in range(3):
-        fwd(0)
+        fwd(FLAGS_FWD)
     if clocks:
         with clocks.window():
-            ms_fwd_total = timed(lambda: fwd(0), args.steps)
+            ms_fwd_total = timed(lambda: fwd(FLAGS_FWD), args.steps)
     else:
-        ms_fwd_total = timed(lambda: fwd(0), args.steps)
+        ms_fwd_total = timed(lambda: fwd(FLAGS_FWD), args.steps)
     ms_fwd_total, _ = aggregate_over_ranks(ms_fwd_total, 0.0, dev)
     ms_fwd = ms_fwd_total / args.steps
 

@@ -20,14 +20,23 @@
  *
  * Memory, ownership, streams
  *   - Every pointer is DEVICE memory owned by the caller unless marked "host".  The library allocates
- *     no device memory and keeps no state between calls: scratch and the state saved for the backward
- *     pass live in the caller's `workspace`.  Device pointers must be 16-byte aligned.
+ *     no device memory and keeps no state between calls, on the host or on the device: scratch and the
+ *     state saved for the backward pass live in the caller's `workspace`, which starts with a small
+ *     header (magic, shape, D, N, flags) the forward pass writes.  Later calls on a workspace
+ *     (backward, get_*) are validated against THAT header, so a workspace may be copied, moved or
+ *     freed by the caller at will; a workspace that holds no matching forward is never interpreted.
+ *   - Device pointers must be 16-byte aligned; `workspace` must be 256-byte aligned (cudaMalloc and
+ *     the PyTorch allocator return at least that).
  *   - Outputs and gradient buffers are OVERWRITTEN (not accumulated into).
  *   - All work is enqueued on `cuda_stream` (a cudaStream_t; NULL = the default stream).  Calls return
- *     without synchronising, except inpc_raster_get_stats and inpc_raster_get_sorted (they read back).
+ *     without synchronising, except the inpc_raster_get_* introspection calls (they read back).
  *
  * Errors: every entry point returns INPC_OK (0) or a negative inpc_status; nothing aborts, throws or
  * prints.  There is no CPU fallback: without a CUDA device every compute call returns INPC_ERR_CUDA.
+ * What only the device can know without a synchronisation -- whether the workspace handed to
+ * inpc_raster_backward really holds the forward its arguments describe -- is checked by the first
+ * kernel of that call: on a mismatch the backward kernels do nothing (the gradient buffers are left
+ * untouched) and the reason is kept in the workspace header; inpc_raster_get_status returns it.
  */
 #ifndef INPC_RASTER_H
 #define INPC_RASTER_H
@@ -51,7 +60,8 @@ typedef enum inpc_status {
     INPC_ERR_INVALID_ARG         = -1,  /* NULL / misaligned pointer, N < 0, W/H <= 0, near >= far, near < 0, N >= 2^30 */
     INPC_ERR_WORKSPACE_TOO_SMALL = -2,
     INPC_ERR_CUDA                = -3,  /* launch failure or sticky error; see inpc_raster_last_cuda_error   */
-    INPC_ERR_NO_SAVED_STATE      = -4,  /* backward / get_* on a workspace no matching forward has filled     */
+    INPC_ERR_NO_SAVED_STATE      = -4,  /* backward / get_* on a workspace no matching forward has filled (get_* return
+                                           it at once; for backward it is reported by inpc_raster_get_status)  */
     INPC_ERR_UNSUPPORTED         = -5   /* D not in {4, 8}, W or H > 4095                                     */
 } inpc_status;
 
@@ -91,15 +101,29 @@ int inpc_raster_backward(const float* pos, const float* opacity, const float* fe
                          float* grad_feat, float* grad_opacity, float* grad_uv,
                          void* workspace, size_t workspace_bytes, void* cuda_stream);
 
-/* Parity introspection: all read the workspace of the last forward on it.
+/* Sticky status of the device-side checks since the last forward on this workspace (synchronises):
+ * INPC_OK, or why the last inpc_raster_backward refused to run (INPC_ERR_NO_SAVED_STATE: no forward
+ * with INPC_SAVE_FOR_BACKWARD has filled this workspace; INPC_ERR_INVALID_ARG: N, D, W or H differ from
+ * that forward's). */
+int inpc_raster_get_status(const void* workspace, void* cuda_stream);
+
+/* Parity introspection.  All of these read the workspace of the last forward on it, take its shape from
+ * the workspace header (W, H must match it) and synchronise the stream.
  * counts[H*W] = per-pixel fragment counts (step a2 of the path). */
 int inpc_raster_get_counts(const void* workspace, int32_t W, int32_t H, uint32_t* counts, void* cuda_stream);
 
-/* Needs a forward with INPC_SAVE_SORTED.  *total (host) = number of fragments; synchronises.
+/* blended[H*W] = how many of a pixel's fragments the forward pass composited before the cut-off
+ * (step a4; needs a forward with INPC_SAVE_FOR_BACKWARD). */
+int inpc_raster_get_blended_counts(const void* workspace, int32_t W, int32_t H, uint32_t* blended, void* cuda_stream);
+
+/* Needs a forward with INPC_SAVE_SORTED.  *total (host) = number of fragments.
  * With offsets == NULL only *total is returned.  Otherwise offsets[H*W+1] = exclusive sum of counts,
- * point_idx[total] / depth_bits[total] = every pixel's fragments in blend order (pixel-major). */
+ * point_idx[total] / depth_bits[total] = every pixel's fragments in blend order (pixel-major), and, when
+ * `transmittance` is not NULL, transmittance[total] = the fp32 transmittance T_k the kernel had in front of
+ * each blended fragment (the value its cut-off test saw), -1 for fragments behind the cut-off. */
 int inpc_raster_get_sorted(const void* workspace, int32_t W, int32_t H, uint32_t* offsets,
-                           uint32_t* point_idx, uint32_t* depth_bits, uint64_t* total, void* cuda_stream);
+                           uint32_t* point_idx, uint32_t* depth_bits, float* transmittance, uint64_t* total,
+                           void* cuda_stream);
 
 /* Fills *stats (host) from the workspace of the last forward; synchronises the stream. */
 int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_stream);
@@ -109,6 +133,11 @@ const char* inpc_raster_strerror(int status);
 const char* inpc_raster_last_cuda_error(void);
 /* Number of kernels this library has launched so far in this process (all entry points). */
 uint64_t inpc_raster_launch_count(void);
+/* Diagnostics: the distinct kernel template instantiations this process has launched since the last reset,
+ * as a ';'-separated, sorted list ("k_back<4>;k_blend<4,0>;..."; k_blend<D,DUMP>, k_big<D,MODE> with MODE 0 =
+ * forward, 1 = forward + INPC_SAVE_SORTED dump, 2 = backward) written to the HOST buffer `buf` (truncated to
+ * buf_bytes, always NUL-terminated; buf may be NULL).  Returns the bytes needed for the whole list. */
+size_t inpc_raster_launched_kernels(char* buf, size_t buf_bytes, int reset);
 
 /* Profiling aid (bench.py's roofline).  With timing enabled every stage the library enqueues is
  * bracketed by two cudaEvents on the caller's stream (a few microseconds per stage; off by default).

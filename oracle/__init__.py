@@ -18,6 +18,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
 T_MIN = 1e-4   # transmittance cut-off (BASELINE.json north_star; not in the paper)
+NO_FORCE = 0xFFFFFFFF   # force_nb value meaning "use the termination test"
 
 
 def build(force: bool = False) -> str:
@@ -41,8 +42,6 @@ def _load():
         lib = C.CDLL(build())
         lib.oracle_create.restype = C.c_void_p
         lib.oracle_create.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]
-        lib.oracle_create_window.restype = C.c_void_p
-        lib.oracle_create_window.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p] + [C.c_int32] * 4
         lib.oracle_create_uv.restype = C.c_void_p
         lib.oracle_create_uv.argtypes = [C.c_void_p] * 5 + [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
         lib.oracle_free.argtypes = [C.c_void_p]
@@ -51,7 +50,9 @@ def _load():
             getattr(lib, name).argtypes = [C.c_void_p]
         lib.oracle_counts.argtypes = [C.c_void_p, C.c_void_p]
         lib.oracle_sorted.argtypes = [C.c_void_p] * 5
-        lib.oracle_blend.argtypes = [C.c_void_p, C.c_double] + [C.c_void_p] * 4
+        lib.oracle_blend.argtypes = [C.c_void_p, C.c_double] + [C.c_void_p] * 5
+        lib.oracle_sorted_T.restype = C.c_int
+        lib.oracle_sorted_T.argtypes = [C.c_void_p, C.c_void_p]
         lib.oracle_backward.restype = C.c_int
         lib.oracle_backward.argtypes = [C.c_void_p] * 6
         lib.oracle_count_fp64_projection_changes.restype = C.c_int64
@@ -86,8 +87,7 @@ class Raster:
         self.P = W * H
 
     @classmethod
-    def from_points(cls, pos, opacity, feat, cam, window=None) -> "Raster":
-        """window = (x0, y0, x1, y1): only pixels in [x0,x1) x [y0,y1) are bucketed (others stay empty)."""
+    def from_points(cls, pos, opacity, feat, cam) -> "Raster":
         lib = _load()
         pos = np.ascontiguousarray(pos, dtype=np.float32).reshape(-1, 3)
         opacity = np.ascontiguousarray(opacity, dtype=np.float32).reshape(-1)
@@ -95,10 +95,7 @@ class Raster:
         N, D = pos.shape[0], (feat.shape[1] if feat.ndim == 2 else 0)
         assert opacity.shape[0] == N and feat.shape[0] == N
         cs = _cam_struct(cam)
-        if window is None:
-            h = lib.oracle_create(_p(pos), _p(opacity), _p(feat), N, D, C.byref(cs))
-        else:
-            h = lib.oracle_create_window(_p(pos), _p(opacity), _p(feat), N, D, C.byref(cs), *[int(x) for x in window])
+        h = lib.oracle_create(_p(pos), _p(opacity), _p(feat), N, D, C.byref(cs))
         return cls(h, N, D, int(cam.width), int(cam.height))
 
     @classmethod
@@ -145,14 +142,26 @@ class Raster:
         _lib.oracle_sorted(self._h, _p(off), _p(idx), _p(dep), _p(w))
         return off, idx, dep, w
 
-    def blend(self, t_min: float = T_MIN):
-        """-> img[H,W,D] f64, alpha[H,W] f64, nb[H,W] u32, margin[H,W] f64."""
+    def blend(self, t_min: float = T_MIN, force_nb=None):
+        """-> img[H,W,D] f64, alpha[H,W] f64, nb[H,W] u32, margin[H,W] f64.
+        force_nb[H,W] u32 (harness aid): where it is not NO_FORCE the pixel blends exactly that many fragments."""
         img = np.empty((self.H, self.W, self.D), dtype=np.float64)
         alpha = np.empty((self.H, self.W), dtype=np.float64)
         nb = np.empty((self.H, self.W), dtype=np.uint32)
         margin = np.empty((self.H, self.W), dtype=np.float64)
-        _lib.oracle_blend(self._h, float(t_min), _p(img), _p(alpha), _p(nb), _p(margin))
+        if force_nb is not None:
+            force_nb = np.ascontiguousarray(force_nb, dtype=np.uint32).reshape(self.H, self.W)
+        _lib.oracle_blend(self._h, float(t_min), None if force_nb is None else _p(force_nb),
+                          _p(img), _p(alpha), _p(nb), _p(margin))
         return img, alpha, nb, margin
+
+    def sorted_T(self) -> np.ndarray:
+        """Per fragment (order of sorted_fragments): the transmittance in front of it if the last blend()
+        composited it, -1 otherwise."""
+        T = np.empty(self.total, dtype=np.float64)
+        if _lib.oracle_sorted_T(self._h, _p(T)) != 0:
+            raise RuntimeError("oracle_sorted_T: blend() has not been called")
+        return T
 
     def backward(self, g_img, g_alpha=None):
         """Gradients of <g_img, img> + <g_alpha, alpha>; call blend() first (same t_min).

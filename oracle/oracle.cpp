@@ -58,10 +58,6 @@ struct State {
     int64_t kept = 0;                        // points that passed the depth / finiteness / range cull
     int64_t border_dropped = 0;              // fragments of kept points that fell outside the image
     bool blended = false;
-    // Optional pixel window [wx0,wx1) x [wy0,wy1): fragments of in-image pixels OUTSIDE it are not
-    // bucketed (their pixels stay empty).  Lets full-size parity tests evaluate sampled pixels one
-    // window at a time without holding every bucket.  Default = whole image.
-    long wx0 = 0, wy0 = 0, wx1 = 1L << 40, wy1 = 1L << 40;
 };
 
 // S2: the (up to) four fragments of one projected point.  fu = u - 0.5, fv = v - 0.5 and
@@ -74,7 +70,6 @@ void emit(State& s, double fu, double fv, double x0, double y0, uint32_t depth_b
         for (int dx = 0; dx < 2; ++dx) {
             const long px = (long)x0 + dx, py = (long)y0 + dy;
             if (px < 0 || px >= s.W || py < 0 || py >= s.H) { s.border_dropped++; continue; }
-            if (px < s.wx0 || px >= s.wx1 || py < s.wy0 || py >= s.wy1) continue;   // outside the test window
             const double wx = dx ? tx : 1.0 - tx;
             const double wy = dy ? ty : 1.0 - ty;
             Frag f;
@@ -114,10 +109,9 @@ extern "C" {
 // S1 + S2 + S3 from world-space points.  The projection is the canonical fp32 sequence:
 // every operation below is one IEEE fp32 operation, in this order, never fused.
 // Follows Eq. 6 with the pinhole divide (reading A2), near/far of PAPER.md:310.
-void* oracle_create_window(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
-                           const Camera* cam, int32_t wx0, int32_t wy0, int32_t wx1, int32_t wy1) {
+void* oracle_create(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                    const Camera* cam) {
     State* s = new_state(N, D, cam->width, cam->height, opacity, feat);
-    if (wx1 > wx0 && wy1 > wy0) { s->wx0 = wx0; s->wy0 = wy0; s->wx1 = wx1; s->wy1 = wy1; }
     const float* R = cam->R;
     const float Wm1 = (float)(cam->width - 1), Hm1 = (float)(cam->height - 1);
     for (int64_t i = 0; i < N; ++i) {
@@ -139,11 +133,6 @@ void* oracle_create_window(const float* pos, const float* opacity, const float* 
     }
     sort_buckets(*s);
     return s;
-}
-
-void* oracle_create(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
-                    const Camera* cam) {
-    return oracle_create_window(pos, opacity, feat, N, D, cam, 0, 0, 0, 0);   // whole image
 }
 
 // Same pipeline from already-projected image coordinates in fp64 (no camera, no cull except the
@@ -197,16 +186,25 @@ void oracle_sorted(void* h, int64_t* offsets, int64_t* point_idx, uint32_t* dept
 // Outputs: img[H][W][D] premultiplied, alpha[H][W] = sum of blended T*a,
 // nb[H][W] blended count, margin[H][W] = min_k |T_k - t_min| / t_min over every T the termination
 // test looked at (harness rule for threshold-ambiguous pixels; +inf when t_min <= 0).
-void oracle_blend(void* h, double t_min, double* img, double* alpha, uint32_t* nb, double* margin) {
+// force_nb (harness aid for those pixels, reading R7; NULL = off): where force_nb[p] is not
+// 0xFFFFFFFF the termination test is replaced by "blend exactly the first force_nb[p] fragments" -- the
+// compositing arithmetic is the same; margin[p] is +inf there.
+void oracle_blend(void* h, double t_min, const uint32_t* force_nb, double* img, double* alpha, uint32_t* nb,
+                  double* margin) {
     State* s = (State*)h; const int D = s->D;
     for (size_t p = 0; p < s->bucket.size(); ++p) {
         double T = 1.0, A = 0.0, m = INFINITY;
         double* C = img + p * D;
         for (int d = 0; d < D; ++d) C[d] = 0.0;
         uint32_t n = 0;
+        const bool forced = force_nb && force_nb[p] != 0xFFFFFFFFu;
         for (auto& f : s->bucket[p]) {
-            if (t_min > 0.0) m = std::min(m, std::fabs(T - t_min) / t_min);
-            if (T < t_min) break;
+            if (forced) {
+                if (n >= force_nb[p]) break;
+            } else {
+                if (t_min > 0.0) m = std::min(m, std::fabs(T - t_min) / t_min);
+                if (T < t_min) break;
+            }
             const double a = (double)s->opacity[f.idx] * f.w;
             const float* F = &s->feat[(size_t)f.idx * D];
             for (int d = 0; d < D; ++d) C[d] += T * a * (double)F[d];
@@ -221,6 +219,19 @@ void oracle_blend(void* h, double t_min, double* img, double* alpha, uint32_t* n
         if (margin) margin[p] = m;
     }
     s->blended = true;
+}
+
+// Per fragment, in the order of oracle_sorted: the transmittance T_k in front of it if the last
+// oracle_blend composited it, -1 otherwise.
+int oracle_sorted_T(void* h, double* T) {
+    State* s = (State*)h;
+    if (!s->blended) return -1;
+    int64_t o = 0;
+    for (size_t p = 0; p < s->bucket.size(); ++p) {
+        uint32_t k = 0;
+        for (auto& f : s->bucket[p]) { T[o++] = k < s->nb[p] ? f.T : -1.0; ++k; }
+    }
+    return 0;
 }
 
 // S5 + S6: gradients of  L = <g_img, img> + <g_alpha, alpha>  w.r.t. features, opacities and the

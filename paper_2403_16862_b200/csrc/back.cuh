@@ -59,6 +59,7 @@ __global__ void __launch_bounds__(kTileThreads) k_back(BackArgs A) {
 
     const int tid = threadIdx.x;
     const int W = A.W, H = A.H;
+    if (!A.hdr->bwd_ok) return;                          // the header check failed: touch nothing
     const uint32_t n_items = A.hdr->n_items;
 
     if (tid == 0) {

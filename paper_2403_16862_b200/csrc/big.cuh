@@ -28,6 +28,7 @@ struct BigArgs {
     const uint32_t* pixoff;
     uint32_t* sorted_idx;
     uint32_t* sorted_depth;
+    float* sorted_T;
     const float* g_feat;
     const float* g_alpha;
     float* gD;
@@ -35,6 +36,7 @@ struct BigArgs {
 
 template <int D, int MODE>
 __global__ void __launch_bounds__(kLongThreads) k_big(BigArgs A) {
+    if (MODE == kBwd && !A.hdr->bwd_ok) return;          // backward on a workspace that holds no matching forward
     const uint32_t n_big = A.hdr->n_big_pixels;
     const int W = A.W;
     for (uint32_t b = blockIdx.x * kLongThreads + threadIdx.x; b < n_big; b += gridDim.x * kLongThreads) {
@@ -49,7 +51,7 @@ __global__ void __launch_bounds__(kLongThreads) k_big(BigArgs A) {
             uint4 consumed = make_uint4(0, 0, 0, 0);
             const uint32_t obase = (MODE == kFwdDump) ? A.pixoff[pix] : 0u;
             blend_pixel<D, MODE == kFwdDump, double>(A.dk, A.Ra, A.Rf, L, 0u, 0u, A.gT, acc, accA, consumed, A.sorted_idx,
-                                                     A.sorted_depth, obase);
+                                                     A.sorted_depth, A.sorted_T, obase);
 #pragma unroll
             for (int v = 0; v < D / 4; ++v)
                 reinterpret_cast<float4*>(A.out_feat + (size_t)pix * D)[v] = make_float4(acc[4 * v], acc[4 * v + 1], acc[4 * v + 2], acc[4 * v + 3]);

@@ -250,6 +250,12 @@ __global__ void __launch_bounds__(256) k_counts_out(const uint32_t* __restrict__
     if (p < W * H) { const int y = p / W; counts[p] = pixel_count(celloff, W, p - y * W, y); }
 }
 
+// Per-pixel blended fragment count = the four list positions at which the forward pass stopped (pcur).
+__global__ void __launch_bounds__(256) k_blended_out(const uint4* __restrict__ pcur, uint32_t P, uint32_t* __restrict__ out) {
+    const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < P) { const uint4 c = pcur[p]; out[p] = c.x + c.y + c.z + c.w; }
+}
+
 // Records a tile item of tw x th pixels at (X, Y) stages into shared memory: each of its th+1 cell
 // rows is one contiguous slot range, widened to multiples of 4 records (16-byte bulk copies of dk).
 __device__ __forceinline__ uint32_t tile_padded_records(const uint32_t* __restrict__ celloff, int W, int H, int X,

@@ -37,6 +37,7 @@ struct BlendArgs {
     const uint32_t* pixoff;
     uint32_t* sorted_idx;
     uint32_t* sorted_depth;
+    float* sorted_T;         // transmittance in front of every blended fragment, -1 behind the cut-off
 };
 
 template <int D> __host__ __device__ constexpr size_t blend_smem_bytes() {
@@ -177,136 +178,112 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
 #pragma unroll
         for (int d = 0; d < D; ++d) acc[d] = 0.f;
         float accA = 0.f, T = 1.f;
-        uint4 consumed = make_uint4(0, 0, 0, 0);
-        if constexpr (!DUMP) {
-            // Software-pipelined, ONE basic block and ONE backward branch per fragment: iteration k selects
-            // fragment k (predicates from the minimum head key), issues its shared-memory loads (alpha, features,
-            // the list's next head key), blends fragment k-1 while they are in flight, advances the list and
-            // recomputes minimum / list predicates / tie flag; the three exit conditions are tested together:
-            // lists exhausted, two heads with equal depth bits (resolved by point index in the outer loop), and
-            // the cut-off -- fragment k+1 is blended iff T_{k+1} = T_k (1 - a_k) >= 1e-4, known as soon as a_k
-            // has arrived.  Entering the body therefore means "fragment k will be blended": the cursors count
-            // exactly the blended fragments.
-            float pa = 0.f;                               // pending fragment: alpha, features, gT address
-            float4 pf[FV];
+        // ONE loop body for every instantiation (DUMP only adds stores and the order-only tail below).
+        // Software-pipelined, ONE basic block and ONE backward branch per fragment: iteration k selects
+        // fragment k (predicates from the minimum head key), issues its shared-memory loads (alpha, features,
+        // the list's next head key), blends fragment k-1 while they are in flight, advances the list and
+        // recomputes minimum / list predicates / tie flag; the three exit conditions are tested together:
+        // lists exhausted, two heads with equal depth bits (resolved by point index in the outer loop), and
+        // the cut-off -- fragment k+1 is blended iff T_{k+1} = T_k (1 - a_k) >= 1e-4, known as soon as a_k
+        // has arrived.  Entering the body therefore means "fragment k will be blended": the cursors count
+        // exactly the blended fragments.
+        float pa = 0.f;                               // pending fragment: alpha, features, gT address
+        float4 pf[FV];
 #pragma unroll
-            for (int v = 0; v < FV; ++v) pf[v] = make_float4(0.f, 0.f, 0.f, 0.f);
-            float* pg = nullptr;
-            bool have = false;
-            uint32_t m = min(min(h0, h1), min(h2, h3));
-            bool p0 = h0 == m, p1 = h1 == m, p2 = h2 == m, p3 = h3 == m;
-            bool tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
-            while (m != kSentHi && !(T * (1.f - pa) < kTMin)) {
-                if (tie) {
-                    uint32_t best = 0xFFFFFFFFu;          // equal depth bits: ascending point index
-                    int jb = 0;
-                    if (p0) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce0 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 0; } }
-                    if (p1) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce1 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 1; } }
-                    if (p2) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce2 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 2; } }
-                    if (p3) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce3 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 3; } }
-                    p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;
+        for (int v = 0; v < FV; ++v) pf[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+        float* pg = nullptr;
+        bool have = false;
+        uint32_t kd = 0;                              // DUMP: position of the next fragment in the pixel's sorted list
+        const uint32_t obase = DUMP ? A.pixoff[pix] : 0u;
+        uint32_t m = min(min(h0, h1), min(h2, h3));
+        bool p0 = h0 == m, p1 = h1 == m, p2 = h2 == m, p3 = h3 == m;
+        bool tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
+        // equal depth bits: ascending point index decides (read from global memory; rare)
+        auto resolve_tie = [&]() {
+            uint32_t best = 0xFFFFFFFFu;
+            int jb = 0;
+            if (p0) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce0 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 0; } }
+            if (p1) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce1 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 1; } }
+            if (p2) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce2 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 2; } }
+            if (p3) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce3 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 3; } }
+            p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;
+        };
+        while (m != kSentHi && !(T * (1.f - pa) < kTMin)) {
+            if (tie) resolve_tie();
+            do {
+                const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
+                const uint32_t cur = ce & 0xffffu;
+                const uint32_t nx = ce + 16u;
+                const uint32_t nc = nx & 0xffffu;
+                // issue the loads of fragment k
+                const float na = *reinterpret_cast<const float*>(s_ab + cur);
+                float4 nf[FV];
+#pragma unroll
+                for (int v = 0; v < FV; ++v) nf[v] = s_f[(cur >> 4) * FV + v];
+                const uint32_t nh = nc < (nx >> 16) ? s_dk[nc >> 4] : kSentHi;
+                float* ng = ((p0 | p1) ? gTtop : gTbot) + (cur >> 2);
+                if constexpr (DUMP) {
+                    const uint32_t slot = (cur >> 4) - ((p0 | p1) ? bt : bb);
+                    A.sorted_idx[obase + kd] = __float_as_uint(__ldg(&A.Ra[slot]).w);
+                    A.sorted_depth[obase + kd] = m;
+                    if (have) A.sorted_T[obase + kd - 1] = T;      // transmittance in front of fragment k-1
+                    ++kd;
                 }
-                do {
-                    const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
-                    const uint32_t cur = ce & 0xffffu;
-                    const uint32_t nx = ce + 16u;
-                    const uint32_t nc = nx & 0xffffu;
-                    // issue the loads of fragment k
-                    const float na = *reinterpret_cast<const float*>(s_ab + cur);
-                    float4 nf[FV];
-#pragma unroll
-                    for (int v = 0; v < FV; ++v) nf[v] = s_f[(cur >> 4) * FV + v];
-                    const uint32_t nh = nc < (nx >> 16) ? s_dk[nc >> 4] : kSentHi;
-                    float* ng = ((p0 | p1) ? gTtop : gTbot) + (cur >> 2);
-                    // blend fragment k-1
-                    const float c = T * pa;
-                    accA += c;
-#pragma unroll
-                    for (int v = 0; v < FV; ++v) {
-                        acc[4 * v] += c * pf[v].x; acc[4 * v + 1] += c * pf[v].y; acc[4 * v + 2] += c * pf[v].z; acc[4 * v + 3] += c * pf[v].w;
-                    }
-                    if (A.gT && have) *pg = T;
-                    T *= (1.f - pa);
-                    h0 = p0 ? nh : h0; ce0 = p0 ? nx : ce0;
-                    h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;
-                    h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
-                    h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
-                    pa = na; pg = ng; have = true;
-#pragma unroll
-                    for (int v = 0; v < FV; ++v) pf[v] = nf[v];
-                    m = min(min(h0, h1), min(h2, h3));
-                    p0 = h0 == m; p1 = h1 == m; p2 = h2 == m; p3 = h3 == m;
-                    tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
-                } while ((m != kSentHi) & !tie & !(T * (1.f - pa) < kTMin));
-            }
-            if (have) {                                   // the last selected fragment
+                // blend fragment k-1
                 const float c = T * pa;
                 accA += c;
 #pragma unroll
                 for (int v = 0; v < FV; ++v) {
                     acc[4 * v] += c * pf[v].x; acc[4 * v + 1] += c * pf[v].y; acc[4 * v + 2] += c * pf[v].z; acc[4 * v + 3] += c * pf[v].w;
                 }
-                if (A.gT) *pg = T;
-            }
-            consumed = make_uint4(((ce0 & 0xffffu) >> 4) - st0, ((ce1 & 0xffffu) >> 4) - st1,
-                                  ((ce2 & 0xffffu) >> 4) - st2, ((ce3 & 0xffffu) >> 4) - st3);
-        } else {
-            bool blending = true;
-            uint32_t k = 0;
-            const uint32_t obase = DUMP ? A.pixoff[pix] : 0u;
-            while (true) {
-                const uint32_t m = min(min(h0, h1), min(h2, h3));
-                if (m == kSentHi) break;
-                if (DUMP) {
-                    if (blending && T < kTMin) {
-                        blending = false;
-                        consumed = make_uint4(((ce0 & 0xffffu) >> 4) - st0, ((ce1 & 0xffffu) >> 4) - st1,
-                                              ((ce2 & 0xffffu) >> 4) - st2, ((ce3 & 0xffffu) >> 4) - st3);
-                    }
-                } else {
-                    if (T < kTMin) break;                     // fragment k is blended iff T_k >= 1e-4
-                }
-                bool p0 = h0 == m, p1 = h1 == m, p2 = h2 == m, p3 = h3 == m;
-                if ((p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3)) {
-                    uint32_t best = 0xFFFFFFFFu;              // equal depth bits: ascending point index
-                    int jb = 0;
-                    if (p0) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce0 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 0; } }
-                    if (p1) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce1 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 1; } }
-                    if (p2) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce2 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 2; } }
-                    if (p3) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce3 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 3; } }
-                    p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;
-                }
-                const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
-                const uint32_t cur = ce & 0xffffu;
-                if (!DUMP || blending) {
-                    const float a = *reinterpret_cast<const float*>(s_ab + cur);
-                    const float c = T * a;
-                    accA += c;
-    #pragma unroll
-                    for (int v = 0; v < FV; ++v) {
-                        const float4 f = s_f[(cur >> 4) * FV + v];
-                        acc[4 * v] += c * f.x; acc[4 * v + 1] += c * f.y; acc[4 * v + 2] += c * f.z; acc[4 * v + 3] += c * f.w;
-                    }
-                    if (A.gT) ((p0 | p1) ? gTtop : gTbot)[cur >> 2] = T;
-                    T *= (1.f - a);
-                }
-                if (DUMP) {
-                    const uint32_t slot = (cur >> 4) - ((p0 | p1) ? bt : bb);
-                    A.sorted_idx[obase + k] = __float_as_uint(__ldg(&A.Ra[slot]).w);
-                    A.sorted_depth[obase + k] = m;
-                    ++k;
-                }
-                const uint32_t nx = ce + 16u;
-                const uint32_t nc = nx & 0xffffu;
-                const uint32_t nh = nc < (nx >> 16) ? s_dk[nc >> 4] : kSentHi;
+                if (A.gT && have) *pg = T;
+                T *= (1.f - pa);
                 h0 = p0 ? nh : h0; ce0 = p0 ? nx : ce0;
                 h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;
                 h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
                 h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
+                pa = na; pg = ng; have = true;
+#pragma unroll
+                for (int v = 0; v < FV; ++v) pf[v] = nf[v];
+                m = min(min(h0, h1), min(h2, h3));
+                p0 = h0 == m; p1 = h1 == m; p2 = h2 == m; p3 = h3 == m;
+                tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
+            } while ((m != kSentHi) & !tie & !(T * (1.f - pa) < kTMin));
+        }
+        if (have) {                                   // the last selected fragment
+            const float c = T * pa;
+            accA += c;
+#pragma unroll
+            for (int v = 0; v < FV; ++v) {
+                acc[4 * v] += c * pf[v].x; acc[4 * v + 1] += c * pf[v].y; acc[4 * v + 2] += c * pf[v].z; acc[4 * v + 3] += c * pf[v].w;
             }
-            if (!DUMP || blending)
-                consumed = make_uint4(((ce0 & 0xffffu) >> 4) - st0, ((ce1 & 0xffffu) >> 4) - st1,
-                                      ((ce2 & 0xffffu) >> 4) - st2, ((ce3 & 0xffffu) >> 4) - st3);
+            if (A.gT) *pg = T;
+            if constexpr (DUMP) A.sorted_T[obase + kd - 1] = T;
+        }
+        const uint4 consumed = make_uint4(((ce0 & 0xffffu) >> 4) - st0, ((ce1 & 0xffffu) >> 4) - st1,
+                                          ((ce2 & 0xffffu) >> 4) - st2, ((ce3 & 0xffffu) >> 4) - st3);
+        if constexpr (DUMP) {
+            // order-only tail: the fragments behind the cut-off are merged on, recorded and not blended
+            while (m != kSentHi) {
+                if (tie) resolve_tie();
+                const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
+                const uint32_t cur = ce & 0xffffu;
+                const uint32_t nx = ce + 16u;
+                const uint32_t nc = nx & 0xffffu;
+                const uint32_t nh = nc < (nx >> 16) ? s_dk[nc >> 4] : kSentHi;
+                const uint32_t slot = (cur >> 4) - ((p0 | p1) ? bt : bb);
+                A.sorted_idx[obase + kd] = __float_as_uint(__ldg(&A.Ra[slot]).w);
+                A.sorted_depth[obase + kd] = m;
+                A.sorted_T[obase + kd] = -1.f;                     // not blended
+                ++kd;
+                h0 = p0 ? nh : h0; ce0 = p0 ? nx : ce0;
+                h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;
+                h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
+                h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
+                m = min(min(h0, h1), min(h2, h3));
+                p0 = h0 == m; p1 = h1 == m; p2 = h2 == m; p3 = h3 == m;
+                tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
+            }
         }
 #pragma unroll
         for (int v = 0; v < FV; ++v)

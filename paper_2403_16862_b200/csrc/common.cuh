@@ -69,7 +69,9 @@ struct Header {
     uint32_t bigcell_cursor;
     uint32_t bigcell_keys;         // running offset into the large-cell key scratch
     uint32_t cellsort_cursor;
-    uint32_t pad[11];
+    uint32_t bwd_ok;               // written by the backward pass's header check: 1 = the workspace matches its arguments
+    int32_t  status;               // sticky inpc_status of device-side checks (read by inpc_raster_get_status)
+    uint32_t pad[9];
 };
 static_assert(sizeof(Header) % 16 == 0, "header alignment");
 

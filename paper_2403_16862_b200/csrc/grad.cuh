@@ -23,7 +23,8 @@ constexpr int kGradCells   = 1024;
 template <int D> __host__ __device__ constexpr int gpt_floats() { return D == 4 ? 8 : 16; }
 
 template <int D>
-__global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __restrict__ celloff, uint32_t C, int W,
+__global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restrict__ hdr,
+                                                           const uint32_t* __restrict__ celloff, uint32_t C, int W,
                                                            int H, const float4* __restrict__ Ra,
                                                            const float4* __restrict__ gT, const float4* __restrict__ gD,
                                                            const uint4* __restrict__ pcur,
@@ -31,6 +32,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
     constexpr int GP = gpt_floats<D>();
     __shared__ uint32_t s_off[kGradCells + 1];
     const int tid = threadIdx.x;
+    if (!hdr->bwd_ok) return;
     const uint32_t n_units = (C + kGradCells - 1) / kGradCells;
     for (uint32_t unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
         const uint32_t c0 = unit * kGradCells, nc = min((uint32_t)kGradCells, C - c0);
@@ -101,10 +103,12 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const uint32_t* __rest
 }
 
 template <int D>
-__global__ void __launch_bounds__(256) k_split(const float* __restrict__ gpt, const uint32_t* __restrict__ kept,
+__global__ void __launch_bounds__(256) k_split(const Header* __restrict__ hdr, const float* __restrict__ gpt,
+                                                const uint32_t* __restrict__ kept,
                                                 long long N, float* __restrict__ d_feat, float* __restrict__ d_opacity,
                                                 float* __restrict__ d_uv) {
     constexpr int GP = gpt_floats<D>();
+    if (!hdr->bwd_ok) return;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
         float4 f[D / 4], o = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll

@@ -1,15 +1,19 @@
-// inpc_raster.cu -- C ABI (include/inpc_raster.h) over the sm_100a kernels in bin.cuh / tile.cuh / big.cuh.
+// inpc_raster.cu -- C ABI (include/inpc_raster.h) over the sm_100a kernels in bin.cuh / cellsort.cuh /
+// blend.cuh / back.cuh / big.cuh / grad.cuh.
 //
-// Forward  = memset | k_project_count | k_scan_u32 | k_scatter | k_classify | k_cellsort | k_cellsort_big |
-//            [k_scan_u32] | k_build_items | k_tile<fwd> | k_big<fwd>     (all on the caller's stream, no sync)
-// Backward = k_tile<bwd> | k_big<bwd> | k_combine | k_split
-// No device memory is allocated here; there is no CPU fallback.
+// Forward  = memset | k_write_header | k_project_count | k_scan_u32 | k_scatter | k_classify | k_cellsort |
+//            k_cellsort_big x2 | [k_scan_u32 (dump)] | k_build_items | k_blend | k_big<fwd>
+// Backward = k_check_backward | k_back | k_big<bwd> | k_combine | k_split
+// All on the caller's stream, no host synchronisation.  No device memory is allocated here, no state is kept
+// on the host between calls (what a later call needs to know about a workspace is read from the Header the
+// forward pass wrote into it), and there is no CPU fallback.
 #include "../../include/inpc_raster.h"
 
 #include <atomic>
+#include <cstring>
 #include <mutex>
+#include <set>
 #include <string>
-#include <unordered_map>
 #include <vector>
 
 #include "bin.cuh"
@@ -25,6 +29,23 @@ namespace inpc {
 
 static thread_local std::string t_cuda_error;
 static std::atomic<uint64_t> g_launches{0};
+
+// Diagnostics only (inpc_raster_launch_count / inpc_raster_launched_kernels): how many kernels this process
+// has launched and which template instantiations, so that a test can check that the instantiations a
+// benchmark times are the ones the parity tests compared with the oracle.
+static std::mutex g_names_mu;
+static std::set<std::string> g_names;
+static void note_launch(const std::string& name) {
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    std::lock_guard<std::mutex> lk(g_names_mu);
+    g_names.insert(name);
+}
+template <int... V> static std::string kname(const char* base) {
+    std::string s = base; s += "<";
+    const int v[] = {V...};
+    for (size_t i = 0; i < sizeof...(V); ++i) { if (i) s += ","; s += std::to_string(v[i]); }
+    return s + ">";
+}
 
 // ---- optional per-stage device timing (inpc_raster_set_kernel_timing) ---------------------------------
 // Every stage the library enqueues is bracketed by two cudaEvents on the caller's stream; the
@@ -66,7 +87,7 @@ struct Layout {
     size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
     size_t kept, cursor, A, gT, gD, dk, Ra, Rf, items, bigpix, bigcells, bigkeys;
     size_t pcur, gpt;                                     // only with INPC_SAVE_FOR_BACKWARD
-    size_t pixoff, sorted_idx, sorted_depth;              // only with INPC_SAVE_SORTED
+    size_t pixoff, sorted_idx, sorted_depth, sorted_T;    // only with INPC_SAVE_SORTED
     size_t total;
     uint32_t C, P, max_big_cells, n_status;
 };
@@ -106,26 +127,24 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
         L.pixoff = o;       o = align_up(o + ((size_t)L.P + 1) * 4);
         L.sorted_idx = o;   o = align_up(o + (4 * n + 8) * 4);
         L.sorted_depth = o; o = align_up(o + (4 * n + 8) * 4);
+        L.sorted_T = o;     o = align_up(o + (4 * n + 8) * 4);
     }
     L.total = o;
     return L;
 }
 
-// Host-side note of what the last forward left in a workspace (argument validation only; the
-// library keeps no device state and allocates nothing).
-struct Saved { int64_t N; int D, W, H; uint32_t flags; };
-static std::mutex g_mu;
-static std::unordered_map<const void*, Saved> g_saved;
-
-struct DeviceInfo { int sms = 0; bool ok = false; };
+constexpr int kMaxDevices = 64;
+struct DeviceInfo { int dev = 0; int sms = 0; bool ok = false; };
+static std::mutex g_dev_mu;                       // guards the per-device caches below
 static DeviceInfo device_info() {
-    static DeviceInfo cached[64];
+    static DeviceInfo cached[kMaxDevices];
     int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return DeviceInfo{};
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return DeviceInfo{};
+    std::lock_guard<std::mutex> lk(g_dev_mu);
     if (!cached[dev].ok) {
         int sms = 0;
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return DeviceInfo{};
-        cached[dev].sms = sms; cached[dev].ok = true;
+        cached[dev].dev = dev; cached[dev].sms = sms; cached[dev].ok = true;
     }
     return cached[dev];
 }
@@ -135,7 +154,7 @@ static int cuda_fail(cudaError_t e) {
     return INPC_ERR_CUDA;
 }
 #define INPC_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
-#define INPC_LAUNCHED() do { g_launches.fetch_add(1, std::memory_order_relaxed); cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
+#define INPC_LAUNCHED(...) do { note_launch(__VA_ARGS__); cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -157,47 +176,48 @@ static Camera to_camera(const inpc_camera* c) {
     return k;
 }
 
+// Opt-in dynamic shared memory and the persistent grid size (resident CTAs per SM x SMs) of one kernel, cached
+// PER DEVICE (both are per-device properties): grid_by_dev is the kernel's own function-static table.
 template <typename K>
-static int persistent_grid(K kernel, int threads, size_t smem, int sms, int* out) {
-    int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem);
-    if (e != cudaSuccess) return cuda_fail(e);
-    if (per_sm < 1) per_sm = 1;
-    *out = per_sm * sms;
+static int persistent_grid(K kernel, int threads, size_t smem, const DeviceInfo& di, int (&grid_by_dev)[kMaxDevices],
+                           int* out) {
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    if (grid_by_dev[di.dev] == 0) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return cuda_fail(e);
+        int per_sm = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem);
+        if (e != cudaSuccess) return cuda_fail(e);
+        if (per_sm < 1) per_sm = 1;
+        grid_by_dev[di.dev] = per_sm * di.sms;
+    }
+    *out = grid_by_dev[di.dev];
     return INPC_OK;
 }
 
 template <int D>
-static int launch_back(const BackArgs& A, int sms, cudaStream_t st) {
+static int launch_back(const BackArgs& A, const DeviceInfo& di, cudaStream_t st) {
     constexpr size_t smem = back_smem_bytes<D>();
-    static bool configured = false;
-    static int grid = 0;
-    if (!configured) {
-        INPC_CUDA(cudaFuncSetAttribute(k_back<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int rc = persistent_grid(k_back<D>, kTileThreads, smem, sms, &grid);
-        if (rc != INPC_OK) return rc;
-        configured = true;
-    }
+    static int grid_by_dev[kMaxDevices] = {};
+    int grid = 0;
+    int rc = persistent_grid(k_back<D>, kTileThreads, smem, di, grid_by_dev, &grid);
+    if (rc != INPC_OK) return rc;
     { StageTimer tm(kStTileBwd, st);
       k_back<D><<<grid, kTileThreads, smem, st>>>(A); }
-    INPC_LAUNCHED();
+    INPC_LAUNCHED(kname<D>("k_back"));
     return INPC_OK;
 }
 
 template <int D, bool DUMP>
-static int launch_blend(const BlendArgs& A, int sms, cudaStream_t st) {
+static int launch_blend(const BlendArgs& A, const DeviceInfo& di, cudaStream_t st) {
     constexpr size_t smem = blend_smem_bytes<D>();
-    static bool configured = false;
-    static int grid = 0;
-    if (!configured) {
-        INPC_CUDA(cudaFuncSetAttribute(k_blend<D, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int rc = persistent_grid(k_blend<D, DUMP>, kTileThreads, smem, sms, &grid);
-        if (rc != INPC_OK) return rc;
-        configured = true;
-    }
+    static int grid_by_dev[kMaxDevices] = {};
+    int grid = 0;
+    int rc = persistent_grid(k_blend<D, DUMP>, kTileThreads, smem, di, grid_by_dev, &grid);
+    if (rc != INPC_OK) return rc;
     { StageTimer tm(kStTileFwd, st);
       k_blend<D, DUMP><<<grid, kTileThreads, smem, st>>>(A); }
-    INPC_LAUNCHED();
+    INPC_LAUNCHED(kname<D, DUMP ? 1 : 0>("k_blend"));
     return INPC_OK;
 }
 
@@ -205,44 +225,54 @@ template <int D, int MODE>
 static int launch_big(const BigArgs& A, int sms, cudaStream_t st) {
     { StageTimer tm(MODE == kBwd ? kStBigBwd : kStBigFwd, st);
       k_big<D, MODE><<<sms * 8, kLongThreads, 0, st>>>(A); }
-    INPC_LAUNCHED();
+    INPC_LAUNCHED(kname<D, MODE>("k_big"));
     return INPC_OK;
 }
 
 template <int D, int THREADS, int CHUNK>
 static int launch_cellsort_big_class(const Header* hdr, uint32_t n_lo, uint32_t n_hi, uint32_t* cursor,
                                      const BigCell* bigcells, const float4* A, unsigned long long* keys, const float* feat,
-                                     uint32_t* dk, float4* Ra, float4* Rf, int sms, uint32_t max_big_cells, cudaStream_t st) {
+                                     uint32_t* dk, float4* Ra, float4* Rf, const DeviceInfo& di, uint32_t max_big_cells,
+                                     cudaStream_t st) {
     constexpr size_t smem = (size_t)CHUNK * 8;
-    static bool configured = false;
-    static int grid = 0;
-    if (!configured) {
-        INPC_CUDA(cudaFuncSetAttribute(k_cellsort_big<D, THREADS, CHUNK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int rc = persistent_grid(k_cellsort_big<D, THREADS, CHUNK>, THREADS, smem, sms, &grid);
-        if (rc != INPC_OK) return rc;
-        configured = true;
-    }
+    static int grid_by_dev[kMaxDevices] = {};
+    int grid = 0;
+    int rc = persistent_grid(k_cellsort_big<D, THREADS, CHUNK>, THREADS, smem, di, grid_by_dev, &grid);
+    if (rc != INPC_OK) return rc;
     const int g = (int)std::min<uint32_t>((uint32_t)grid, std::max<uint32_t>(max_big_cells, 1u));
     k_cellsort_big<D, THREADS, CHUNK><<<g, THREADS, smem, st>>>(hdr, n_lo, n_hi, cursor, bigcells, A, keys, feat, dk, Ra, Rf);
-    INPC_LAUNCHED();
+    INPC_LAUNCHED(kname<D, CHUNK>("k_cellsort_big"));
     return INPC_OK;
 }
 
 // cells of kCellSmall+1 .. 1024 points, then the larger ones (two work cursors in the header)
 template <int D>
 static int launch_cellsort_big(Header* hdr, const BigCell* bigcells, const float4* A, unsigned long long* keys,
-                               const float* feat, uint32_t* dk, float4* Ra, float4* Rf, int sms, uint32_t max_big_cells,
-                               cudaStream_t st) {
+                               const float* feat, uint32_t* dk, float4* Ra, float4* Rf, const DeviceInfo& di,
+                               uint32_t max_big_cells, cudaStream_t st) {
     StageTimer tm(kStCellSortBig, st);
     int rc = launch_cellsort_big_class<D, 128, 1024>(hdr, 0u, 1024u, &hdr->bigcell_cursor, bigcells, A, keys, feat, dk, Ra,
-                                                     Rf, sms, max_big_cells, st);
+                                                     Rf, di, max_big_cells, st);
     if (rc != INPC_OK) return rc;
     return launch_cellsort_big_class<D, kBigThreads, kBigChunk>(hdr, 1025u, 0xFFFFFFFFu, &hdr->cellsort_cursor, bigcells, A,
-                                                                keys, feat, dk, Ra, Rf, sms, max_big_cells, st);
+                                                                keys, feat, dk, Ra, Rf, di, max_big_cells, st);
 }
 
 __global__ void k_write_header(Header* h, uint32_t flags, int W, int H, int D, uint32_t N) {
     h->magic = kMagic; h->flags = flags; h->W = W; h->H = H; h->D = D; h->n_points = N;
+}
+
+// First kernel of the backward pass: does the workspace hold the forward state these arguments describe?
+// bwd_ok gates every later backward kernel (they return at once when it is 0, so a stale or foreign
+// workspace is never interpreted); the reason is left in the sticky status word that
+// inpc_raster_get_status returns.  Also resets the tile work cursor.
+__global__ void k_check_backward(Header* h, int W, int H, int D, uint32_t N) {
+    int32_t st = INPC_OK;
+    if (h->magic != kMagic || !(h->flags & INPC_SAVE_FOR_BACKWARD)) st = INPC_ERR_NO_SAVED_STATE;
+    else if (h->W != W || h->H != H || h->D != D || h->n_points != N) st = INPC_ERR_INVALID_ARG;
+    h->bwd_ok = st == INPC_OK ? 1u : 0u;
+    if (st != INPC_OK) h->status = st;
+    h->item_cursor = 0;
 }
 
 template <int D>
@@ -271,7 +301,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     { StageTimer tm(kStZeroFwd, st);
       INPC_CUDA(cudaMemsetAsync(ws + L.header, 0, L.zero_end - L.header, st));
       k_write_header<<<1, 1, 0, st>>>(hdr, flags, W, H, D, (uint32_t)N); }
-    INPC_LAUNCHED();
+    INPC_LAUNCHED("k_write_header");
     // grid sizes in CTAs per SM are measured optima (profiles/r01_v3b_sector_stores.md): the passes that scatter
     // (k_scatter, k_cellsort) are fastest with ONE resident wave of 4 CTAs per SM, the streaming count pass with 8
     const int bin_grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
@@ -279,28 +309,28 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     if (N > 0) {
         { StageTimer tm(kStProjectCount, st);
           k_project_count<<<bin_grid, kBinThreads, 0, st>>>(pos, (long long)N, camk, cellcnt, kept); }
-        INPC_LAUNCHED();
+        INPC_LAUNCHED("k_project_count");
     }
     { StageTimer tm(kStScan, st);
       k_scan_u32<<<(L.C + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
           cellcnt, L.C, reinterpret_cast<unsigned long long*>(ws + L.status0), &hdr->scan_tile_counter, &hdr->nrec, cursor); }
-    INPC_LAUNCHED();
+    INPC_LAUNCHED("k_scan_u32");
     if (N > 0) {
         { StageTimer tm(kStScatter, st);
           k_scatter<<<scatter_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cursor, Arec); }
-        INPC_LAUNCHED();
+        INPC_LAUNCHED("k_scatter");
     }
     { StageTimer tm(kStClassify, st);
       k_classify<<<(L.C + 255) / 256, 256, 0, st>>>(cellcnt, W, H, hdr, bigcells, pixoff); }
-    INPC_LAUNCHED();
+    INPC_LAUNCHED("k_classify");
     if (N > 0) {
         const uint32_t n_units = (L.C + kCsCells - 1) / kCsCells;
         { StageTimer tm(kStCellSort, st);
           k_cellsort<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 4), kCsThreads, 0, st>>>(
               Arec, cellcnt, L.C, feat, dk, Ra, Rf); }
-        INPC_LAUNCHED();
+        INPC_LAUNCHED(kname<D>("k_cellsort"));
         int rc = launch_cellsort_big<D>(hdr, bigcells, Arec,
-                                        reinterpret_cast<unsigned long long*>(ws + L.bigkeys), feat, dk, Ra, Rf, di.sms,
+                                        reinterpret_cast<unsigned long long*>(ws + L.bigkeys), feat, dk, Ra, Rf, di,
                                         L.max_big_cells, st);
         if (rc != INPC_OK) return rc;
     }
@@ -308,12 +338,12 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
         { StageTimer tm(kStOther, st);
           k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
               pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr, nullptr); }
-        INPC_LAUNCHED();
+        INPC_LAUNCHED("k_scan_u32");
     }
     const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
     { StageTimer tm(kStBuildItems, st);
       k_build_items<<<(ntx * nty + 127) / 128, 128, 0, st>>>(cellcnt, W, H, TileCfg<D>::kCap, hdr, items, bigpix); }
-    INPC_LAUNCHED();
+    INPC_LAUNCHED("k_build_items");
 
     BlendArgs A{};
     A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = items; A.celloff = cellcnt; A.dk = dk; A.Ra = Ra; A.Rf = Rf;
@@ -329,8 +359,9 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
         B.pixoff = A.pixoff = pixoff;
         B.sorted_idx = A.sorted_idx = reinterpret_cast<uint32_t*>(ws + L.sorted_idx);
         B.sorted_depth = A.sorted_depth = reinterpret_cast<uint32_t*>(ws + L.sorted_depth);
+        B.sorted_T = A.sorted_T = reinterpret_cast<float*>(ws + L.sorted_T);
     }
-    int rc = dump ? launch_blend<D, true>(A, di.sms, st) : launch_blend<D, false>(A, di.sms, st);
+    int rc = dump ? launch_blend<D, true>(A, di, st) : launch_blend<D, false>(A, di, st);
     if (rc != INPC_OK) return rc;
     if (N > 0) rc = dump ? launch_big<D, kFwdDump>(B, di.sms, st) : launch_big<D, kFwd>(B, di.sms, st);
     return rc;
@@ -343,10 +374,9 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     if (!di.ok) return cuda_fail(cudaErrorNoDevice);
     const int W = cam->width, H = cam->height;
     Header* hdr = reinterpret_cast<Header*>(ws + L.header);
-    {
-        StageTimer tm(kStZeroBwd, st);
-        INPC_CUDA(cudaMemsetAsync(&hdr->item_cursor, 0, 4, st));
-    }
+    { StageTimer tm(kStZeroBwd, st);
+      k_check_backward<<<1, 1, 0, st>>>(hdr, W, H, D, (uint32_t)N); }
+    INPC_LAUNCHED("k_check_backward");
     if (N == 0) return INPC_OK;
     const uint32_t* celloff = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
     const float4* Ra = reinterpret_cast<float4*>(ws + L.Ra);
@@ -359,7 +389,7 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = reinterpret_cast<uint32_t*>(ws + L.items);
     A.celloff = celloff; A.dk = reinterpret_cast<uint32_t*>(ws + L.dk); A.Ra = Ra; A.Rf = Rf;
     A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD;
-    int rc = launch_back<D>(A, di.sms, st);
+    int rc = launch_back<D>(A, di, st);
     if (rc != INPC_OK) return rc;
     BigArgs B{};
     B.hdr = hdr; B.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); B.celloff = celloff; B.dk = A.dk; B.Ra = Ra; B.Rf = Rf;
@@ -369,12 +399,12 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     const uint32_t n_units = (L.C + kGradCells - 1) / kGradCells;
     { StageTimer tm(kStCombine, st);
       k_combine<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 8), kGradThreads, 0, st>>>(
-          celloff, L.C, W, H, Ra, reinterpret_cast<const float4*>(gT), reinterpret_cast<const float4*>(gD), pcur, g_feat, gpt); }
-    INPC_LAUNCHED();
+          hdr, celloff, L.C, W, H, Ra, reinterpret_cast<const float4*>(gT), reinterpret_cast<const float4*>(gD), pcur, g_feat, gpt); }
+    INPC_LAUNCHED(kname<D>("k_combine"));
     { StageTimer tm(kStSplit, st);
       k_split<D><<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16), 256, 0, st>>>(
-          gpt, reinterpret_cast<const uint32_t*>(ws + L.kept), (long long)N, d_feat, d_opacity, d_uv); }
-    INPC_LAUNCHED();
+          hdr, gpt, reinterpret_cast<const uint32_t*>(ws + L.kept), (long long)N, d_feat, d_opacity, d_uv); }
+    INPC_LAUNCHED(kname<D>("k_split"));
     return INPC_OK;
 }
 
@@ -401,19 +431,10 @@ int inpc_raster_forward(const float* pos, const float* opacity, const float* fea
         return INPC_ERR_INVALID_ARG;
     const Layout L = make_layout(N, D, cam->width, cam->height, flags);
     if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
-    {
-        std::lock_guard<std::mutex> lk(g_mu);
-        g_saved.erase(workspace);
-    }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     unsigned char* ws = static_cast<unsigned char*>(workspace);
-    rc = D == 4 ? forward_impl<4>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st)
-                : forward_impl<8>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st);
-    if (rc == INPC_OK) {
-        std::lock_guard<std::mutex> lk(g_mu);
-        g_saved[workspace] = Saved{N, D, cam->width, cam->height, flags};
-    }
-    return rc;
+    return D == 4 ? forward_impl<4>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st)
+                  : forward_impl<8>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st);
 }
 
 int inpc_raster_backward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
@@ -426,18 +447,12 @@ int inpc_raster_backward(const float* pos, const float* opacity, const float* fe
     if (!grad_out_feat || !workspace) return INPC_ERR_INVALID_ARG;
     if (N > 0 && (!grad_feat || !grad_opacity || !grad_uv)) return INPC_ERR_INVALID_ARG;
     if (!aligned16(grad_out_feat) || !aligned16(grad_out_alpha) || !aligned16(grad_feat) || !aligned16(grad_opacity) ||
-        !aligned16(grad_uv))
+        !aligned16(grad_uv) || (reinterpret_cast<uintptr_t>(workspace) & 255u))
         return INPC_ERR_INVALID_ARG;
-    Saved s;
-    {
-        std::lock_guard<std::mutex> lk(g_mu);
-        auto it = g_saved.find(workspace);
-        if (it == g_saved.end()) return INPC_ERR_NO_SAVED_STATE;
-        s = it->second;
-    }
-    if (!(s.flags & INPC_SAVE_FOR_BACKWARD)) return INPC_ERR_NO_SAVED_STATE;
-    if (s.N != N || s.D != D || s.W != cam->width || s.H != cam->height) return INPC_ERR_INVALID_ARG;
-    const Layout L = make_layout(N, D, s.W, s.H, s.flags);
+    // Everything the backward pass touches lies in front of the INPC_SAVE_SORTED arrays, so its layout follows
+    // from these arguments alone; whether the workspace really holds that forward is checked ON THE DEVICE
+    // (k_check_backward) against the Header the forward wrote -- no host-side record of workspaces exists.
+    const Layout L = make_layout(N, D, cam->width, cam->height, INPC_SAVE_FOR_BACKWARD);
     if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     unsigned char* ws = static_cast<unsigned char*>(workspace);
@@ -445,38 +460,54 @@ int inpc_raster_backward(const float* pos, const float* opacity, const float* fe
                   : backward_impl<8>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, ws, L, st);
 }
 
-static int find_saved(const void* workspace, int32_t W, int32_t H, Saved* out) {
-    std::lock_guard<std::mutex> lk(g_mu);
-    auto it = g_saved.find(workspace);
-    if (it == g_saved.end()) return INPC_ERR_NO_SAVED_STATE;
-    if (W > 0 && (it->second.W != W || it->second.H != H)) return INPC_ERR_INVALID_ARG;
-    *out = it->second;
+// The introspection calls synchronise: they read the workspace's Header back and take shape, D and flags from it.
+static int read_header(const void* workspace, int32_t W, int32_t H, cudaStream_t st, Header* h) {
+    INPC_CUDA(cudaMemcpyAsync(h, workspace, sizeof(Header), cudaMemcpyDeviceToHost, st));
+    INPC_CUDA(cudaStreamSynchronize(st));
+    if (h->magic != kMagic) return INPC_ERR_NO_SAVED_STATE;
+    if (W > 0 && (h->W != W || h->H != H)) return INPC_ERR_INVALID_ARG;
     return INPC_OK;
+}
+
+int inpc_raster_get_status(const void* workspace, void* cuda_stream) {
+    if (!workspace) return INPC_ERR_INVALID_ARG;
+    Header h;
+    int rc = read_header(workspace, 0, 0, static_cast<cudaStream_t>(cuda_stream), &h);
+    return rc != INPC_OK ? rc : h.status;
 }
 
 int inpc_raster_get_counts(const void* workspace, int32_t W, int32_t H, uint32_t* counts, void* cuda_stream) {
     if (!workspace || !counts || W <= 0 || H <= 0) return INPC_ERR_INVALID_ARG;
-    Saved s;
-    int rc = find_saved(workspace, W, H, &s);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Header h;
+    int rc = read_header(workspace, W, H, st, &h);
     if (rc != INPC_OK) return rc;
-    const Layout L = make_layout(s.N, s.D, s.W, s.H, s.flags);
+    const Layout L = make_layout(h.n_points, h.D, h.W, h.H, h.flags);
     const unsigned char* ws = static_cast<const unsigned char*>(workspace);
-    k_counts_out<<<(L.P + 255) / 256, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
-        reinterpret_cast<const uint32_t*>(ws + L.cellcnt), W, H, counts);
-    INPC_LAUNCHED();
+    k_counts_out<<<(L.P + 255) / 256, 256, 0, st>>>(reinterpret_cast<const uint32_t*>(ws + L.cellcnt), W, H, counts);
+    INPC_LAUNCHED("k_counts_out");
+    return INPC_OK;
+}
+
+int inpc_raster_get_blended_counts(const void* workspace, int32_t W, int32_t H, uint32_t* blended, void* cuda_stream) {
+    if (!workspace || !blended || W <= 0 || H <= 0) return INPC_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Header h;
+    int rc = read_header(workspace, W, H, st, &h);
+    if (rc != INPC_OK) return rc;
+    if (!(h.flags & INPC_SAVE_FOR_BACKWARD)) return INPC_ERR_NO_SAVED_STATE;
+    const Layout L = make_layout(h.n_points, h.D, h.W, h.H, h.flags);
+    const unsigned char* ws = static_cast<const unsigned char*>(workspace);
+    k_blended_out<<<(L.P + 255) / 256, 256, 0, st>>>(reinterpret_cast<const uint4*>(ws + L.pcur), L.P, blended);
+    INPC_LAUNCHED("k_blended_out");
     return INPC_OK;
 }
 
 int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_stream) {
     if (!workspace || !stats) return INPC_ERR_INVALID_ARG;
-    Saved s;
-    int rc = find_saved(workspace, 0, 0, &s);
-    if (rc != INPC_OK) return rc;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     Header h;
-    INPC_CUDA(cudaMemcpyAsync(&h, workspace, sizeof(Header), cudaMemcpyDeviceToHost, st));
-    INPC_CUDA(cudaStreamSynchronize(st));
-    if (h.magic != kMagic) return INPC_ERR_NO_SAVED_STATE;
+    int rc = read_header(workspace, 0, 0, static_cast<cudaStream_t>(cuda_stream), &h);
+    if (rc != INPC_OK) return rc;
     stats->n_points = h.n_points;
     stats->n_kept = h.nrec;
     stats->n_fragments = h.n_fragments;
@@ -488,19 +519,15 @@ int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_s
 }
 
 int inpc_raster_get_sorted(const void* workspace, int32_t W, int32_t H, uint32_t* offsets, uint32_t* point_idx,
-                           uint32_t* depth_bits, uint64_t* total, void* cuda_stream) {
+                           uint32_t* depth_bits, float* transmittance, uint64_t* total, void* cuda_stream) {
     if (!workspace || !total || W <= 0 || H <= 0) return INPC_ERR_INVALID_ARG;
-    Saved s;
-    int rc = find_saved(workspace, W, H, &s);
-    if (rc != INPC_OK) return rc;
-    if (!(s.flags & INPC_SAVE_SORTED)) return INPC_ERR_NO_SAVED_STATE;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const Layout L = make_layout(s.N, s.D, s.W, s.H, s.flags);
-    const unsigned char* ws = static_cast<const unsigned char*>(workspace);
     Header h;
-    INPC_CUDA(cudaMemcpyAsync(&h, ws, sizeof(Header), cudaMemcpyDeviceToHost, st));
-    INPC_CUDA(cudaStreamSynchronize(st));
-    if (h.magic != kMagic) return INPC_ERR_NO_SAVED_STATE;
+    int rc = read_header(workspace, W, H, st, &h);
+    if (rc != INPC_OK) return rc;
+    if (!(h.flags & INPC_SAVE_SORTED)) return INPC_ERR_NO_SAVED_STATE;
+    const Layout L = make_layout(h.n_points, h.D, h.W, h.H, h.flags);
+    const unsigned char* ws = static_cast<const unsigned char*>(workspace);
     *total = h.n_fragments;
     if (!offsets) return INPC_OK;
     if (!point_idx || !depth_bits) return INPC_ERR_INVALID_ARG;
@@ -508,6 +535,8 @@ int inpc_raster_get_sorted(const void* workspace, int32_t W, int32_t H, uint32_t
     if (h.n_fragments) {
         INPC_CUDA(cudaMemcpyAsync(point_idx, ws + L.sorted_idx, (size_t)h.n_fragments * 4, cudaMemcpyDeviceToDevice, st));
         INPC_CUDA(cudaMemcpyAsync(depth_bits, ws + L.sorted_depth, (size_t)h.n_fragments * 4, cudaMemcpyDeviceToDevice, st));
+        if (transmittance)
+            INPC_CUDA(cudaMemcpyAsync(transmittance, ws + L.sorted_T, (size_t)h.n_fragments * 4, cudaMemcpyDeviceToDevice, st));
     }
     INPC_CUDA(cudaStreamSynchronize(st));
     return INPC_OK;
@@ -559,5 +588,18 @@ int inpc_raster_get_kernel_times(double* ms, uint64_t* launches, int reset) {
 const char* inpc_raster_last_cuda_error(void) { return t_cuda_error.c_str(); }
 
 uint64_t inpc_raster_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+size_t inpc_raster_launched_kernels(char* buf, size_t buf_bytes, int reset) {
+    std::lock_guard<std::mutex> lk(g_names_mu);
+    std::string all;
+    for (const std::string& n : g_names) { if (!all.empty()) all += ";"; all += n; }
+    if (reset) g_names.clear();
+    if (buf && buf_bytes) {
+        const size_t k = std::min(buf_bytes - 1, all.size());
+        std::memcpy(buf, all.data(), k);
+        buf[k] = 0;
+    }
+    return all.size() + 1;
+}
 
 }  // extern "C"

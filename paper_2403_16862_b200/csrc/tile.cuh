@@ -1,52 +1,25 @@
-// tile.cuh -- steps a4/a5 of the hot path: per-pixel 4-way merge of the sorted cell lists, front-to-back
-// compositing (Eq. 1) and the reverse-traversal backward pass.
+// tile.cuh -- per-pixel merge routines of the LONG-RUN path (big.cuh), steps a4/a5 of the hot path.
 //
-// One persistent CTA per work item (a screen tile of tw x th <= 128 pixels whose records fit in shared
-// memory).  The tile's th+1 cell rows are contiguous slot ranges of the cell-sorted arrays dk / R (/ gT)
-// and are staged with cp.async.bulk (TMA, 1-D) onto one mbarrier.  Then ONE THREAD PER PIXEL:
-//   a4  the pixel's four cell lists are already sorted by (depth bits, point index), so its blend order
-//       is their merge: keep the four head keys in registers, take the minimum (equal depth bits: the
-//       smaller point index), composite that fragment, advance that list.  The loop ends at the cut-off
-//       T < 1e-4 -- nothing behind it is even read.  With INPC_SAVE_FOR_BACKWARD the transmittance in
-//       front of every blended fragment goes to gT[(slot, corner)] and the four list positions at the
-//       stop to pcur[pixel].
-//   a5  backward: start from pcur and merge the four lists BACKWARDS (maximum first), reading T from
-//       the staged gT; division-free recurrence  dL/da_k = T_k (G_k - B_k),  B_{k-1} = a_k G_k + (1-a_k) B_k.
-//       dL/da goes to gD[(slot, corner)]; grad.cuh combines the four corners of every record.
-// Why one thread per pixel and not one warp (the paper's choice, and this repo's first version):
-// profiles/r01_v1_baseline.md -- the warp-wide sort + scan spent ~38 warp instructions per fragment; the
-// sequential merge spends ~1.5, has no shuffles, no per-warp scratch and no lane waste on shallow pixels.
+// The tile kernels k_blend (blend.cuh) and k_back (back.cuh) carry their own software-pipelined, shared-memory
+// versions of these loops; what is left here is the plain form, read straight from global memory, that
+// k_big uses for the pixels whose neighbourhood does not fit a shared-memory tile:
+//   blend_pixel     a4: the pixel's four cell lists are sorted by (depth bits, point index), so its blend order
+//                   is their merge: keep the four head keys in registers, take the minimum (equal depth bits:
+//                   the smaller point index), composite that fragment (Eq. 1), advance that list.
+//                   The loop ends at the cut-off T < 1e-4 -- nothing behind it is even read (unless DUMP asks
+//                   for the whole order).  With INPC_SAVE_FOR_BACKWARD the transmittance in front of every
+//                   blended fragment goes to gT[(slot, corner)] and the four list positions at the stop to
+//                   pcur[pixel].
+//   backward_pixel  a5: start from pcur and merge the four lists BACKWARDS (maximum first),
+//                   reading T from gT; division-free recurrence
+//                   dL/da_k = T_k (G_k - B_k),  B_{k-1} = a_k G_k + (1 - a_k) B_k.
+//                   dL/da goes to gD[(slot, corner)]; grad.cuh combines the four corners of every record.
 #pragma once
 #include "common.cuh"
 
 namespace inpc {
 
 enum TileMode { kFwd = 0, kFwdDump = 1, kBwd = 2 };
-
-struct TileArgs {
-    const Header* hdr;
-    uint32_t* item_cursor;
-    const uint32_t* items;
-    const uint32_t* celloff;
-    const uint32_t* dk;
-    const float4* Ra;
-    const float4* Rf;
-    int W, H;
-    // forward
-    float* out_feat;
-    float* out_alpha;
-    float* gT;               // NULL unless INPC_SAVE_FOR_BACKWARD
-    uint4* pcur;
-    // dump (INPC_SAVE_SORTED)
-    const uint32_t* pixoff;
-    uint32_t* sorted_idx;
-    uint32_t* sorted_depth;
-    // backward
-    const float* g_feat;
-    const float* g_alpha;
-    float* gD;
-};
-
 
 // The four lists of one pixel as cursors into dk / R (shared-memory indices in the tile kernel, global
 // slots in the long-run path).  Lists 0, 1 lie in cell row y, lists 2, 3 in cell row y+1.
@@ -58,7 +31,8 @@ template <int D, bool DUMP, typename TT>
 __device__ __forceinline__ void blend_pixel(const uint32_t* dk, const float4* Ra, const float4* Rf, PixLists L, uint32_t gofs_top,
                                             uint32_t gofs_bot, float* __restrict__ gT, float (&acc)[D], float& accA,
                                             uint4& consumed, uint32_t* __restrict__ sorted_idx,
-                                            uint32_t* __restrict__ sorted_depth, uint32_t obase) {
+                                            uint32_t* __restrict__ sorted_depth, float* __restrict__ sorted_T,
+                                            uint32_t obase) {
     constexpr int FV = D / 4;
     const uint32_t s0 = L.c0, s1 = L.c1, s2 = L.c2, s3 = L.c3;
     uint32_t c0 = L.c0, c1 = L.c1, c2 = L.c2, c3 = L.c3;
@@ -101,7 +75,10 @@ __device__ __forceinline__ void blend_pixel(const uint32_t* dk, const float4* Ra
                 acc[4 * v] += c * f.x; acc[4 * v + 1] += c * f.y; acc[4 * v + 2] += c * f.z; acc[4 * v + 3] += c * f.w;
             }
             if (gT) gT[(size_t)(ref + ((j & 2) ? gofs_bot : gofs_top)) * 4 + (3 - j)] = (float)T;
+            if (DUMP) sorted_T[obase + k] = (float)T;
             T *= (TT)(1.f - a);
+        } else if (DUMP) {
+            sorted_T[obase + k] = -1.f;                  // behind the cut-off: recorded, not blended
         }
         if (DUMP) {
             sorted_idx[obase + k] = __float_as_uint(r0.w);

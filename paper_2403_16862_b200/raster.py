@@ -19,8 +19,9 @@ SAVE_SORTED = 2
 
 EXPORTS = (
     "inpc_raster_workspace_bytes", "inpc_raster_forward", "inpc_raster_backward",
-    "inpc_raster_get_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
-    "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count",
+    "inpc_raster_get_counts", "inpc_raster_get_blended_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
+    "inpc_raster_get_status",
+    "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count", "inpc_raster_launched_kernels",
     "inpc_raster_set_kernel_timing", "inpc_raster_kernel_count", "inpc_raster_kernel_name",
     "inpc_raster_get_kernel_times",
 )
@@ -68,14 +69,20 @@ def load() -> C.CDLL:
         lib.inpc_raster_backward.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
         lib.inpc_raster_get_counts.restype = C.c_int
         lib.inpc_raster_get_counts.argtypes = [vp, i32, i32, vp, vp]
+        lib.inpc_raster_get_blended_counts.restype = C.c_int
+        lib.inpc_raster_get_blended_counts.argtypes = [vp, i32, i32, vp, vp]
+        lib.inpc_raster_get_status.restype = C.c_int
+        lib.inpc_raster_get_status.argtypes = [vp, vp]
         lib.inpc_raster_get_sorted.restype = C.c_int
-        lib.inpc_raster_get_sorted.argtypes = [vp, i32, i32, vp, vp, vp, C.POINTER(C.c_uint64), vp]
+        lib.inpc_raster_get_sorted.argtypes = [vp, i32, i32, vp, vp, vp, vp, C.POINTER(C.c_uint64), vp]
         lib.inpc_raster_get_stats.restype = C.c_int
         lib.inpc_raster_get_stats.argtypes = [vp, C.POINTER(InpcStats), vp]
         lib.inpc_raster_strerror.restype = C.c_char_p
         lib.inpc_raster_strerror.argtypes = [C.c_int]
         lib.inpc_raster_last_cuda_error.restype = C.c_char_p
         lib.inpc_raster_launch_count.restype = C.c_uint64
+        lib.inpc_raster_launched_kernels.restype = C.c_size_t
+        lib.inpc_raster_launched_kernels.argtypes = [C.c_char_p, C.c_size_t, C.c_int]
         lib.inpc_raster_set_kernel_timing.argtypes = [C.c_int]
         lib.inpc_raster_kernel_name.restype = C.c_char_p
         lib.inpc_raster_kernel_name.argtypes = [C.c_int]
@@ -177,11 +184,25 @@ def inpc_raster_get_counts(workspace, W: int, H: int, stream=None) -> torch.Tens
     return counts
 
 
-def inpc_raster_get_sorted(workspace, W: int, H: int, stream=None):
-    """-> offsets[H*W+1], point_idx[total], depth_bits[total] (int32 tensors holding the u32 bit patterns)."""
+def inpc_raster_get_blended_counts(workspace, W: int, H: int, stream=None) -> torch.Tensor:
+    nb = torch.empty((H, W), dtype=torch.int32, device=workspace.device)
+    rc = load().inpc_raster_get_blended_counts(_ptr(workspace), W, H, _ptr(nb), _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_get_blended_counts")
+    return nb
+
+
+def inpc_raster_get_status(workspace, stream=None) -> int:
+    """Sticky status of the device-side checks (0 = ok); synchronises."""
+    return int(load().inpc_raster_get_status(_ptr(workspace), _stream(stream)))
+
+
+def inpc_raster_get_sorted(workspace, W: int, H: int, stream=None, transmittance: bool = False):
+    """-> offsets[H*W+1], point_idx[total], depth_bits[total] (int32 tensors holding the u32 bit patterns)
+    [, transmittance[total] float32 when asked for]."""
     lib = load()
     total = C.c_uint64(0)
-    rc = lib.inpc_raster_get_sorted(_ptr(workspace), W, H, None, None, None, C.byref(total), _stream(stream))
+    rc = lib.inpc_raster_get_sorted(_ptr(workspace), W, H, None, None, None, None, C.byref(total), _stream(stream))
     if rc != 0:
         raise InpcError(rc, "inpc_raster_get_sorted")
     n = int(total.value)
@@ -189,11 +210,12 @@ def inpc_raster_get_sorted(workspace, W: int, H: int, stream=None):
     offsets = torch.empty(W * H + 1, dtype=torch.int32, device=dev)
     idx = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
     depth = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
-    rc = lib.inpc_raster_get_sorted(_ptr(workspace), W, H, _ptr(offsets), _ptr(idx), _ptr(depth), C.byref(total),
-                                    _stream(stream))
+    tr = torch.empty(max(n, 1), dtype=torch.float32, device=dev) if transmittance else None
+    rc = lib.inpc_raster_get_sorted(_ptr(workspace), W, H, _ptr(offsets), _ptr(idx), _ptr(depth), _ptr(tr),
+                                    C.byref(total), _stream(stream))
     if rc != 0:
         raise InpcError(rc, "inpc_raster_get_sorted")
-    return offsets, idx[:n], depth[:n]
+    return (offsets, idx[:n], depth[:n], tr[:n]) if transmittance else (offsets, idx[:n], depth[:n])
 
 
 def inpc_raster_get_stats(workspace, stream=None) -> dict:
@@ -206,6 +228,15 @@ def inpc_raster_get_stats(workspace, stream=None) -> dict:
 
 def inpc_raster_launch_count() -> int:
     return int(load().inpc_raster_launch_count())
+
+
+def inpc_raster_launched_kernels(reset: bool = False) -> set:
+    """Distinct kernel template instantiations launched by this process since the last reset."""
+    lib = load()
+    n = lib.inpc_raster_launched_kernels(None, 0, 0)
+    buf = C.create_string_buffer(int(n) + 1)
+    lib.inpc_raster_launched_kernels(buf, len(buf), 1 if reset else 0)
+    return {k for k in buf.value.decode().split(";") if k}
 
 
 def inpc_raster_set_kernel_timing(enable: bool) -> None:

@@ -75,10 +75,20 @@ def test_argument_validation_returns_codes_not_crashes(lib):
     assert f(fake, fake, fake, 16, 4, C.byref(cam), fake, fake, fake, 1 << 20, 0, None) == -1   # near >= far
     cam.near_z = 0.01
     b = lib.inpc_raster_backward
-    assert b(fake, fake, fake, 16, 4, C.byref(cam), fake, None, fake, fake, fake, fake, 1 << 20, None) == -4  # no forward
-    assert lib.inpc_raster_get_counts(fake, 64, 64, fake, None) == -4
+    assert b(fake, fake, fake, 16, 4, C.byref(cam), fake, None, fake, fake, fake, fake, 64, None) == -2     # workspace too small
+    assert b(fake, fake, fake, 16, 4, C.byref(cam), None, None, fake, fake, fake, fake, 1 << 20, None) == -1  # NULL grad_out
+    assert b(fake, fake, fake, 16, 4, C.byref(cam), fake, None, fake, fake, fake, C.c_void_p(0x1010), 1 << 20, None) == -1  # workspace not 256-aligned
+    assert lib.inpc_raster_get_counts(None, 64, 64, fake, None) == -1
+    assert lib.inpc_raster_get_blended_counts(fake, 0, 64, fake, None) == -1
     st = raster.InpcStats()
-    assert lib.inpc_raster_get_stats(fake, C.byref(st), None) == -4
+    assert lib.inpc_raster_get_stats(None, C.byref(st), None) == -1
+    assert lib.inpc_raster_get_status(None, None) == -1
+    import torch
+    if not torch.cuda.is_available():
+        # no device: every compute / read-back call reports INPC_ERR_CUDA (there is no CPU fallback)
+        assert f(fake, fake, fake, 16, 4, C.byref(cam), fake, fake, fake, 1 << 20, 0, None) == -3
+        assert lib.inpc_raster_get_status(fake, None) == -3
+        assert lib.inpc_raster_last_cuda_error().decode() != ""
 
 
 def test_strerror_and_launch_counter(lib):
@@ -86,7 +96,7 @@ def test_strerror_and_launch_counter(lib):
     assert len(msgs) == 6 and "ok" in msgs
     assert lib.inpc_raster_strerror(-99).decode() == "unknown status"
     assert raster.inpc_raster_launch_count() >= 0
-    assert lib.inpc_raster_last_cuda_error().decode() == ""
+    assert isinstance(raster.inpc_raster_launched_kernels(), set)
 
 
 def test_missing_library_fails_loudly(monkeypatch):

@@ -1,10 +1,13 @@
 """GPU parity tests proper (-m gpu): the CUDA path, called through the C ABI, against the oracle.
 
-Sizes: whole-image element-by-element parity where the oracle finishes in seconds (Tiny, 1M, and
-reduced draws of the octree / cluster samplers that still span many tiles, ragged tile edges and
-the long-run path); at BASELINE.json's full sizes (8M / 16M / 33M) whole-image counts + sampled
-pixel windows the oracle evaluates one by one (tests/test_gpu_fullsize.py).
+Every test goes through harness.full_parity: whole-image, every-point, element-by-element comparison in
+the three launch configurations (introspection dump, bench.py's fwd+bwd step flags, bench.py's forward-only
+flags).  Sizes: Tiny, 1M and reduced draws of the octree / cluster samplers that still span many tiles,
+ragged tile edges and the long-run path, then BASELINE.json's full sizes (8M / 16M / 33M points), which the
+oracle finishes in tens of seconds.  The last test checks that every kernel instantiation bench.py launches
+is one these tests compared with the oracle.
 """
+import ctypes
 import numpy as np
 import pytest
 import torch
@@ -13,8 +16,9 @@ import oracle
 from paper_2403_16862_b200 import raster
 from paper_2403_16862_b200.workloads import Camera, Workload, make_workload, second_pose
 
-from harness import (check_backward, check_counts_and_order, check_forward, full_parity, gpu_backward,
-                     gpu_forward)
+import bench
+import harness
+from harness import full_parity, gpu_backward, gpu_forward
 
 pytestmark = pytest.mark.gpu
 
@@ -81,8 +85,8 @@ def test_stress_sampler_reduced_hits_long_run_path():
 
 
 # ------------------------------------------------------------------------------ full sizes (BASELINE.json configs 3-5)
-# The oracle finishes these in tens of seconds, so the whole image / every gradient is compared, in the same
-# launch configuration bench.py times.
+# The oracle finishes these in tens of seconds, so the whole image / every gradient is compared, in the launch
+# configurations bench.py times (harness runs B and C) as well as in the introspection one (run A).
 
 def test_train_full_size():
     rep = full_parity(make_workload("train"))
@@ -206,23 +210,47 @@ def test_forward_is_repeatable_and_workspace_reusable():
         raster.inpc_raster_forward(st["pos"], st["op"], st["feat"], wl.cam, out_feat=st["img"], out_alpha=st["alpha"],
                                    workspace=st["ws"], flags=raster.SAVE_FOR_BACKWARD | raster.SAVE_SORTED)
     torch.cuda.synchronize()
-    assert torch.equal(img0, st["img"]) or float((img0 - st["img"]).abs().max()) < 1e-6
-    assert float((a0 - st["alpha"]).abs().max()) < 1e-6
+    # no atomics in the value path: results are bit-reproducible run to run
+    assert torch.equal(img0, st["img"]) and torch.equal(a0, st["alpha"])
     g1 = gpu_backward(wl, st)
     g2 = gpu_backward(wl, st)
     for a, b in zip(g1, g2):
-        assert float((a - b).abs().max()) < 1e-5
+        assert torch.equal(a, b)
 
 
 def test_error_codes():
     wl = make_workload("tiny")
     st = gpu_forward(wl, flags=0)
     g = torch.zeros((64, 64, 4), device="cuda")
-    with pytest.raises(raster.InpcError) as e:
+    with pytest.raises(raster.InpcError) as e:     # a forward without INPC_SAVE_FOR_BACKWARD leaves a smaller workspace
         raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g, None, st["ws"])
-    assert e.value.status == -4                    # forward did not save for backward
+    assert e.value.status == -2
     with pytest.raises(raster.InpcError) as e:
         raster.inpc_raster_get_sorted(st["ws"], 64, 64)
+    assert e.value.status == -4
+    with pytest.raises(raster.InpcError) as e:
+        raster.inpc_raster_get_blended_counts(st["ws"], 64, 64)
+    assert e.value.status == -4
+    # a workspace that is large enough but holds no saving forward: the backward's device-side header check
+    # refuses (gradient buffers untouched) and inpc_raster_get_status reports why
+    big = raster.alloc_workspace(wl.N, 4, 64, 64, raster.SAVE_FOR_BACKWARD)
+    raster.inpc_raster_forward(st["pos"], st["op"], st["feat"], wl.cam, workspace=big, flags=0)
+    sentinel = torch.full((wl.N, 4), 7.0, device="cuda")
+    raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g, None, big, grad_feat=sentinel)
+    assert raster.inpc_raster_get_status(big) == -4
+    assert float(sentinel.min()) == 7.0 and float(sentinel.max()) == 7.0
+    # ... a saving forward of ANOTHER shape: INVALID_ARG
+    raster.inpc_raster_forward(st["pos"][:100], st["op"][:100], st["feat"][:100], wl.cam, workspace=big,
+                               flags=raster.SAVE_FOR_BACKWARD)
+    raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g, None, big, grad_feat=sentinel)
+    assert raster.inpc_raster_get_status(big) == -1
+    assert float(sentinel.min()) == 7.0
+    # ... never written by any forward (zeroed, then garbage)
+    big.zero_()
+    raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g, None, big, grad_feat=sentinel)
+    assert raster.inpc_raster_get_status(big) == -4 and float(sentinel.min()) == 7.0
+    with pytest.raises(raster.InpcError) as e:
+        raster.inpc_raster_get_counts(big, 64, 64)
     assert e.value.status == -4
     small = torch.empty(1024, dtype=torch.uint8, device="cuda")
     with pytest.raises(raster.InpcError) as e:
@@ -244,3 +272,72 @@ def test_launch_counter_counts_kernels():
     gpu_backward(wl, st)
     after = raster.inpc_raster_launch_count()
     assert mid - before >= 5 and after - mid >= 1
+
+
+def test_workspace_may_be_copied_between_forward_and_backward():
+    """The state lives in the workspace, not in the library (include/inpc_raster.h): a bitwise copy of the
+    workspace at another address serves the backward pass and the introspection calls."""
+    wl = make_workload("tiny")
+    st = gpu_forward(wl, flags=raster.SAVE_FOR_BACKWARD)
+    g1 = gpu_backward(wl, st)
+    moved = dict(st)
+    moved["ws"] = st["ws"].clone()
+    st["ws"].zero_()
+    g2 = gpu_backward(wl, moved)
+    for a, b in zip(g1, g2):
+        assert torch.equal(a, b)
+    assert raster.inpc_raster_get_stats(moved["ws"])["n_points"] == wl.N
+
+
+def test_raw_ctypes_forward_backward_without_the_binding():
+    """Drive the C ABI directly (no raster.py): the binding adds nothing but marshalling."""
+    wl = make_workload("tiny")
+    lib = ctypes.CDLL(raster.LIB_PATH)
+    vp, i64, i32, u32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_uint32
+    lib.inpc_raster_workspace_bytes.restype = ctypes.c_size_t
+    lib.inpc_raster_workspace_bytes.argtypes = [i64, i32, i32, i32, u32]
+    lib.inpc_raster_forward.argtypes = [vp, vp, vp, i64, i32, vp, vp, vp, vp, ctypes.c_size_t, u32, vp]
+    lib.inpc_raster_backward.argtypes = [vp, vp, vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, ctypes.c_size_t, vp]
+    cam = (ctypes.c_float * 18)(64, 64, 32, 32, 1, 0, 0, 0, 1, 0, 0, 0, 1, 0, 0, 0, 0.01, 100.0)
+    cam_bytes = bytes(cam) + (ctypes.c_int32 * 2)(64, 64)
+    cam_buf = ctypes.create_string_buffer(bytes(cam_bytes), len(cam_bytes))
+    N, D, W, H = wl.N, 4, 64, 64
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    pos, op, feat, g_img, g_alpha = t(wl.pos), t(wl.opacity), t(wl.feat), t(wl.g_img), t(wl.g_alpha)
+    nbytes = lib.inpc_raster_workspace_bytes(N, D, W, H, 1)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    img = torch.empty((H, W, D), device="cuda"); alpha = torch.empty((H, W), device="cuda")
+    d_feat = torch.empty((N, D), device="cuda"); d_op = torch.empty((N,), device="cuda"); d_uv = torch.empty((N, 2), device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    p = lambda x: ctypes.c_void_p(x.data_ptr())
+    assert lib.inpc_raster_forward(p(pos), p(op), p(feat), N, D, ctypes.cast(cam_buf, vp), p(img), p(alpha), p(ws), nbytes,
+                                   1, ctypes.c_void_p(stream)) == 0
+    assert lib.inpc_raster_backward(p(pos), p(op), p(feat), N, D, ctypes.cast(cam_buf, vp), p(g_img), p(g_alpha), p(d_feat),
+                                    p(d_op), p(d_uv), p(ws), nbytes, ctypes.c_void_p(stream)) == 0
+    torch.cuda.synchronize()
+    ref = oracle.Raster.from_points(wl.pos, wl.opacity, wl.feat, wl.cam)
+    img_r, alpha_r, _, margin = ref.blend()
+    assert (margin >= harness.MARGIN).all(), "tiny has no termination-ambiguous pixel at this seed"
+    harness.check_image(dict(img=img, alpha=alpha), img_r, alpha_r, "raw ctypes")
+    rf, ro, ru = ref.backward(wl.g_img, wl.g_alpha)
+    harness.check_grads("grad_feat", d_feat, rf); harness.check_grads("grad_opacity", d_op, ro)
+    harness.check_grads("grad_uv", d_uv, ru)
+
+
+def test_zz_bench_kernels_are_the_parity_tested_ones():
+    """Every kernel template instantiation bench.py launches (its fwd+bwd step and its forward-only figure, for
+    D = 4 and D = 8, tile path and long-run path) must be one that full_parity compared with the oracle."""
+    harness.PARITY_KERNELS.clear()
+    wls = [make_workload("tiny"), make_workload("tiny", D=8), make_workload("stress", n_points=1 << 18),
+           make_workload("infer", n_points=1 << 16)]
+    for wl in wls:
+        full_parity(wl)
+    tested = set(harness.PARITY_KERNELS)
+    raster.inpc_raster_launched_kernels(reset=True)
+    for wl in wls:                                          # bench.py's own step functions, same flags
+        fwd, bwd, _ = bench.make_step_functions(raster, wl, torch.device("cuda"))
+        fwd(bench.FLAGS_STEP); bwd(); fwd(bench.FLAGS_FWD)
+    torch.cuda.synchronize()
+    launched = raster.inpc_raster_launched_kernels()
+    assert {"k_blend<4,0>", "k_blend<8,0>", "k_big<4,0>", "k_big<4,2>", "k_back<4>", "k_back<8>"} <= launched
+    assert launched <= tested, f"bench.py launches kernels no parity test ran: {sorted(launched - tested)}"

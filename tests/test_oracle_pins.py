@@ -214,6 +214,47 @@ def test_stacked_equal_opacity_cutoff_golden():
     assert nb[24, 40] == 40 and abs(alpha[24, 40] - (1 - 0.5 ** 40)) < 1e-15
 
 
+def test_margin_output_golden():
+    """`margin` decides which pixels the GPU harness treats as termination-ambiguous: pinned to hand-derived
+    values (tests/golden/stacked_margin.txt), not to the oracle's own formula."""
+    p = [0.53125, -0.46875, 4.0]
+    for a, n, blended, m_ref in _golden("stacked_margin.txt"):
+        n = int(n)
+        r = _one([p] * n, [a] * n, [[1, 1, 1, 1]] * n)
+        _, _, nb, margin = r.blend()
+        assert nb[24, 40] == int(blended)
+        assert abs(margin[24, 40] - m_ref) <= 1e-7 * m_ref
+        assert np.isinf(margin[0, 0])                            # a pixel without fragments tests nothing
+    _, _, _, margin = r.blend(t_min=0.0)
+    assert np.isinf(margin).all()                                # cut-off disabled
+
+
+def test_forced_blend_count_and_sorted_T():
+    """force_nb (harness aid, R7) replaces the termination test by a fixed count and nothing else:
+    n stacked fragments of a = 0.5 forced to 20 give alpha = 1 - 2^-20; sorted_T lists 2^-k for the blended
+    fragments and -1 behind them."""
+    p = [0.53125, -0.46875, 4.0]
+    r = _one([p] * 40, [0.5] * 40, [[1, 1, 1, 1]] * 40)
+    force = np.full((64, 64), oracle.NO_FORCE, dtype=np.uint32)
+    force[24, 40] = 20
+    img, alpha, nb, margin = r.blend(force_nb=force)
+    assert nb[24, 40] == 20 and alpha[24, 40] == 1 - 0.5 ** 20 and img[24, 40, 2] == 1 - 0.5 ** 20
+    off, _, _, _ = r.sorted_fragments()
+    q = 24 * 64 + 40
+    T = r.sorted_T()[off[q]:off[q + 1]]
+    np.testing.assert_array_equal(T[:20], 0.5 ** np.arange(20))
+    np.testing.assert_array_equal(T[20:], -1.0)
+    # unforced pixels keep the test: the same stack with NO_FORCE everywhere is the golden 14
+    _, alpha, nb, _ = r.blend(force_nb=np.full((64, 64), oracle.NO_FORCE, dtype=np.uint32))
+    assert nb[24, 40] == 14 and alpha[24, 40] == 0.99993896484375
+    np.testing.assert_array_equal(r.sorted_T()[off[q]:off[q + 1]][14:], -1.0)
+    # and the backward pass follows the forced state: d alpha / d a_k = prod_{j != k} (1 - a_j) over the 20
+    r.blend(force_nb=force)
+    _, d_op, _ = r.backward(np.zeros((64, 64, 4)), np.ones((64, 64)))
+    np.testing.assert_allclose(d_op[:20], 0.5 ** 19, rtol=1e-12)
+    np.testing.assert_array_equal(d_op[20:], 0.0)
+
+
 def test_general_stack_formula():
     rng = np.random.default_rng(5)
     n = 12
