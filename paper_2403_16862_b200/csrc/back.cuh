@@ -20,7 +20,8 @@ namespace inpc {
 
 struct BackArgs {
     const Header* hdr;
-    uint32_t* item_cursor;
+    uint32_t* item_cursor;   // this band's work cursor ...
+    const uint32_t* n_items; // ... and item count (device)
     const uint32_t* items;
     const uint32_t* celloff;
     const uint32_t* dk;
@@ -60,7 +61,7 @@ __global__ void __launch_bounds__(kTileThreads) k_back(BackArgs A) {
     const int tid = threadIdx.x;
     const int W = A.W, H = A.H;
     if (!A.hdr->bwd_ok) return;                          // the header check failed: touch nothing
-    const uint32_t n_items = A.hdr->n_items;
+    const uint32_t n_items = *A.n_items;
 
     if (tid == 0) {
         mbar_init(&s_bar, 1); fence_mbar_init();

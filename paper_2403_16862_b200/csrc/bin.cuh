@@ -275,13 +275,22 @@ __device__ __forceinline__ uint32_t tile_padded_records(const uint32_t* __restri
 // One thread per base tile: emit it if its records fit the shared-memory capacity, otherwise halve
 // its larger side and retry.  A sub-tile of kMinTilePix pixels or fewer that still does not fit sends
 // its pixels to the long-run list (they are merged straight from global memory, big.cuh).
+// Bands: tile row r belongs to band min(r / rows_per_band, n_bands - 1); band b's items go to items + band_base[b].
+struct BandPlan {
+    int n_bands, rows_per_band;
+    uint32_t item_base[kMaxBands];       // start of the band's item list inside items[]
+};
+
 __global__ void __launch_bounds__(128) k_build_items(const uint32_t* __restrict__ celloff, int W, int H, int cap,
-                                                      Header* __restrict__ hdr, uint32_t* __restrict__ items,
-                                                      uint32_t* __restrict__ bigpix) {
+                                                      BandPlan plan, Header* __restrict__ hdr,
+                                                      uint32_t* __restrict__ items_all, uint32_t* __restrict__ bigpix) {
     const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntx * nty) return;
     const int X0 = (t % ntx) * kTileW, Y0 = (t / ntx) * kTileH;
+    const int band = min((t / ntx) / plan.rows_per_band, plan.n_bands - 1);
+    uint32_t* items = items_all + plan.item_base[band];
+    uint32_t* n_items = &hdr->band_items[band];
     uint32_t stack[12];                                  // binary DFS: depth <= 7, one sibling pending per level
     int sp = 0;
     stack[sp++] = encode_item(X0, Y0, kTileLW, kTileLH);
@@ -292,7 +301,7 @@ __global__ void __launch_bounds__(128) k_build_items(const uint32_t* __restrict_
         const int tw = 1 << lw, th = 1 << lh;
         const uint32_t n = tile_padded_records(celloff, W, H, X, Y, tw, th);
         if (n <= (uint32_t)cap) {
-            items[atomicAdd(&hdr->n_items, 1u)] = it;    // empty tiles too: their pixels must be zeroed
+            items[atomicAdd(n_items, 1u)] = it;          // empty tiles too: their pixels must be zeroed
             continue;
         }
         if (tw * th <= kMinTilePix) {

@@ -22,7 +22,8 @@ namespace inpc {
 
 struct BlendArgs {
     const Header* hdr;
-    uint32_t* item_cursor;
+    uint32_t* item_cursor;   // this band's work cursor ...
+    const uint32_t* n_items; // ... and item count (device)
     const uint32_t* items;
     const uint32_t* celloff;
     const uint32_t* dk;
@@ -50,8 +51,22 @@ __device__ __forceinline__ uint32_t pack_list(uint32_t start_rec, uint32_t end_r
     return (start_rec * 16u + 4u * corner) | ((end_rec * 16u + 4u * corner) << 16);
 }
 
-template <int D, bool DUMP>
-__global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
+// Two heads with equal depth bits (rare): ascending point index decides, read from global memory.  A macro, not a
+// lambda: with by-reference captures of the list predicates the compiler kept a branch inside the merge loop
+// (k_blend 301 -> 352 us).
+#define INPC_BLEND_RESOLVE_TIE()                                                                                          \
+    do {                                                                                                                  \
+        uint32_t best = 0xFFFFFFFFu;                                                                                      \
+        int jb = 0;                                                                                                       \
+        if (p0) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce0 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 0; } } \
+        if (p1) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce1 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 1; } } \
+        if (p2) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce2 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 2; } } \
+        if (p3) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce3 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 3; } } \
+        p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;                                                           \
+    } while (0)
+
+template <int D, bool SAVE, bool DUMP>
+__global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
     constexpr int FV  = D / 4;                     // float4 of features per record
     constexpr int CAP = TileCfg<D>::kCap;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -69,7 +84,7 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
 
     const int tid = threadIdx.x;
     const int W = A.W, H = A.H;
-    const uint32_t n_items = A.hdr->n_items;
+    const uint32_t n_items = *A.n_items;
 
     if (tid == 0) {
         mbar_init(&s_bar, 1); fence_mbar_init();
@@ -171,101 +186,119 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
         uint32_t h0 = st0 < st1 ? s_dk[st0] : kSentHi, h1 = st1 < en1 ? s_dk[st1] : kSentHi;
         uint32_t h2 = st2 < st3 ? s_dk[st2] : kSentHi, h3 = st3 < en3 ? s_dk[st3] : kSentHi;
         // global float index of (slot, corner) = (cursor >> 2) + 4 * (slot - smem record)
-        float* gTtop = A.gT ? A.gT + 4 * ((ptrdiff_t)(int32_t)(0u - bt)) : nullptr;
-        float* gTbot = A.gT ? A.gT + 4 * ((ptrdiff_t)(int32_t)(0u - bb)) : nullptr;
+        float* gTtop = SAVE ? A.gT + 4 * ((ptrdiff_t)(int32_t)(0u - bt)) : nullptr;
+        float* gTbot = SAVE ? A.gT + 4 * ((ptrdiff_t)(int32_t)(0u - bb)) : nullptr;
+        (void)gTtop; (void)gTbot;
 
         float acc[D];
 #pragma unroll
         for (int d = 0; d < D; ++d) acc[d] = 0.f;
         float accA = 0.f, T = 1.f;
-        // ONE loop body for every instantiation (DUMP only adds stores and the order-only tail below).
-        // Software-pipelined, ONE basic block and ONE backward branch per fragment: iteration k selects
-        // fragment k (predicates from the minimum head key), issues its shared-memory loads (alpha, features,
-        // the list's next head key), blends fragment k-1 while they are in flight, advances the list and
-        // recomputes minimum / list predicates / tie flag; the three exit conditions are tested together:
-        // lists exhausted, two heads with equal depth bits (resolved by point index in the outer loop), and
-        // the cut-off -- fragment k+1 is blended iff T_{k+1} = T_k (1 - a_k) >= 1e-4, known as soon as a_k
-        // has arrived.  Entering the body therefore means "fragment k will be blended": the cursors count
-        // exactly the blended fragments.
-        float pa = 0.f;                               // pending fragment: alpha, features, gT address
-        float4 pf[FV];
-#pragma unroll
-        for (int v = 0; v < FV; ++v) pf[v] = make_float4(0.f, 0.f, 0.f, 0.f);
-        float* pg = nullptr;
-        bool have = false;
+        // ONE loop body for every instantiation (SAVE adds the gT store, DUMP the order stores and the tail below).
+        //
+        // The loop is bound by the LATENCY of one pixel's chain, not by throughput: a tile's shared memory is held
+        // until its deepest pixel is done, and that pixel's warp runs mostly alone (ncu: 41 % of the warp samples
+        // sit at the end-of-tile barrier, the running warps issue once per ~3 cycles).  So the body is arranged for
+        // few instructions and a short dependent chain:
+        //   * two register sets (A, B), the loop unrolled by two: the loads of fragment k (alpha, features) land
+        //     in one set while fragment k-1 is blended out of the other -- no register is read in the half-step
+        //     that loaded it;
+        //   * the cut-off is tested LAZILY: fragment k+1 is selected (list advanced, loads issued) before
+        //     T_{k+1} = T_k (1 - a_k) is known; the test then uses an alpha that arrived a half-step ago, and
+        //     when it fails the selection is rolled back (its list steps back by one), so the cursors still
+        //     count exactly the blended fragments.  The arithmetic of the test is unchanged:
+        //     fragment k+1 is blended iff the fp32 product T_k (1 - a_k) >= 1e-4;
+        //   * shared memory is addressed through 32-bit shared-window addresses (lds_*).
+        // Invariant at the top of a half-step: the pending fragment (set X) is one that WILL be blended.
+        const uint32_t sa = smem_u32(s_ab), sf = smem_u32(s_f), sk = smem_u32(s_dk);
         uint32_t kd = 0;                              // DUMP: position of the next fragment in the pixel's sorted list
         const uint32_t obase = DUMP ? A.pixoff[pix] : 0u;
         uint32_t m = min(min(h0, h1), min(h2, h3));
-        bool p0 = h0 == m, p1 = h1 == m, p2 = h2 == m, p3 = h3 == m;
-        bool tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
-        // equal depth bits: ascending point index decides (read from global memory; rare)
-        auto resolve_tie = [&]() {
-            uint32_t best = 0xFFFFFFFFu;
-            int jb = 0;
-            if (p0) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce0 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 0; } }
-            if (p1) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce1 & 0xffffu) >> 4) - bt]).w); if (i < best) { best = i; jb = 1; } }
-            if (p2) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce2 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 2; } }
-            if (p3) { const uint32_t i = __float_as_uint(__ldg(&A.Ra[((ce3 & 0xffffu) >> 4) - bb]).w); if (i < best) { best = i; jb = 3; } }
-            p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;
-        };
-        while (m != kSentHi && !(T * (1.f - pa) < kTMin)) {
-            if (tie) resolve_tie();
-            do {
-                const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
-                const uint32_t cur = ce & 0xffffu;
-                const uint32_t nx = ce + 16u;
-                const uint32_t nc = nx & 0xffffu;
-                // issue the loads of fragment k
-                const float na = *reinterpret_cast<const float*>(s_ab + cur);
-                float4 nf[FV];
-#pragma unroll
-                for (int v = 0; v < FV; ++v) nf[v] = s_f[(cur >> 4) * FV + v];
-                const uint32_t nh = nc < (nx >> 16) ? s_dk[nc >> 4] : kSentHi;
-                float* ng = ((p0 | p1) ? gTtop : gTbot) + (cur >> 2);
-                if constexpr (DUMP) {
-                    const uint32_t slot = (cur >> 4) - ((p0 | p1) ? bt : bb);
-                    A.sorted_idx[obase + kd] = __float_as_uint(__ldg(&A.Ra[slot]).w);
-                    A.sorted_depth[obase + kd] = m;
-                    if (have) A.sorted_T[obase + kd - 1] = T;      // transmittance in front of fragment k-1
-                    ++kd;
-                }
-                // blend fragment k-1
-                const float c = T * pa;
-                accA += c;
-#pragma unroll
-                for (int v = 0; v < FV; ++v) {
-                    acc[4 * v] += c * pf[v].x; acc[4 * v + 1] += c * pf[v].y; acc[4 * v + 2] += c * pf[v].z; acc[4 * v + 3] += c * pf[v].w;
-                }
-                if (A.gT && have) *pg = T;
-                T *= (1.f - pa);
-                h0 = p0 ? nh : h0; ce0 = p0 ? nx : ce0;
-                h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;
-                h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
-                h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
-                pa = na; pg = ng; have = true;
-#pragma unroll
-                for (int v = 0; v < FV; ++v) pf[v] = nf[v];
-                m = min(min(h0, h1), min(h2, h3));
-                p0 = h0 == m; p1 = h1 == m; p2 = h2 == m; p3 = h3 == m;
-                tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
-            } while ((m != kSentHi) & !tie & !(T * (1.f - pa) < kTMin));
+        bool p0, p1, p2, p3;
+        float aA = 0.f, aB = 0.f;
+        float4 fA[FV], fB[FV];
+        uint32_t curA = 0, curB = 0, kdA = 0, kdB = 0;
+        (void)kdA; (void)kdB;
+
+// which list holds the minimum head; two heads with equal depth bits (rare) are resolved by point index
+#define INPC_PICK()                                                                                                       \
+        {                                                                                                                 \
+            p0 = h0 == m; p1 = h1 == m; p2 = h2 == m; p3 = h3 == m;                                                       \
+            if ((p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3)) INPC_BLEND_RESOLVE_TIE();                           \
         }
-        if (have) {                                   // the last selected fragment
-            const float c = T * pa;
-            accA += c;
-#pragma unroll
-            for (int v = 0; v < FV; ++v) {
-                acc[4 * v] += c * pf[v].x; acc[4 * v + 1] += c * pf[v].y; acc[4 * v + 2] += c * pf[v].z; acc[4 * v + 3] += c * pf[v].w;
+// issue the loads of the picked fragment into set X, advance its list, recompute the minimum head
+#define INPC_SELECT(X)                                                                                                    \
+        {                                                                                                                 \
+            const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));                                                 \
+            cur##X = ce & 0xffffu;                                                                                        \
+            const uint32_t nx = ce + 16u;                                                                                 \
+            a##X = lds_f32(sa + cur##X);                                                                                  \
+            _Pragma("unroll") for (int v = 0; v < FV; ++v) f##X[v] = lds_v4(sf + (cur##X & 0xfff0u) * FV + 16 * v);       \
+            uint32_t nh = kSentHi;                                                                                        \
+            if ((nx & 0xffffu) < (nx >> 16)) nh = lds_u32(sk + ((nx >> 2) & 0x3ffcu));                                    \
+            if constexpr (DUMP) {                                                                                         \
+                const uint32_t slot = (cur##X >> 4) - ((p0 | p1) ? bt : bb);                                              \
+                A.sorted_idx[obase + kd] = __float_as_uint(__ldg(&A.Ra[slot]).w);                                         \
+                A.sorted_depth[obase + kd] = m;                                                                           \
+                kd##X = kd++;                                                                                             \
+            }                                                                                                             \
+            h0 = p0 ? nh : h0; ce0 = p0 ? nx : ce0;                                                                       \
+            h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;                                                                       \
+            h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;                                                                       \
+            h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;                                                                       \
+            m = min(min(h0, h1), min(h2, h3));                                                                            \
+        }
+// composite the pending fragment of set X (Eq. 1); lists 0, 1 (corners 3, 2: bit 3 of the cursor) lie in the top cell row
+#define INPC_BLEND(X)                                                                                                     \
+        {                                                                                                                 \
+            const float c = T * a##X;                                                                                     \
+            accA += c;                                                                                                    \
+            _Pragma("unroll") for (int v = 0; v < FV; ++v) {                                                              \
+                acc[4 * v] += c * f##X[v].x; acc[4 * v + 1] += c * f##X[v].y;                                             \
+                acc[4 * v + 2] += c * f##X[v].z; acc[4 * v + 3] += c * f##X[v].w;                                         \
+            }                                                                                                             \
+            if constexpr (SAVE) ((cur##X & 8u) ? gTtop : gTbot)[cur##X >> 2] = T;                                         \
+            if constexpr (DUMP) A.sorted_T[obase + kd##X] = T;                                                            \
+            T *= (1.f - a##X);                                                                                            \
+        }
+// the fragment selected into set X turned out to lie behind the cut-off: step its list (3 - corner) back by one
+#define INPC_ROLLBACK(X)                                                                                                  \
+        {                                                                                                                 \
+            const uint32_t cj = (cur##X >> 2) & 3u;                                                                       \
+            ce0 -= cj == 3u ? 16u : 0u; ce1 -= cj == 2u ? 16u : 0u; ce2 -= cj == 1u ? 16u : 0u; ce3 -= cj == 0u ? 16u : 0u; \
+            if constexpr (DUMP) {                                                                                         \
+                const uint32_t hk = s_dk[cur##X >> 4];                                                                    \
+                h0 = cj == 3u ? hk : h0; h1 = cj == 2u ? hk : h1; h2 = cj == 1u ? hk : h2; h3 = cj == 0u ? hk : h3;       \
+                m = min(min(h0, h1), min(h2, h3));                                                                        \
+                --kd;                                                                                                     \
+            }                                                                                                             \
+        }
+
+        if (m != kSentHi) {
+            INPC_PICK();
+            INPC_SELECT(A);                           // fragment 0: T_0 = 1, always blended
+            while (true) {
+                if (m == kSentHi) { INPC_BLEND(A); break; }          // pending: A
+                INPC_PICK();
+                INPC_SELECT(B);
+                INPC_BLEND(A);
+                if (T < kTMin) { INPC_ROLLBACK(B); break; }
+                if (m == kSentHi) { INPC_BLEND(B); break; }          // pending: B
+                INPC_PICK();
+                INPC_SELECT(A);
+                INPC_BLEND(B);
+                if (T < kTMin) { INPC_ROLLBACK(A); break; }
             }
-            if (A.gT) *pg = T;
-            if constexpr (DUMP) A.sorted_T[obase + kd - 1] = T;
         }
+#undef INPC_SELECT
+#undef INPC_BLEND
+#undef INPC_ROLLBACK
         const uint4 consumed = make_uint4(((ce0 & 0xffffu) >> 4) - st0, ((ce1 & 0xffffu) >> 4) - st1,
                                           ((ce2 & 0xffffu) >> 4) - st2, ((ce3 & 0xffffu) >> 4) - st3);
         if constexpr (DUMP) {
             // order-only tail: the fragments behind the cut-off are merged on, recorded and not blended
             while (m != kSentHi) {
-                if (tie) resolve_tie();
+                INPC_PICK();
                 const uint32_t ce = p0 ? ce0 : (p1 ? ce1 : (p2 ? ce2 : ce3));
                 const uint32_t cur = ce & 0xffffu;
                 const uint32_t nx = ce + 16u;
@@ -281,16 +314,17 @@ __global__ void __launch_bounds__(kTileThreads) k_blend(BlendArgs A) {
                 h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
                 h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
                 m = min(min(h0, h1), min(h2, h3));
-                p0 = h0 == m; p1 = h1 == m; p2 = h2 == m; p3 = h3 == m;
-                tie = (p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3);
             }
         }
+#undef INPC_PICK
 #pragma unroll
         for (int v = 0; v < FV; ++v)
             reinterpret_cast<float4*>(A.out_feat + pix * D)[v] = make_float4(acc[4 * v], acc[4 * v + 1], acc[4 * v + 2], acc[4 * v + 3]);
         A.out_alpha[pix] = accA;
-        if (A.gT) A.pcur[pix] = consumed;
+        if constexpr (SAVE) A.pcur[pix] = consumed;
     }
 }
+
+#undef INPC_BLEND_RESOLVE_TIE
 
 }  // namespace inpc

@@ -41,13 +41,13 @@ __device__ __forceinline__ void emit_sorted(const float4 a0, const float4 a1, ui
 template <int D>
 __global__ void __launch_bounds__(kCsThreads) k_cellsort(const float4* __restrict__ A,
                                                           const uint32_t* __restrict__ celloff, uint32_t C,
+                                                          uint32_t unit_begin, uint32_t unit_end,
                                                           const float* __restrict__ feat,
                                                           uint32_t* __restrict__ dk, float4* __restrict__ Ra, float4* __restrict__ Rf) {
     __shared__ uint32_t s_off[kCsCells + 1];
     __shared__ unsigned long long s_key[kCsWindow];
     const int tid = threadIdx.x;
-    const uint32_t n_units = (C + kCsCells - 1) / kCsCells;
-    for (uint32_t unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+    for (uint32_t unit = unit_begin + blockIdx.x; unit < unit_end; unit += gridDim.x) {   // this launch's band of units
         const uint32_t c0 = unit * kCsCells, nc = min((uint32_t)kCsCells, C - c0);
         __syncthreads();
         for (uint32_t c = tid; c <= nc; c += kCsThreads) s_off[c] = __ldg(&celloff[c0 + c]);

@@ -36,6 +36,7 @@ constexpr int kMinTilePix  = 8;     // a sub-tile this small that still does not
 constexpr int kCellSmall   = 256;   // cells up to this many points are ranked by counting; larger: bitonic
 constexpr int kBigThreads  = 512;
 constexpr int kBigChunk    = 8192;  // keys sorted in shared memory at a time by the large-cell sort
+constexpr int kMaxBands    = 8;     // bands of tile rows the forward / backward pipelines overlap (see inpc_raster.cu)
 constexpr float kTMin      = 1e-4f; // transmittance cut-off (BASELINE.json north_star)
 constexpr uint32_t kSentHi = 0xFFFFFFFFu;   // "list exhausted" for the ascending merge (depth bits < 0x7F800000)
 
@@ -57,8 +58,8 @@ struct Header {
     int32_t  W, H, D;
     uint32_t n_points;
     uint32_t nrec;                 // kept points (= celloff[C]), written by the scan
-    uint32_t n_items;              // tile work items
-    uint32_t item_cursor;          // persistent-kernel work cursors
+    uint32_t n_items;              // (unused; the tile work items are counted per band, below)
+    uint32_t item_cursor;
     uint32_t big_cursor;
     uint32_t scan_tile_counter;
     uint32_t pad0;
@@ -72,6 +73,10 @@ struct Header {
     uint32_t bwd_ok;               // written by the backward pass's header check: 1 = the workspace matches its arguments
     int32_t  status;               // sticky inpc_status of device-side checks (read by inpc_raster_get_status)
     uint32_t pad[9];
+    // Tile work items, one list per BAND of tile rows (kMaxBands bands): a band's tiles can be blended as soon as
+    // its cell rows are sorted, while the next band's cells are still being sorted on another stream.
+    uint32_t band_items[8];        // items of band b
+    uint32_t band_cursor[8];       // persistent-kernel work cursor of band b (forward, then backward)
 };
 static_assert(sizeof(Header) % 16 == 0, "header alignment");
 
@@ -106,6 +111,17 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "DONE_%=:\n\t}" ::"r"(smem_u32(bar)),
         "r"(parity)
         : "memory");
+}
+// Shared-memory loads through 32-bit shared-window addresses: the merge loops address their records with plain
+// integer arithmetic (a generic pointer costs a window-base rematerialisation per access inside the loop).
+__device__ __forceinline__ float lds_f32(uint32_t a) {
+    float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v;
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
+    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v;
+}
+__device__ __forceinline__ float4 lds_v4(uint32_t a) {
+    float4 v; asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a)); return v;
 }
 // One 256-bit store: a whole 32-byte sector in ONE instruction.  A lane-divergent store costs L1 wavefronts
 // per instruction, so two 128-bit stores to the same sector cost twice (k_scatter 222 -> 173 us).

@@ -24,7 +24,8 @@ template <int D> __host__ __device__ constexpr int gpt_floats() { return D == 4 
 
 template <int D>
 __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restrict__ hdr,
-                                                           const uint32_t* __restrict__ celloff, uint32_t C, int W,
+                                                           const uint32_t* __restrict__ celloff, uint32_t C,
+                                                           uint32_t unit_begin, uint32_t unit_end, int W,
                                                            int H, const float4* __restrict__ Ra,
                                                            const float4* __restrict__ gT, const float4* __restrict__ gD,
                                                            const uint4* __restrict__ pcur,
@@ -33,8 +34,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
     __shared__ uint32_t s_off[kGradCells + 1];
     const int tid = threadIdx.x;
     if (!hdr->bwd_ok) return;
-    const uint32_t n_units = (C + kGradCells - 1) / kGradCells;
-    for (uint32_t unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+    for (uint32_t unit = unit_begin + blockIdx.x; unit < unit_end; unit += gridDim.x) {   // this launch's band of units
         const uint32_t c0 = unit * kGradCells, nc = min((uint32_t)kGradCells, C - c0);
         __syncthreads();
         for (uint32_t c = tid; c <= nc; c += kGradThreads) s_off[c] = __ldg(&celloff[c0 + c]);

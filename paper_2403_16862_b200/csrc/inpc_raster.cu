@@ -115,7 +115,7 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     L.Ra = o;      o = align_up(o + (n + 8) * 16);
     L.Rf = o;      o = align_up(o + (n + 8) * (size_t)(4 * D));
     const size_t nbase = (size_t)((W + kTileW - 1) / kTileW) * ((H + kTileH - 1) / kTileH);
-    L.items = o;   o = align_up(o + ((size_t)L.P + nbase + 16) * 4);
+    L.items = o;   o = align_up(o + ((size_t)L.P + nbase + 16 * (kMaxBands + 1)) * 4);
     L.bigpix = o;  o = align_up(o + ((size_t)L.P + 16) * 4);
     L.bigcells = o; o = align_up(o + ((size_t)L.max_big_cells + 1) * sizeof(BigCell));
     L.bigkeys = o; o = align_up(o + (n + 8) * 8);
@@ -208,16 +208,16 @@ static int launch_back(const BackArgs& A, const DeviceInfo& di, cudaStream_t st)
     return INPC_OK;
 }
 
-template <int D, bool DUMP>
+template <int D, bool SAVE, bool DUMP>
 static int launch_blend(const BlendArgs& A, const DeviceInfo& di, cudaStream_t st) {
     constexpr size_t smem = blend_smem_bytes<D>();
     static int grid_by_dev[kMaxDevices] = {};
     int grid = 0;
-    int rc = persistent_grid(k_blend<D, DUMP>, kTileThreads, smem, di, grid_by_dev, &grid);
+    int rc = persistent_grid(k_blend<D, SAVE, DUMP>, kTileThreads, smem, di, grid_by_dev, &grid);
     if (rc != INPC_OK) return rc;
     { StageTimer tm(kStTileFwd, st);
-      k_blend<D, DUMP><<<grid, kTileThreads, smem, st>>>(A); }
-    INPC_LAUNCHED(kname<D, DUMP ? 1 : 0>("k_blend"));
+      k_blend<D, SAVE, DUMP><<<grid, kTileThreads, smem, st>>>(A); }
+    INPC_LAUNCHED(kname<D, SAVE ? 1 : 0, DUMP ? 1 : 0>("k_blend"));
     return INPC_OK;
 }
 
@@ -272,7 +272,59 @@ __global__ void k_check_backward(Header* h, int W, int H, int D, uint32_t N) {
     else if (h->W != W || h->H != H || h->D != D || h->n_points != N) st = INPC_ERR_INVALID_ARG;
     h->bwd_ok = st == INPC_OK ? 1u : 0u;
     if (st != INPC_OK) h->status = st;
-    h->item_cursor = 0;
+    for (int b = 0; b < kMaxBands; ++b) h->band_cursor[b] = 0;
+}
+
+// ---- band plan + the library's own side stream --------------------------------------------------------------------
+// The sort / gather kernels are bound by DRAM access rates and leave the SMs idle; the merge kernels are bound by
+// shared-memory residency and latency and leave DRAM idle.  So the image is cut into bands of tile rows and the two
+// kinds of work run on two streams: while band b is blended (backward: combined) on the side stream, band b + 1 is
+// sorted (backward: walked) on the caller's stream.  Fork / join is by events, so from the caller's point of view
+// everything is still ordered on ITS stream.  With kernel timing enabled (inpc_raster_set_kernel_timing) the side
+// stream is not used: the per-stage times are then those of kernels running alone.
+struct Bands {
+    BandPlan plan;                         // n_bands, rows_per_band, item_base
+    uint32_t sort_end[kMaxBands];          // forward: band b may be blended once the cell units < sort_end[b] are sorted
+    uint32_t comb_end[kMaxBands];          // backward: once band b is walked the cell units < comb_end[b] can be combined
+};
+
+static Bands make_bands(int W, int H, uint32_t C, int want) {
+    Bands B{};
+    const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
+    const uint32_t n_units = (C + kCsCells - 1) / kCsCells;
+    int nb = std::max(1, std::min(std::min(want, kMaxBands), nty / 8));      // at least 8 tile rows per band
+    const int rpb = (nty + nb - 1) / nb;
+    nb = (nty + rpb - 1) / rpb;
+    B.plan.n_bands = nb; B.plan.rows_per_band = rpb;
+    uint32_t base = 0;
+    for (int b = 0; b < nb; ++b) {
+        const int r0 = b * rpb, r1 = std::min(nty, (b + 1) * rpb);
+        const int y1 = std::min(H, r1 * kTileH);                             // first pixel row behind the band
+        B.plan.item_base[b] = base;
+        base += (uint32_t)((size_t)(y1 - r0 * kTileH) * W + (size_t)(r1 - r0) * ntx + 16);   // worst case: one item per pixel
+        // forward: the band's pixels read cell rows <= y1
+        const uint64_t c_hi = (uint64_t)(y1 + 1) * (W + 1);
+        B.sort_end[b] = b == nb - 1 ? n_units : (uint32_t)std::min<uint64_t>(n_units, (c_hi + kCsCells - 1) / kCsCells);
+        // backward: cell row j is complete once pixel rows j - 1 and j are walked, i.e. rows j <= y1 - 1
+        B.comb_end[b] = b == nb - 1 ? n_units : (uint32_t)std::min<uint64_t>(n_units, ((uint64_t)y1 * (W + 1)) / kCsCells);
+    }
+    return B;
+}
+
+constexpr int kDefaultBands = 1;      // measured: 4 bands cost more per kernel (tails, <1 wave per launch) than the overlap wins (1.51 -> 1.61 ms)
+constexpr int kSideEvents = 2 * kMaxBands + 4;
+struct Side { cudaStream_t stream = nullptr; cudaEvent_t ev[kSideEvents] = {}; bool ok = false; };
+static std::mutex g_side_mu;              // serialises the enqueue of calls that use the side stream
+static Side* side_for(const DeviceInfo& di) {
+    static Side sides[kMaxDevices];
+    Side& s = sides[di.dev];
+    if (!s.ok) {
+        if (cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
+        for (int i = 0; i < kSideEvents; ++i)
+            if (cudaEventCreateWithFlags(&s.ev[i], cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        s.ok = true;
+    }
+    return &s;
 }
 
 template <int D>
@@ -298,6 +350,21 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     const bool save = (flags & INPC_SAVE_FOR_BACKWARD) != 0;
     uint32_t* pixoff = dump ? reinterpret_cast<uint32_t*>(ws + L.pixoff) : nullptr;
 
+    // two streams unless per-stage timing wants every kernel alone
+    std::unique_lock<std::mutex> side_lock(g_side_mu, std::defer_lock);
+    Side* side = nullptr;
+    if (!g_timing && N > 0) { side_lock.lock(); side = side_for(di); if (!side) return cuda_fail(cudaGetLastError()); }
+    cudaStream_t s2 = side ? side->stream : st;
+    const Bands B = make_bands(W, H, L.C, kDefaultBands);      // a function of the image shape only: backward rebuilds it
+    const int nb = B.plan.n_bands;
+    int ev = 0;
+    auto fork = [&](cudaStream_t from, cudaStream_t to) -> cudaError_t {      // `to` waits for what `from` has enqueued
+        if (from == to) return cudaSuccess;
+        cudaEvent_t e = side->ev[ev++ % kSideEvents];
+        cudaError_t rc = cudaEventRecord(e, from);
+        return rc != cudaSuccess ? rc : cudaStreamWaitEvent(to, e, 0);
+    };
+
     { StageTimer tm(kStZeroFwd, st);
       INPC_CUDA(cudaMemsetAsync(ws + L.header, 0, L.zero_end - L.header, st));
       k_write_header<<<1, 1, 0, st>>>(hdr, flags, W, H, D, (uint32_t)N); }
@@ -315,55 +382,70 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
       k_scan_u32<<<(L.C + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
           cellcnt, L.C, reinterpret_cast<unsigned long long*>(ws + L.status0), &hdr->scan_tile_counter, &hdr->nrec, cursor); }
     INPC_LAUNCHED("k_scan_u32");
+
+    // side stream: everything that needs only the cell offsets (per-pixel counts, large-cell list, tile work lists)
+    INPC_CUDA(fork(st, s2));
+    { StageTimer tm(kStClassify, s2);
+      k_classify<<<(L.C + 255) / 256, 256, 0, s2>>>(cellcnt, W, H, hdr, bigcells, pixoff); }
+    INPC_LAUNCHED("k_classify");
+    if (dump) {
+        { StageTimer tm(kStOther, s2);
+          k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, s2>>>(
+              pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr, nullptr); }
+        INPC_LAUNCHED("k_scan_u32");
+    }
+    const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
+    { StageTimer tm(kStBuildItems, s2);
+      k_build_items<<<(ntx * nty + 127) / 128, 128, 0, s2>>>(cellcnt, W, H, TileCfg<D>::kCap, B.plan, hdr, items, bigpix); }
+    INPC_LAUNCHED("k_build_items");
+
+    // caller's stream: scatter, then the cell sort band by band
     if (N > 0) {
         { StageTimer tm(kStScatter, st);
           k_scatter<<<scatter_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cursor, Arec); }
         INPC_LAUNCHED("k_scatter");
-    }
-    { StageTimer tm(kStClassify, st);
-      k_classify<<<(L.C + 255) / 256, 256, 0, st>>>(cellcnt, W, H, hdr, bigcells, pixoff); }
-    INPC_LAUNCHED("k_classify");
-    if (N > 0) {
-        const uint32_t n_units = (L.C + kCsCells - 1) / kCsCells;
-        { StageTimer tm(kStCellSort, st);
-          k_cellsort<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 4), kCsThreads, 0, st>>>(
-              Arec, cellcnt, L.C, feat, dk, Ra, Rf); }
-        INPC_LAUNCHED(kname<D>("k_cellsort"));
+        INPC_CUDA(fork(s2, st));                                              // the large-cell list
         int rc = launch_cellsort_big<D>(hdr, bigcells, Arec,
                                         reinterpret_cast<unsigned long long*>(ws + L.bigkeys), feat, dk, Ra, Rf, di,
                                         L.max_big_cells, st);
         if (rc != INPC_OK) return rc;
     }
-    if (dump) {
-        { StageTimer tm(kStOther, st);
-          k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, st>>>(
-              pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr, nullptr); }
-        INPC_LAUNCHED("k_scan_u32");
-    }
-    const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
-    { StageTimer tm(kStBuildItems, st);
-      k_build_items<<<(ntx * nty + 127) / 128, 128, 0, st>>>(cellcnt, W, H, TileCfg<D>::kCap, hdr, items, bigpix); }
-    INPC_LAUNCHED("k_build_items");
 
     BlendArgs A{};
-    A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = items; A.celloff = cellcnt; A.dk = dk; A.Ra = Ra; A.Rf = Rf;
+    A.hdr = hdr; A.celloff = cellcnt; A.dk = dk; A.Ra = Ra; A.Rf = Rf;
     A.W = W; A.H = H; A.out_feat = out_feat; A.out_alpha = out_alpha;
-    BigArgs B{};
-    B.hdr = hdr; B.bigpix = bigpix; B.celloff = cellcnt; B.dk = dk; B.Ra = Ra; B.Rf = Rf;
-    B.W = W; B.H = H; B.out_feat = out_feat; B.out_alpha = out_alpha;
+    BigArgs Bg{};
+    Bg.hdr = hdr; Bg.bigpix = bigpix; Bg.celloff = cellcnt; Bg.dk = dk; Bg.Ra = Ra; Bg.Rf = Rf;
+    Bg.W = W; Bg.H = H; Bg.out_feat = out_feat; Bg.out_alpha = out_alpha;
     if (save) {
-        A.gT = B.gT = reinterpret_cast<float*>(ws + L.gT);
-        A.pcur = B.pcur = reinterpret_cast<uint4*>(ws + L.pcur);
+        A.gT = Bg.gT = reinterpret_cast<float*>(ws + L.gT);
+        A.pcur = Bg.pcur = reinterpret_cast<uint4*>(ws + L.pcur);
     }
     if (dump) {
-        B.pixoff = A.pixoff = pixoff;
-        B.sorted_idx = A.sorted_idx = reinterpret_cast<uint32_t*>(ws + L.sorted_idx);
-        B.sorted_depth = A.sorted_depth = reinterpret_cast<uint32_t*>(ws + L.sorted_depth);
-        B.sorted_T = A.sorted_T = reinterpret_cast<float*>(ws + L.sorted_T);
+        Bg.pixoff = A.pixoff = pixoff;
+        Bg.sorted_idx = A.sorted_idx = reinterpret_cast<uint32_t*>(ws + L.sorted_idx);
+        Bg.sorted_depth = A.sorted_depth = reinterpret_cast<uint32_t*>(ws + L.sorted_depth);
+        Bg.sorted_T = A.sorted_T = reinterpret_cast<float*>(ws + L.sorted_T);
     }
-    int rc = dump ? launch_blend<D, true>(A, di, st) : launch_blend<D, false>(A, di, st);
-    if (rc != INPC_OK) return rc;
-    if (N > 0) rc = dump ? launch_big<D, kFwdDump>(B, di.sms, st) : launch_big<D, kFwd>(B, di.sms, st);
+    uint32_t u0 = 0;
+    for (int b = 0; b < nb; ++b) {
+        const uint32_t u1 = B.sort_end[b];
+        if (N > 0 && u1 > u0) {
+            { StageTimer tm(kStCellSort, st);
+              k_cellsort<D><<<(int)std::min<uint32_t>(u1 - u0, (uint32_t)di.sms * 4), kCsThreads, 0, st>>>(
+                  Arec, cellcnt, L.C, u0, u1, feat, dk, Ra, Rf); }
+            INPC_LAUNCHED(kname<D>("k_cellsort"));
+            u0 = u1;
+        }
+        INPC_CUDA(fork(st, s2));                                              // band b is sorted: blend it
+        A.items = items + B.plan.item_base[b]; A.n_items = &hdr->band_items[b]; A.item_cursor = &hdr->band_cursor[b];
+        int rc = dump ? (save ? launch_blend<D, true, true>(A, di, s2) : launch_blend<D, false, true>(A, di, s2))
+                      : (save ? launch_blend<D, true, false>(A, di, s2) : launch_blend<D, false, false>(A, di, s2));
+        if (rc != INPC_OK) return rc;
+    }
+    INPC_CUDA(fork(s2, st));                                                  // join
+    int rc = INPC_OK;
+    if (N > 0) rc = dump ? launch_big<D, kFwdDump>(Bg, di.sms, st) : launch_big<D, kFwd>(Bg, di.sms, st);
     return rc;
 }
 
@@ -378,6 +460,10 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
       k_check_backward<<<1, 1, 0, st>>>(hdr, W, H, D, (uint32_t)N); }
     INPC_LAUNCHED("k_check_backward");
     if (N == 0) return INPC_OK;
+    std::unique_lock<std::mutex> side_lock(g_side_mu, std::defer_lock);
+    Side* side = nullptr;
+    if (!g_timing) { side_lock.lock(); side = side_for(di); if (!side) return cuda_fail(cudaGetLastError()); }
+    cudaStream_t s2 = side ? side->stream : st;
     const uint32_t* celloff = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
     const float4* Ra = reinterpret_cast<float4*>(ws + L.Ra);
     const float4* Rf = reinterpret_cast<float4*>(ws + L.Rf);
@@ -385,22 +471,42 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     float* gD = reinterpret_cast<float*>(ws + L.gD);
     uint4* pcur = reinterpret_cast<uint4*>(ws + L.pcur);
     float* gpt = reinterpret_cast<float*>(ws + L.gpt);
+    uint32_t* items = reinterpret_cast<uint32_t*>(ws + L.items);
+    int ev = 0;
+    auto fork = [&](cudaStream_t from, cudaStream_t to) -> cudaError_t {
+        if (from == to) return cudaSuccess;
+        cudaEvent_t e = side->ev[ev++ % kSideEvents];
+        cudaError_t rc = cudaEventRecord(e, from);
+        return rc != cudaSuccess ? rc : cudaStreamWaitEvent(to, e, 0);
+    };
+    // long-run pixels first: they need nothing but the forward state, and every combine below may touch their cells
+    BigArgs Bg{};
+    Bg.hdr = hdr; Bg.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); Bg.celloff = celloff;
+    Bg.dk = reinterpret_cast<uint32_t*>(ws + L.dk); Bg.Ra = Ra; Bg.Rf = Rf;
+    Bg.W = W; Bg.H = H; Bg.gT = gT; Bg.pcur = pcur; Bg.g_feat = g_feat; Bg.g_alpha = g_alpha; Bg.gD = gD;
+    int rc = launch_big<D, kBwd>(Bg, di.sms, st);
+    if (rc != INPC_OK) return rc;
     BackArgs A{};
-    A.hdr = hdr; A.item_cursor = &hdr->item_cursor; A.items = reinterpret_cast<uint32_t*>(ws + L.items);
-    A.celloff = celloff; A.dk = reinterpret_cast<uint32_t*>(ws + L.dk); A.Ra = Ra; A.Rf = Rf;
+    A.hdr = hdr; A.celloff = celloff; A.dk = Bg.dk; A.Ra = Ra; A.Rf = Rf;
     A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD;
-    int rc = launch_back<D>(A, di, st);
-    if (rc != INPC_OK) return rc;
-    BigArgs B{};
-    B.hdr = hdr; B.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); B.celloff = celloff; B.dk = A.dk; B.Ra = Ra; B.Rf = Rf;
-    B.W = W; B.H = H; B.gT = gT; B.pcur = pcur; B.g_feat = g_feat; B.g_alpha = g_alpha; B.gD = gD;
-    rc = launch_big<D, kBwd>(B, di.sms, st);
-    if (rc != INPC_OK) return rc;
-    const uint32_t n_units = (L.C + kGradCells - 1) / kGradCells;
-    { StageTimer tm(kStCombine, st);
-      k_combine<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 8), kGradThreads, 0, st>>>(
-          hdr, celloff, L.C, W, H, Ra, reinterpret_cast<const float4*>(gT), reinterpret_cast<const float4*>(gD), pcur, g_feat, gpt); }
-    INPC_LAUNCHED(kname<D>("k_combine"));
+    const Bands Bf = make_bands(W, H, L.C, kDefaultBands);     // the plan the forward built the item lists with
+    uint32_t u0 = 0;
+    for (int b = 0; b < Bf.plan.n_bands; ++b) {
+        A.items = items + Bf.plan.item_base[b]; A.n_items = &hdr->band_items[b]; A.item_cursor = &hdr->band_cursor[b];
+        rc = launch_back<D>(A, di, st);
+        if (rc != INPC_OK) return rc;
+        const uint32_t u1 = Bf.comb_end[b];
+        if (u1 > u0) {
+            INPC_CUDA(fork(st, s2));                                          // band b is walked: combine its cells
+            { StageTimer tm(kStCombine, s2);
+              k_combine<D><<<(int)std::min<uint32_t>(u1 - u0, (uint32_t)di.sms * 8), kGradThreads, 0, s2>>>(
+                  hdr, celloff, L.C, u0, u1, W, H, Ra, reinterpret_cast<const float4*>(gT),
+                  reinterpret_cast<const float4*>(gD), pcur, g_feat, gpt); }
+            INPC_LAUNCHED(kname<D>("k_combine"));
+            u0 = u1;
+        }
+    }
+    INPC_CUDA(fork(s2, st));                                                  // join
     { StageTimer tm(kStSplit, st);
       k_split<D><<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16), 256, 0, st>>>(
           hdr, gpt, reinterpret_cast<const uint32_t*>(ws + L.kept), (long long)N, d_feat, d_opacity, d_uv); }
@@ -511,7 +617,8 @@ int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_s
     stats->n_points = h.n_points;
     stats->n_kept = h.nrec;
     stats->n_fragments = h.n_fragments;
-    stats->n_tile_items = h.n_items;
+    stats->n_tile_items = 0;
+    for (int b = 0; b < kMaxBands; ++b) stats->n_tile_items += h.band_items[b];
     stats->n_big_pixels = h.n_big_pixels;
     stats->n_big_fragments = h.n_big_fragments;
     stats->n_big_cells = h.n_big_cells;

@@ -339,5 +339,5 @@ def test_zz_bench_kernels_are_the_parity_tested_ones():
         fwd(bench.FLAGS_STEP); bwd(); fwd(bench.FLAGS_FWD)
     torch.cuda.synchronize()
     launched = raster.inpc_raster_launched_kernels()
-    assert {"k_blend<4,0>", "k_blend<8,0>", "k_big<4,0>", "k_big<4,2>", "k_back<4>", "k_back<8>"} <= launched
+    assert {"k_blend<4,1,0>", "k_blend<4,0,0>", "k_blend<8,1,0>", "k_blend<8,0,0>", "k_big<4,0>", "k_big<4,2>", "k_back<4>", "k_back<8>"} <= launched
     assert launched <= tested, f"bench.py launches kernels no parity test ran: {sorted(launched - tested)}"
