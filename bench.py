@@ -45,15 +45,6 @@ METRIC = "fragments/sec (fwd+bwd step; ms/frame fwd and fwd+bwd beside it)"
 UNIT = "fragments/s"
 L2_BYTES = 126 * 1024 * 1024
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/; the file named in NCU_TRAFFIC_SOURCE).  None until a capture exists for that kernel.
-NCU_TRAFFIC = {   # bytes per launch, train workload
-    "k_project_count": 108.4e6, "k_scatter": 390.4e6, "k_cellsort": 1203.3e6, "k_blend": 632.3e6,
-    "k_back": 804.6e6, "k_combine": 750.6e6, "k_split": 457.4e6,
-}
-NCU_TRAFFIC_SOURCE = "profiles/r01_v3b_sector_stores.md (ncu --set full, train workload; k_cellsort from r01_v2_cellsort_merge.md)"
-
-
 # ------------------------------------------------------------------------------------------------
 # algorithmic bytes: per fragment / pixel / point figures
 def algorithmic_bytes(n_points: int, n_frag: int, n_pix: int, D: int) -> dict:
@@ -201,12 +192,22 @@ def oracle_sample_size(wl, seconds_per_step: float) -> int:
     return min(p, wl.N)
 
 
-def cpu_baseline(wl, budget_s: float = 15.0) -> dict:
-    n = oracle_sample_size(wl, budget_s)
-    dt, frags = oracle_step(wl, n)
-    return {"value": frags / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+def cpu_baseline(wl, budget_s: float = 12.0, openmp: bool = False) -> dict:
+    """The oracle as it stands on the host cores: single-threaded (the build every test uses), or -- openmp=True --
+    the SAME source built with -fopenmp on all cores (SURVEY.md 8d "Oracle timed beside it" (2))."""
+    import oracle
+    threads = oracle.use_openmp(True) if openmp else 1
+    try:
+        n = oracle_sample_size(wl, budget_s)
+        dt, frags = oracle_step(wl, n)
+    finally:
+        if openmp:
+            oracle.use_openmp(False)
+    return {"value": frags / dt, "unit": UNIT, "cores": threads, "nproc": os.cpu_count(),
+            "kind": "oracle (-fopenmp build, all cores)" if openmp else "oracle",
             "sample": f"first {n} of {wl.N} points of '{wl.name}' (same camera, full image), one fwd+bwd, "
-                      f"{frags} fragments in {dt:.2f} s; oracle/oracle.cpp is single-threaded fp64",
+                      f"{frags} fragments in {dt:.2f} s; oracle/oracle.cpp fp64, {threads} thread(s)"
+                      + (" (bucket fill serial; sort, blend and backward parallel over pixels)" if openmp else ""),
             "seconds": dt}
 
 
@@ -239,13 +240,14 @@ def run_reference(args) -> int:
     return 0
 
 
-def workload_config(wl, args) -> dict:
+def workload_config(wl, args, n_sets: int = 1) -> dict:
     return {"workload": f"{wl.name}: BASELINE.json config '{args.workload}', N={wl.N} points, "
                         f"{wl.cam.width}x{wl.cam.height}, D={wl.D}, seed {wl.seed}",
             "n_points": wl.N, "width": wl.cam.width, "height": wl.cam.height, "D": wl.D,
             "pass": "forward + backward (grad_feat, grad_opacity, grad_uv)",
             "parallelism": "replicas only (one cloud per GPU, no data-path collective)",
-            "l2_hygiene": "inputs + records larger than L2 (see l2 key)"}
+            "l2_hygiene": "inputs + records larger than L2 (see l2 key)" if n_sets == 1 else
+                          f"working set fits L2: {n_sets} independent buffer sets rotated (see l2 key)"}
 
 
 def make_step_functions(raster, wl, dev, stream=None):
@@ -280,6 +282,103 @@ def make_step_functions(raster, wl, dev, stream=None):
 
 
 # ------------------------------------------------------------------------------------------------
+# DRAM traffic per launch: read from the committed ncu CSV, never typed in
+def source_hash() -> str:
+    """sha256 over the kernel sources (csrc/*, include/*.h): what a traffic capture is valid for."""
+    import hashlib
+    h = hashlib.sha256()
+    for d in (os.path.join(ROOT, "paper_2403_16862_b200", "csrc"), os.path.join(ROOT, "include")):
+        for fn in sorted(os.listdir(d)):
+            if fn.endswith((".cu", ".cuh", ".h")):
+                h.update(fn.encode())
+                h.update(open(os.path.join(d, fn), "rb").read())
+    return h.hexdigest()[:16]
+
+
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")      # raw `ncu --csv` output, see r02_traffic.md
+
+
+def ncu_traffic(workload: str) -> dict:
+    """{stage name: mean dram read+write bytes per launch} from profiles/r02_traffic.csv, or {} (with the reason)
+    when the capture is for other kernel sources or another workload (profiles/r02_traffic.md records both)."""
+    import csv
+    import re
+    md = TRAFFIC_CSV[:-4] + ".md"
+    if not (os.path.exists(TRAFFIC_CSV) and os.path.exists(md)):
+        return {"_note": "no committed capture (profiles/r02_traffic.csv)"}
+    text = open(md).read()
+    m_hash = re.search(r"source_hash:\s*`?([0-9a-f]{16})", text)
+    m_wl = re.search(r"workload:\s*`?(\w+)", text)
+    if not m_hash or m_hash.group(1) != source_hash():
+        return {"_note": f"capture is for kernel sources {m_hash.group(1) if m_hash else '?'}, this build is {source_hash()}: traffic null"}
+    if not m_wl or m_wl.group(1) != workload:
+        return {"_note": f"capture is for workload {m_wl.group(1) if m_wl else '?'}: traffic null"}
+    rows = [r for r in csv.reader(open(TRAFFIC_CSV)) if len(r) > 5]
+    head = next(r for r in rows if "Kernel Name" in r)
+    ik, im, iv, iu = head.index("Kernel Name"), head.index("Metric Name"), head.index("Metric Value"), head.index("Metric Unit")
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    acc, cnt = {}, {}
+    for r in rows:
+        if r is head or not r[im].startswith("dram__bytes_"):
+            continue
+        name = r[ik].split("(")[0].replace("void ", "").replace("inpc::", "").strip()
+        acc[name] = acc.get(name, 0.0) + float(r[iv].replace(",", "")) * scale.get(r[iu], 1.0)
+        if r[im].startswith("dram__bytes_read"):
+            cnt[name] = cnt.get(name, 0) + 1
+    out = {k: acc[k] / max(cnt.get(k, 1), 1) for k in acc}
+    out["_note"] = f"profiles/r02_traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean per launch; sources {source_hash()})"
+    return out
+
+
+def traffic_of_stage(traffic: dict, stage: str):
+    """Stage names carry no template arguments; the capture's kernel names do (k_blend<4, 1, 0>)."""
+    vals = [v for k, v in traffic.items() if not k.startswith("_") and k.split("<")[0] == stage]
+    return sum(vals) / len(vals) if vals else None
+
+
+# ------------------------------------------------------------------------------------------------
+def workload_statistics(raster, wl, T, dev) -> dict:
+    """the workload characterised, not assumed -- per-pixel fragment counts, how much of them the
+    cut-off lets through, depth ties, termination-ambiguous pixels.  One extra forward with INPC_SAVE_SORTED,
+    outside every timed region; all reductions on the device."""
+    import torch
+    W, H, D, N = wl.cam.width, wl.cam.height, wl.D, wl.N
+    flags = raster.SAVE_FOR_BACKWARD | raster.SAVE_SORTED
+    try:
+        ws = raster.alloc_workspace(N, D, W, H, flags, dev)
+    except Exception as e:                                   # very large configs on a small device
+        return {"note": f"skipped: {e}"}
+    raster.inpc_raster_forward(T["pos"], T["op"], T["feat"], T["cam"], out_feat=T["img"], out_alpha=T["alpha"],
+                               workspace=ws, flags=flags)
+    cnt = raster.inpc_raster_get_counts(ws, W, H).reshape(-1).to(torch.int64)
+    nb = raster.inpc_raster_get_blended_counts(ws, W, H).reshape(-1).to(torch.int64)
+    off, _, dep, tr = raster.inpc_raster_get_sorted(ws, W, H, transmittance=True)
+    total = int(cnt.sum())
+    q = torch.quantile(cnt.to(torch.float32)[:: max(1, cnt.numel() // 4_000_000)], torch.tensor([0.5, 0.9, 0.99], device=dev))
+    # depth ties: consecutive fragments of ONE pixel with equal depth bits
+    ties = 0
+    if total > 1:
+        same = dep[1:] == dep[:-1]
+        starts = torch.zeros(total + 1, dtype=torch.bool, device=dev)
+        starts[off.to(torch.int64).clamp(max=total)] = True          # first fragment of every pixel
+        ties = int((same & ~starts[1:total]).sum())
+    # termination-ambiguous pixels as the KERNEL sees them: a transmittance it tested within 1e-4 (relative) of 1e-4
+    near = ((tr - 1e-4).abs() < 1e-8) & (tr > 0)
+    flagged = 0
+    if total:
+        pix_of = torch.searchsorted(off.to(torch.int64)[1:].contiguous(), torch.nonzero(near).reshape(-1), right=True)
+        flagged = int(torch.unique(pix_of).numel())
+    del ws
+    return {"fragments": total, "pixels": int(cnt.numel()),
+            "fragments_per_pixel": {"mean": total / max(1, cnt.numel()), "p50": float(q[0]), "p90": float(q[1]),
+                                    "p99": float(q[2]), "max": int(cnt.max()) if cnt.numel() else 0},
+            "blended_fragments": int(nb.sum()), "blended_fraction": float(nb.sum()) / max(1, total),
+            "pixels_reaching_cutoff": int((nb < cnt).sum()),
+            "depth_ties": ties, "termination_ambiguous_pixels": flagged,
+            "note": "termination-ambiguous = a blended fragment's fp32 transmittance within 1e-4 (relative) of the 1e-4 cut-off"}
+
+
+# ------------------------------------------------------------------------------------------------
 def run_ours(args) -> int:
     import numpy as np
     import torch
@@ -298,16 +397,35 @@ def run_ours(args) -> int:
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     raster.load()
+    assert FLAGS_STEP == raster.SAVE_FOR_BACKWARD
 
     wl = make_workload(args.workload, seed=CONFIGS[args.workload]["seed"] + rank)
     W, H, D, N = wl.cam.width, wl.cam.height, wl.D, wl.N
-    assert FLAGS_STEP == raster.SAVE_FOR_BACKWARD
-    flags = FLAGS_STEP
     stream = torch.cuda.current_stream()
-    fwd, bwd, T = make_step_functions(raster, wl, dev, stream)
+    # L2 hygiene: a working set that fits the 126 MB L2 would be timed L2-warm, so small workloads rotate through
+    # enough independent buffer sets (inputs, workspace, outputs) that a set is evicted before it comes round again
+    in_bytes = sum(a.nbytes for a in (wl.pos, wl.opacity, wl.feat, wl.g_img, wl.g_alpha))
+    set_bytes = in_bytes + raster.inpc_raster_workspace_bytes(N, D, W, H, FLAGS_STEP) + (W * H * (D + 1) + N * (D + 3)) * 4
+    n_sets = 1 if in_bytes > L2_BYTES else max(4, int(-(-3 * L2_BYTES // set_bytes)))
+    sets = [make_step_functions(raster, wl, dev, stream) for _ in range(n_sets)]
+    fwd0, bwd0, T = sets[0]
     cam, ws = T["cam"], T["ws"]
-    pos, op, feat, g_img, g_alpha = T["pos"], T["op"], T["feat"], T["g_img"], T["g_alpha"]
-    img, alpha, d_feat, d_op, d_uv = T["img"], T["alpha"], T["d_feat"], T["d_op"], T["d_uv"]
+    turn = [0]
+
+    def fwd(f=FLAGS_STEP):
+        sets[turn[0] % n_sets][0](f)
+
+    def bwd():
+        sets[turn[0] % n_sets][1]()
+
+    def step():
+        fwd()
+        bwd()
+        turn[0] += 1
+
+    def fwd_only():
+        fwd(FLAGS_FWD)
+        turn[0] += 1
 
     def barrier():
         if world > 1:
@@ -315,21 +433,30 @@ def run_ours(args) -> int:
         torch.cuda.synchronize()
 
     def timed(fn, steps):
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        """-> (total ms of exactly `steps` calls, per-call ms list); CUDA events on the launch stream."""
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
         barrier()
-        e0.record(stream)
-        for _ in range(steps):
+        ev[0].record(stream)
+        for i in range(steps):
             fn()
-        e1.record(stream)
+            ev[i + 1].record(stream)
         barrier()
-        return e0.elapsed_time(e1)
+        per = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+        return ev[0].elapsed_time(ev[steps]), per
 
-    def step():
-        fwd()
-        bwd()
+    def med_min(per):
+        s = sorted(per)
+        return s[len(s) // 2], s[0]
 
     clocks = ClockSampler(local_rank) if rank == 0 else None
-    for _ in range(max(args.warmup, 3)):
+
+    def windowed(fn, steps):
+        if clocks:
+            with clocks.window():
+                return timed(fn, steps)
+        return timed(fn, steps)
+
+    for _ in range(max(args.warmup, 3) * (2 if n_sets > 1 else 1)):
         step()
     torch.cuda.synchronize()
     stats = raster.inpc_raster_get_stats(ws)
@@ -337,39 +464,32 @@ def run_ours(args) -> int:
 
     # ---- the headline: exactly K fwd+bwd steps, device-resident inputs -------------------------------
     l0 = raster.inpc_raster_launch_count()
-    if clocks:
-        with clocks.window():
-            ms_total = timed(step, args.steps)
-    else:
-        ms_total = timed(step, args.steps)
+    ms_total, per_step = windowed(step, args.steps)
     launches = raster.inpc_raster_launch_count() - l0
     ms_total, units = aggregate_over_ranks(ms_total, float(n_frag) * args.steps, dev)
     ms_step = ms_total / args.steps
     value = throughput(units, ms_total)
+    ms_step_med, ms_step_min = med_min(per_step)
 
     # ---- forward only (inference flags) ---------------------------------------------------------------
     for _ in range(3):
-        fwd(FLAGS_FWD)
-    if clocks:
-        with clocks.window():
-            ms_fwd_total = timed(lambda: fwd(FLAGS_FWD), args.steps)
-    else:
-        ms_fwd_total = timed(lambda: fwd(FLAGS_FWD), args.steps)
+        fwd_only()
+    ms_fwd_total, per_fwd = windowed(fwd_only, args.steps)
     ms_fwd_total, _ = aggregate_over_ranks(ms_fwd_total, 0.0, dev)
     ms_fwd = ms_fwd_total / args.steps
+    ms_fwd_med, ms_fwd_min = med_min(per_fwd)
 
-    # ---- per-stage device times (library-side CUDA events on the launching stream) --------------------
+    # ---- per-stage device times (library-side CUDA events on the launching stream; every kernel alone) -----
     raster.inpc_raster_set_kernel_timing(True)
     raster.inpc_raster_get_kernel_times(reset=True)
-    if clocks:
-        with clocks.window():
-            ms_staged = timed(step, args.steps)
-    else:
-        ms_staged = timed(step, args.steps)
+    ms_staged, _ = windowed(step, args.steps)
     stages = raster.inpc_raster_get_kernel_times(reset=True)
     raster.inpc_raster_set_kernel_timing(False)
 
     # ---- end to end: host buffers in, host buffers out, copies inside the timed region ----------------
+    pos, op, feat, g_img, g_alpha = T["pos"], T["op"], T["feat"], T["g_img"], T["g_alpha"]
+    img, alpha, d_feat, d_op, d_uv = T["img"], T["alpha"], T["d_feat"], T["d_op"], T["d_uv"]
+    flags = FLAGS_STEP
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_in = [pin(wl.pos), pin(wl.opacity), pin(wl.feat), pin(wl.g_img), pin(wl.g_alpha)]
     d_in = [pos, op, feat, g_img, g_alpha]
@@ -382,14 +502,14 @@ def run_ours(args) -> int:
     # device->host copy overlap (PCIe is full duplex); every step still copies ITS inputs in and ITS results out
     # inside the timed region.
     s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
-    sets = []
+    esets = []
     for b in range(2):
         di = d_in if b == 0 else [torch.empty_like(t) for t in d_in]
         do = d_out if b == 0 else [torch.empty_like(t) for t in d_out]
         wsb = ws if b == 0 else raster.alloc_workspace(N, D, W, H, flags, dev)
         ho = h_out if b == 0 else [torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in d_out]
-        sets.append({"d_in": di, "d_out": do, "ws": wsb, "h_out": ho,
-                     "in_ready": torch.cuda.Event(), "done": torch.cuda.Event(), "out_free": torch.cuda.Event()})
+        esets.append({"d_in": di, "d_out": do, "ws": wsb, "h_out": ho,
+                      "in_ready": torch.cuda.Event(), "done": torch.cuda.Event(), "out_free": torch.cuda.Event()})
 
     def e2e_pipeline(steps):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -397,7 +517,7 @@ def run_ours(args) -> int:
         s_in.wait_stream(stream); s_out.wait_stream(stream)
         e0.record(s_in)
         for i in range(steps):
-            S = sets[i % 2]
+            S = esets[i % 2]
             if i >= 2:
                 s_in.wait_event(S["done"])               # step i-2 has finished reading these inputs
             with torch.cuda.stream(s_in):
@@ -427,14 +547,14 @@ def run_ours(args) -> int:
     def e2e_step():                                       # the same, one stream, nothing overlapped
         for h, d in zip(h_in, d_in):
             d.copy_(h, non_blocking=True)
-        fwd()
-        bwd()
+        fwd0()
+        bwd0()
         for d, h in zip(d_out, h_out):
             h.copy_(d, non_blocking=True)
 
     e2e_steps = max(2, min(args.steps, 10))
     e2e_step()
-    ms_e2e_serial = timed(e2e_step, e2e_steps) / e2e_steps
+    ms_e2e_serial = timed(e2e_step, e2e_steps)[0] / e2e_steps
     e2e_pipeline(2)
     if clocks:
         with clocks.window():
@@ -450,6 +570,8 @@ def run_ours(args) -> int:
             dist.destroy_process_group()
         return 0
 
+    wstats = workload_statistics(raster, wl, T, dev) if not args.no_stats else {"note": "skipped (--no-stats)"}
+
     # ---- roofline --------------------------------------------------------------------------------------
     peak, peak_src = measured_peak_gbs()
     P = W * H
@@ -457,28 +579,47 @@ def run_ours(args) -> int:
     per_stage = {k: (ms / n if n else 0.0) for k, (ms, n) in stages.items()}
     step_stage_ms = {k: ms / args.steps for k, (ms, n) in stages.items() if n}
     kernels = {k: v for k, v in step_stage_ms.items() if k.startswith("k_")}
+    traffic = ncu_traffic(args.workload)
+    groups = {}
+    for g in ("a1_a2", "a3_a4", "a5_walk", "a5_out"):
+        g_ms = sum(v for k, v in step_stage_ms.items() if STAGE_ROWS.get(k) == g)
+        if g_ms <= 0:
+            continue
+        tr = [traffic_of_stage(traffic, k) for k in step_stage_ms if STAGE_ROWS.get(k) == g and k.startswith("k_")]
+        tr = [t for t in tr if t is not None]
+        ach = alg[g] / (g_ms * 1e-3) / 1e9
+        groups[g] = {"algorithmic_bytes": alg[g], "ms": g_ms, "achieved": ach, "frac": ach / peak,
+                     "kernels": sorted(k for k in step_stage_ms if STAGE_ROWS.get(k) == g),
+                     "traffic": sum(tr) if tr else None}
     dom = max(kernels, key=kernels.get)
     rows = STAGE_ROWS[dom]
-    group_ms = sum(v for k, v in per_stage.items() if STAGE_ROWS.get(k) == rows)    # every kernel sharing these rows
-    achieved = alg[rows] / (group_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": dom, "rows": rows, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg[rows], "ms_per_launch": per_stage[dom],
-                "ms_rows": group_ms, "kernels_of_rows": sorted(k for k in per_stage if STAGE_ROWS.get(k) == rows and per_stage[k] > 0),
+    worst = min(groups, key=lambda g: groups[g]["frac"])
+    roofline = {"bound": "hbm", "kernel": dom, "rows": rows, "achieved": groups[rows]["achieved"], "peak": peak,
+                "unit": "GB/s", "frac": groups[rows]["frac"], "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg[rows], "ms_per_launch": per_stage[dom], "ms_rows": groups[rows]["ms"],
+                "kernels_of_rows": groups[rows]["kernels"],
                 "share_of_step": kernels[dom] / sum(step_stage_ms.values()),
-                "traffic": NCU_TRAFFIC.get(dom), "traffic_source": NCU_TRAFFIC_SOURCE}
+                "traffic": traffic_of_stage(traffic, dom), "traffic_source": traffic.get("_note"),
+                "furthest_below_roof": {"rows": worst, "frac": groups[worst]["frac"], "ms": groups[worst]["ms"],
+                                        "kernels": groups[worst]["kernels"]},
+                "note": "achieved = SURVEY 8d algorithmic bytes of the rows the dominant kernel implements / summed launch "
+                        "time of the kernels implementing those rows (each timed alone); every group is in roofline_groups, "
+                        "the whole step in roofline_step"}
     ach_step = alg["fwd_bwd"] / (ms_step * 1e-3) / 1e9
     ach_fwd = alg["fwd"] / (ms_fwd * 1e-3) / 1e9
     roofline_step = {"bound": "hbm", "algorithmic_bytes_fwd_bwd": alg["fwd_bwd"], "achieved": ach_step,
                      "peak": peak, "unit": "GB/s", "frac": ach_step / peak, "frac_of_8TBps_nominal": ach_step / 8000.0,
+                     "target_ms_for_50pct_of_8TBps": alg["fwd_bwd"] / 4000.0 / 1e6,
                      "fwd_only": {"algorithmic_bytes": alg["fwd"], "achieved": ach_fwd, "frac": ach_fwd / peak}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic", "config": workload_config(wl, args),
-        "ms_fwd": ms_fwd, "ms_fwd_bwd": ms_step, "fragments_per_sec_fwd": throughput(float(n_frag) * world, ms_fwd),
-        "fragments_per_step_per_gpu": n_frag, "stats": stats,
+        "ms_per_step": ms_step, "ms_per_step_median": ms_step_med, "ms_per_step_min": ms_step_min,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": workload_config(wl, args, n_sets),
+        "ms_fwd": ms_fwd, "ms_fwd_median": ms_fwd_med, "ms_fwd_min": ms_fwd_min, "ms_fwd_bwd": ms_step,
+        "fragments_per_sec_fwd": throughput(float(n_frag) * world, ms_fwd),
+        "fragments_per_step_per_gpu": n_frag, "stats": stats, "workload_statistics": wstats,
         "e2e": {"value": throughput(units_e2e, ms_e2e_total), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e_total / e2e_steps, "steps": e2e_steps,
                 "ms_per_step_one_stream": ms_e2e_serial,
@@ -487,14 +628,17 @@ def run_ours(args) -> int:
                        "sets overlap step i's H2D, step i-1's kernels and step i-2's D2H (ms_per_step_one_stream: "
                        "the same without overlap)"},
         "gpu_launches": launches,
-        "roofline": roofline, "roofline_step": roofline_step,
+        "roofline": roofline, "roofline_groups": groups, "roofline_step": roofline_step,
         "stage_ms_per_step": step_stage_ms, "stage_timed_ms_per_step": ms_staged / args.steps,
         "l2": {"l2_bytes": L2_BYTES, "input_bytes": h2d, "record_bytes": stats["n_kept"] * (20 + 4 * D),
-               "policy": "inputs larger than L2" if h2d > L2_BYTES else "inputs fit L2: numbers are L2-warm"},
+               "buffer_sets": n_sets,
+               "policy": "inputs larger than L2" if n_sets == 1 else
+                         f"inputs fit L2: {n_sets} independent buffer sets ({n_sets * set_bytes >> 20} MiB) rotated, one per step"},
         "clocks": clock_info,
     }
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(wl)
+        line["cpu_baseline_all_cores"] = cpu_baseline(wl, openmp=True)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
@@ -510,7 +654,12 @@ def main(argv=None) -> int:
     ap.add_argument("--workload", default="train", choices=["tiny", "1m", "train", "infer", "stress"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle leg (profiling runs)")
+    ap.add_argument("--no-stats", action="store_true", help="skip the workload statistics (profiling runs)")
+    ap.add_argument("--print-source-hash", action="store_true", help="print the kernel-source hash a traffic capture is recorded with")
     args = ap.parse_args(argv)
+    if args.print_source_hash:
+        print(source_hash())
+        return 0
     if args.impl == "reference":
         return run_reference(args)
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -101,6 +101,20 @@ int inpc_raster_backward(const float* pos, const float* opacity, const float* fe
                          float* grad_feat, float* grad_opacity, float* grad_uv,
                          void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* The same backward pass with the per-point BLENDING WEIGHT fused in (NEXT row f1 of the scope table):
+ *   blend_weight[N] = max over the point's blended fragments of alpha_c T_c, alpha_c = opacity w_c (Eq. 7) and
+ *   T_c the transmittance in front of that fragment (Eq. 1) -- "the transmitted blending weight b_j = alpha_j T_j"
+ *   that the probability update p_i' = max(lambda_u p_i, max{b_0..b_n}) of the octree consumes (Eq. 3,
+ *   PAPER.md:75-78; "the blending weight computation required for updating P [is] fused into this pipeline",
+ *   PAPER.md:370).  Culled points and points none of whose fragments was blended get exactly 0.  The max over
+ *   the points of a leaf (Eq. 3's outer max) is the sampler's business, not the rasterizer's.
+ *   It costs one extra coalesced 4-byte store per point: the four T_c a_c are already formed for grad_feat. */
+int inpc_raster_backward_weights(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                                 const inpc_camera* cam,
+                                 const float* grad_out_feat, const float* grad_out_alpha,
+                                 float* grad_feat, float* grad_opacity, float* grad_uv, float* blend_weight,
+                                 void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Sticky status of the device-side checks since the last forward on this workspace (synchronises):
  * INPC_OK, or why the last inpc_raster_backward refused to run (INPC_ERR_NO_SAVED_STATE: no forward
  * with INPC_SAVE_FOR_BACKWARD has filled this workspace; INPC_ERR_INVALID_ARG: N, D, W or H differ from

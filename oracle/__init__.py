@@ -15,18 +15,30 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
+_LIB_OMP = os.path.join(_HERE, "liboracle_omp.so")
 _lib = None
 
 T_MIN = 1e-4   # transmittance cut-off (BASELINE.json north_star; not in the paper)
 NO_FORCE = 0xFFFFFFFF   # force_nb value meaning "use the termination test"
 
 
-def build(force: bool = False) -> str:
-    """g++ -O2 -ffp-contract=off (the canonical fp32 projection must not be contracted to FMA)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c++17",
-                               "-shared", "-fPIC", "-o", _LIB, _SRC])
-    return _LIB
+def build(force: bool = False, openmp: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off (the canonical fp32 projection must not be contracted to FMA).
+    openmp=True builds the SAME source a second time with -fopenmp (liboracle_omp.so): only bench.py's
+    all-cores baseline leg uses it (use_openmp); every test runs the single-threaded build."""
+    lib = _LIB_OMP if openmp else _LIB
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c++17"] +
+                              (["-fopenmp"] if openmp else []) + ["-shared", "-fPIC", "-o", lib, _SRC])
+    return lib
+
+
+def use_openmp(on: bool) -> int:
+    """Switch this process to the -fopenmp build (bench.py only) or back; returns the threads it will use."""
+    global _lib
+    _lib = None
+    _load(openmp=on)
+    return int(_lib.oracle_threads())
 
 
 class _Camera(C.Structure):
@@ -36,10 +48,11 @@ class _Camera(C.Structure):
                 ("width", C.c_int32), ("height", C.c_int32)]
 
 
-def _load():
+def _load(openmp: bool = False):
     global _lib
     if _lib is None:
-        lib = C.CDLL(build())
+        lib = C.CDLL(build(openmp=openmp))
+        lib.oracle_threads.restype = C.c_int
         lib.oracle_create.restype = C.c_void_p
         lib.oracle_create.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]
         lib.oracle_create_uv.restype = C.c_void_p
@@ -53,6 +66,8 @@ def _load():
         lib.oracle_blend.argtypes = [C.c_void_p, C.c_double] + [C.c_void_p] * 5
         lib.oracle_sorted_T.restype = C.c_int
         lib.oracle_sorted_T.argtypes = [C.c_void_p, C.c_void_p]
+        lib.oracle_blend_weights.restype = C.c_int
+        lib.oracle_blend_weights.argtypes = [C.c_void_p, C.c_void_p]
         lib.oracle_backward.restype = C.c_int
         lib.oracle_backward.argtypes = [C.c_void_p] * 6
         lib.oracle_count_fp64_projection_changes.restype = C.c_int64
@@ -162,6 +177,14 @@ class Raster:
         if _lib.oracle_sorted_T(self._h, _p(T)) != 0:
             raise RuntimeError("oracle_sorted_T: blend() has not been called")
         return T
+
+    def blend_weights(self) -> np.ndarray:
+        """Per-point blending weight b = max over the point's blended fragments of alpha T (Eq. 3's input); call
+        blend() first.  -> [N] f64."""
+        bw = np.empty(self.N, dtype=np.float64)
+        if _lib.oracle_blend_weights(self._h, _p(bw)) != 0:
+            raise RuntimeError("oracle_blend_weights: blend() has not been called")
+        return bw
 
     def backward(self, g_img, g_alpha=None):
         """Gradients of <g_img, img> + <g_alpha, alpha>; call blend() first (same t_min).

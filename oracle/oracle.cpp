@@ -21,6 +21,11 @@
 //   fragments kept and counted; fragment k blended iff the transmittance before it is >= t_min
 //   (1e-4 in BASELINE.json's north_star; not in the paper); premultiplied features; alpha output.
 //
+// Threads: none.  The `#pragma omp` lines below are inert in the build every test uses (no -fopenmp);
+// bench.py's all-cores baseline leg builds the SAME source a second time with -fopenmp (liboracle_omp.so,
+// SURVEY.md section 8d "Oracle timed beside it" (2)): pixels are independent in S3 / S4, and in the backward
+// pass the per-point sums become `omp atomic` updates.  The arithmetic is untouched.
+//
 // Pins (tests/test_oracle_*.py, -m "not gpu"): closed forms, invariants, brute force, the adjoint
 // of torch grid_sample, central finite differences, an independent torch-autograd restatement.
 // No function here is "parity unpinned".
@@ -29,6 +34,9 @@
 #include <cstdint>
 #include <cstring>
 #include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 namespace {
 
@@ -85,11 +93,15 @@ void emit(State& s, double fu, double fv, double x0, double y0, uint32_t depth_b
 
 // S3: ascending (depth_bits, idx).
 void sort_buckets(State& s) {
-    for (auto& b : s.bucket)
+    const long P = (long)s.bucket.size();
+#pragma omp parallel for schedule(dynamic, 256)
+    for (long p = 0; p < P; ++p) {
+        auto& b = s.bucket[p];
         std::sort(b.begin(), b.end(), [](const Frag& x, const Frag& y) {
             if (x.depth_bits != y.depth_bits) return x.depth_bits < y.depth_bits;
             return x.idx < y.idx;
         });
+    }
 }
 
 State* new_state(int64_t N, int D, int W, int H, const float* opacity, const float* feat) {
@@ -159,6 +171,20 @@ int64_t oracle_total(void* h) {
     return t;
 }
 int64_t oracle_kept(void* h) { return ((State*)h)->kept; }
+// threads the build can use: 1 unless compiled with -fopenmp (bench.py's all-cores leg)
+int oracle_threads(void) {
+#ifdef _OPENMP
+    int n = 1;
+#pragma omp parallel
+    {
+#pragma omp master
+        n = omp_get_num_threads();
+    }
+    return n;
+#else
+    return 1;
+#endif
+}
 int64_t oracle_border_dropped(void* h) { return ((State*)h)->border_dropped; }
 
 void oracle_counts(void* h, uint32_t* counts) {
@@ -192,7 +218,9 @@ void oracle_sorted(void* h, int64_t* offsets, int64_t* point_idx, uint32_t* dept
 void oracle_blend(void* h, double t_min, const uint32_t* force_nb, double* img, double* alpha, uint32_t* nb,
                   double* margin) {
     State* s = (State*)h; const int D = s->D;
-    for (size_t p = 0; p < s->bucket.size(); ++p) {
+    const long P = (long)s->bucket.size();
+#pragma omp parallel for schedule(dynamic, 256)
+    for (long p = 0; p < P; ++p) {
         double T = 1.0, A = 0.0, m = INFINITY;
         double* C = img + p * D;
         for (int d = 0; d < D; ++d) C[d] = 0.0;
@@ -234,6 +262,24 @@ int oracle_sorted_T(void* h, double* T) {
     return 0;
 }
 
+// NEXT row f1 -- per-point blending weight, the input of the octree's probability update (Eq. 3,
+// PAPER.md:75-78): "we use the transmitted blending weight b_j = alpha_j T_j (Eq. (1)) for the updates".
+// A point has up to four fragments (Eq. 7); its weight is the largest alpha T among those the last
+// oracle_blend composited (reading: a point "generated using the i-th leaf" contributes through whichever
+// of its splats is most visible; the max over the points of a leaf is the sampler's).  Points without a
+// blended fragment (culled, outside the image, or entirely behind the cut-off) get 0.
+int oracle_blend_weights(void* h, double* bw) {
+    State* s = (State*)h;
+    if (!s->blended) return -1;
+    for (int64_t i = 0; i < s->N; ++i) bw[i] = 0.0;
+    for (size_t p = 0; p < s->bucket.size(); ++p)
+        for (uint32_t k = 0; k < s->nb[p]; ++k) {
+            const Frag& f = s->bucket[p][k];
+            bw[f.idx] = std::max(bw[f.idx], f.a * f.T);
+        }
+    return 0;
+}
+
 // S5 + S6: gradients of  L = <g_img, img> + <g_alpha, alpha>  w.r.t. features, opacities and the
 // projected position (u, v) of every point (per-splat gradients in forward order,
 // four splat gradients combined with the bilinear weights).  Division-free reverse recurrence:
@@ -247,7 +293,9 @@ int oracle_backward(void* h, const double* g_img, const double* g_alpha,
     if (!s->blended) return -1;
     for (int64_t i = 0; i < s->N * D; ++i) d_feat[i] = 0.0;
     for (int64_t i = 0; i < s->N; ++i) { d_opacity[i] = 0.0; d_uv[2 * i] = 0.0; d_uv[2 * i + 1] = 0.0; }
-    for (size_t p = 0; p < s->bucket.size(); ++p) {
+    const long P = (long)s->bucket.size();
+#pragma omp parallel for schedule(dynamic, 256)
+    for (long p = 0; p < P; ++p) {
         const double* g = g_img + p * D;
         const double gA = g_alpha ? g_alpha[p] : 0.0;
         auto& b = s->bucket[p];
@@ -259,10 +307,16 @@ int oracle_backward(void* h, const double* g_img, const double* g_alpha,
             for (int d = 0; d < D; ++d) G += (double)F[d] * g[d];
             const double dLda = f.T * (G - B);
             B = f.a * G + (1.0 - f.a) * B;
-            for (int d = 0; d < D; ++d) d_feat[(size_t)f.idx * D + d] += f.T * f.a * g[d];
+            for (int d = 0; d < D; ++d) {
+#pragma omp atomic
+                d_feat[(size_t)f.idx * D + d] += f.T * f.a * g[d];
+            }
             const double op = (double)s->opacity[f.idx];
+#pragma omp atomic
             d_opacity[f.idx] += f.w * dLda;
+#pragma omp atomic
             d_uv[2 * f.idx]     += op * f.dwdu * dLda;
+#pragma omp atomic
             d_uv[2 * f.idx + 1] += op * f.dwdv * dLda;
         }
     }

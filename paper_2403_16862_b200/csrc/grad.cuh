@@ -7,11 +7,13 @@
 //                 dL/dfeat    = sum_c T_c a_c g_img[pixel_c]            (S5)
 //                 dL/dopacity = sum_c w_c dL/da_c                        (S6)
 //                 dL/d(u, v)  = opacity * sum_c (dw_c/du, dw_c/dv) dL/da_c
+//              and, in the same pass, the point's BLENDING WEIGHT  b = max_c T_c a_c  over its blended
+//              fragments (Eq. 3's update input; "fused into this pipeline"),
 //              and writes them as ONE (D = 4) or TWO (D = 8) full 32-byte sectors to gpt[point_idx]: the
 //              only scattered write of the backward pass, and never narrower than a sector.  No atomics:
 //              every fragment has exactly one writer, so gradients are bit-reproducible run to run.
-//   k_split    one thread per POINT: gpt -> grad_feat[N][D], grad_opacity[N], grad_uv[N][2] (coalesced);
-//              culled points (their bit of the kept mask is 0) get exact zeros.
+//   k_split    one thread per POINT: gpt -> grad_feat[N][D], grad_opacity[N], grad_uv[N][2] and, when asked for,
+//              blend_weight[N] (coalesced); culled points (their bit of the kept mask is 0) get exact zeros.
 #pragma once
 #include "common.cuh"
 
@@ -72,7 +74,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
             float df[D];
 #pragma unroll
             for (int d = 0; d < D; ++d) df[d] = 0.f;
-            float dop = 0.f, du = 0.f, dv = 0.f;
+            float dop = 0.f, du = 0.f, dv = 0.f, bw = 0.f;
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const int dx = c & 1, dy = c >> 1;
@@ -81,6 +83,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                 const float wx = dx ? r0.x : 1.f - r0.x, wy = dy ? r0.y : 1.f - r0.y;
                 const float Ta = tc[c] * (r0.z * (wx * wy));
                 const float dl = dc[c];
+                bw = fmaxf(bw, Ta);                                        // b = alpha T of this fragment (Eq. 3)
                 dop += wx * wy * dl;
                 du += (dx ? wy : -wy) * dl;
                 dv += (dy ? wx : -wx) * dl;
@@ -93,10 +96,10 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
             du *= r0.z; dv *= r0.z;
             float4* out = reinterpret_cast<float4*>(gpt + (size_t)__float_as_uint(r0.w) * GP);
             if (D == 4) {
-                st_sector(out, make_float4(df[0], df[1], df[2], df[3]), make_float4(dop, du, dv, 0.f));
+                st_sector(out, make_float4(df[0], df[1], df[2], df[3]), make_float4(dop, du, dv, bw));
             } else {
                 st_sector(out, make_float4(df[0], df[1], df[2], df[3]), make_float4(df[4], df[5], df[6], df[7]));
-                st_sector(out + 2, make_float4(dop, du, dv, 0.f), make_float4(0.f, 0.f, 0.f, 0.f));
+                st_sector(out + 2, make_float4(dop, du, dv, bw), make_float4(0.f, 0.f, 0.f, 0.f));
             }
         }
     }
@@ -106,7 +109,7 @@ template <int D>
 __global__ void __launch_bounds__(256) k_split(const Header* __restrict__ hdr, const float* __restrict__ gpt,
                                                 const uint32_t* __restrict__ kept,
                                                 long long N, float* __restrict__ d_feat, float* __restrict__ d_opacity,
-                                                float* __restrict__ d_uv) {
+                                                float* __restrict__ d_uv, float* __restrict__ blend_weight) {
     constexpr int GP = gpt_floats<D>();
     if (!hdr->bwd_ok) return;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
@@ -123,6 +126,7 @@ __global__ void __launch_bounds__(256) k_split(const Header* __restrict__ hdr, c
         for (int v = 0; v < D / 4; ++v) __stcs(reinterpret_cast<float4*>(d_feat + (size_t)i * D) + v, f[v]);
         __stcs(&d_opacity[i], o.x);
         __stcs(reinterpret_cast<float2*>(d_uv) + i, make_float2(o.y, o.z));
+        if (blend_weight) __stcs(&blend_weight[i], o.w);
     }
 }
 

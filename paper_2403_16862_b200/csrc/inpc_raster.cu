@@ -451,7 +451,8 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
 
 template <int D>
 static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat, const float* g_alpha, float* d_feat,
-                         float* d_opacity, float* d_uv, unsigned char* ws, const Layout& L, cudaStream_t st) {
+                         float* d_opacity, float* d_uv, float* blend_weight, unsigned char* ws, const Layout& L,
+                         cudaStream_t st) {
     const DeviceInfo di = device_info();
     if (!di.ok) return cuda_fail(cudaErrorNoDevice);
     const int W = cam->width, H = cam->height;
@@ -509,7 +510,7 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     INPC_CUDA(fork(s2, st));                                                  // join
     { StageTimer tm(kStSplit, st);
       k_split<D><<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16), 256, 0, st>>>(
-          hdr, gpt, reinterpret_cast<const uint32_t*>(ws + L.kept), (long long)N, d_feat, d_opacity, d_uv); }
+          hdr, gpt, reinterpret_cast<const uint32_t*>(ws + L.kept), (long long)N, d_feat, d_opacity, d_uv, blend_weight); }
     INPC_LAUNCHED(kname<D>("k_split"));
     return INPC_OK;
 }
@@ -543,17 +544,15 @@ int inpc_raster_forward(const float* pos, const float* opacity, const float* fea
                   : forward_impl<8>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st);
 }
 
-int inpc_raster_backward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
-                         const inpc_camera* cam, const float* grad_out_feat, const float* grad_out_alpha,
-                         float* grad_feat, float* grad_opacity, float* grad_uv, void* workspace,
-                         size_t workspace_bytes, void* cuda_stream) {
-    (void)pos; (void)opacity; (void)feat;   // the records saved by the forward hold what the backward needs
+static int backward_entry(int64_t N, int32_t D, const inpc_camera* cam, const float* grad_out_feat,
+                          const float* grad_out_alpha, float* grad_feat, float* grad_opacity, float* grad_uv,
+                          float* blend_weight, void* workspace, size_t workspace_bytes, void* cuda_stream) {
     int rc = check_common(N, D, cam);
     if (rc != INPC_OK) return rc;
     if (!grad_out_feat || !workspace) return INPC_ERR_INVALID_ARG;
     if (N > 0 && (!grad_feat || !grad_opacity || !grad_uv)) return INPC_ERR_INVALID_ARG;
     if (!aligned16(grad_out_feat) || !aligned16(grad_out_alpha) || !aligned16(grad_feat) || !aligned16(grad_opacity) ||
-        !aligned16(grad_uv) || (reinterpret_cast<uintptr_t>(workspace) & 255u))
+        !aligned16(grad_uv) || !aligned16(blend_weight) || (reinterpret_cast<uintptr_t>(workspace) & 255u))
         return INPC_ERR_INVALID_ARG;
     // Everything the backward pass touches lies in front of the INPC_SAVE_SORTED arrays, so its layout follows
     // from these arguments alone; whether the workspace really holds that forward is checked ON THE DEVICE
@@ -562,8 +561,27 @@ int inpc_raster_backward(const float* pos, const float* opacity, const float* fe
     if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     unsigned char* ws = static_cast<unsigned char*>(workspace);
-    return D == 4 ? backward_impl<4>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, ws, L, st)
-                  : backward_impl<8>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, ws, L, st);
+    return D == 4 ? backward_impl<4>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight, ws, L, st)
+                  : backward_impl<8>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight, ws, L, st);
+}
+
+int inpc_raster_backward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                         const inpc_camera* cam, const float* grad_out_feat, const float* grad_out_alpha,
+                         float* grad_feat, float* grad_opacity, float* grad_uv, void* workspace,
+                         size_t workspace_bytes, void* cuda_stream) {
+    (void)pos; (void)opacity; (void)feat;   // the records saved by the forward hold what the backward needs
+    return backward_entry(N, D, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, nullptr, workspace,
+                          workspace_bytes, cuda_stream);
+}
+
+int inpc_raster_backward_weights(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                                 const inpc_camera* cam, const float* grad_out_feat, const float* grad_out_alpha,
+                                 float* grad_feat, float* grad_opacity, float* grad_uv, float* blend_weight,
+                                 void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    (void)pos; (void)opacity; (void)feat;
+    if (N > 0 && !blend_weight) return INPC_ERR_INVALID_ARG;
+    return backward_entry(N, D, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight,
+                          workspace, workspace_bytes, cuda_stream);
 }
 
 // The introspection calls synchronise: they read the workspace's Header back and take shape, D and flags from it.

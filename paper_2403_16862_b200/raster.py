@@ -18,7 +18,7 @@ SAVE_FOR_BACKWARD = 1
 SAVE_SORTED = 2
 
 EXPORTS = (
-    "inpc_raster_workspace_bytes", "inpc_raster_forward", "inpc_raster_backward",
+    "inpc_raster_workspace_bytes", "inpc_raster_forward", "inpc_raster_backward", "inpc_raster_backward_weights",
     "inpc_raster_get_counts", "inpc_raster_get_blended_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
     "inpc_raster_get_status",
     "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count", "inpc_raster_launched_kernels",
@@ -67,6 +67,8 @@ def load() -> C.CDLL:
         lib.inpc_raster_forward.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, C.c_size_t, u32, vp]
         lib.inpc_raster_backward.restype = C.c_int
         lib.inpc_raster_backward.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        lib.inpc_raster_backward_weights.restype = C.c_int
+        lib.inpc_raster_backward_weights.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
         lib.inpc_raster_get_counts.restype = C.c_int
         lib.inpc_raster_get_counts.argtypes = [vp, i32, i32, vp, vp]
         lib.inpc_raster_get_blended_counts.restype = C.c_int
@@ -153,8 +155,10 @@ def inpc_raster_forward(pos, opacity, feat, cam, out_feat=None, out_alpha=None, 
 
 
 def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha, workspace,
-                         grad_feat=None, grad_opacity=None, grad_uv=None, stream=None):
-    """-> (grad_feat[N,D], grad_opacity[N], grad_uv[N,2]).  Enqueues on the current stream; no sync."""
+                         grad_feat=None, grad_opacity=None, grad_uv=None, stream=None, blend_weight=None):
+    """-> (grad_feat[N,D], grad_opacity[N], grad_uv[N,2]).  Enqueues on the current stream; no sync.
+    With blend_weight (True, or a float32 tensor [N]) the fused per-point blending weights (Eq. 3) come back
+    as a fourth result (inpc_raster_backward_weights)."""
     lib = load()
     N, D = int(pos.shape[0]), int(feat.shape[1])
     cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
@@ -168,6 +172,15 @@ def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha,
         grad_opacity = torch.empty((N,), dtype=torch.float32, device=dev)
     if grad_uv is None:
         grad_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
+    if blend_weight is not None and blend_weight is not False:
+        if blend_weight is True:
+            blend_weight = torch.empty((N,), dtype=torch.float32, device=dev)
+        rc = lib.inpc_raster_backward_weights(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(grad_out_feat),
+                                              _ptr(grad_out_alpha), _ptr(grad_feat), _ptr(grad_opacity), _ptr(grad_uv),
+                                              _ptr(blend_weight), _ptr(workspace), workspace.numel(), _stream(stream))
+        if rc != 0:
+            raise InpcError(rc, "inpc_raster_backward_weights")
+        return grad_feat, grad_opacity, grad_uv, blend_weight
     rc = lib.inpc_raster_backward(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(grad_out_feat),
                                   _ptr(grad_out_alpha), _ptr(grad_feat), _ptr(grad_opacity), _ptr(grad_uv),
                                   _ptr(workspace), workspace.numel(), _stream(stream))

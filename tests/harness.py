@@ -5,6 +5,7 @@ inputs and compare them element by element (BASELINE.json north_star tolerances)
   per-pixel blended fragment counts                    : bit-exact outside termination-ambiguous pixels
   feature image, alpha                                 : max abs error <= 1e-4, EVERY pixel
   gradients                                            : |gpu - ref| <= max(1e-3 |ref|, 1e-5), EVERY point
+  fused per-point blending weights (f1, Eq. 3 input)   : max abs error <= 1e-5, EVERY point
 
 Every workload is run in the three launch configurations that exist:
   A  flags SAVE_FOR_BACKWARD | SAVE_SORTED  (k_blend<D,1>, k_big<D,1>): counts, order, per-fragment transmittance
@@ -34,6 +35,7 @@ from paper_2403_16862_b200 import raster
 FWD_ATOL = 1e-4
 GRAD_RTOL = 1e-3
 GRAD_ATOL = 1e-5
+BW_ATOL = 1e-5         # blending weights are alpha T <= 1; the fp32 transmittance drifts by ~1e-5 relative at most
 MARGIN = 1e-4          # relative distance of a tested transmittance to the cut-off below which a pixel is ambiguous
 
 FLAGS_DUMP = raster.SAVE_FOR_BACKWARD | raster.SAVE_SORTED
@@ -53,10 +55,11 @@ def gpu_forward(wl, flags=FLAGS_DUMP, inputs=None):
     return dict(pos=pos, op=op, feat=feat, img=img, alpha=alpha, ws=ws, flags=flags)
 
 
-def gpu_backward(wl, st, g_alpha=True):
+def gpu_backward(wl, st, g_alpha=True, weights=False):
     g_img = to_dev(wl.g_img)
     g_a = to_dev(wl.g_alpha) if g_alpha else None
-    out = raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g_img, g_a, st["ws"])
+    out = raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g_img, g_a, st["ws"],
+                                      blend_weight=True if weights else None)
     torch.cuda.synchronize()
     assert raster.inpc_raster_get_status(st["ws"]) == 0
     return out
@@ -158,12 +161,19 @@ def check_grads(name, got, want):
 
 
 def check_backward(wl, st, ref_grads, g_alpha=True, what=""):
-    """ref_grads = oracle gradients for the blend state the forward was compared with.  Every point is compared."""
-    d_feat, d_op, d_uv = gpu_backward(wl, st, g_alpha)
-    rf, ro, ru = ref_grads
+    """ref_grads = oracle gradients (+ blending weights) for the blend state the forward was compared with.
+    Every point is compared."""
+    d_feat, d_op, d_uv, bw = gpu_backward(wl, st, g_alpha, weights=True)
+    rf, ro, ru, rbw = ref_grads
     e = max(check_grads(what + "grad_feat", d_feat, rf), check_grads(what + "grad_opacity", d_op, ro),
             check_grads(what + "grad_uv", d_uv, ru))
-    return (d_feat, d_op, d_uv), e
+    ebw = np.abs(bw.cpu().numpy().astype(np.float64) - rbw)
+    assert ebw.size == 0 or ebw.max() <= BW_ATOL, f"{what}blend_weight: max error {ebw.max():.3e} at point {int(ebw.argmax())}"
+    # the plain entry point (no weights) gives the same gradients, bit for bit
+    plain = gpu_backward(wl, st, g_alpha)
+    for a, b in zip(plain, (d_feat, d_op, d_uv)):
+        assert torch.equal(a, b), what + "inpc_raster_backward and inpc_raster_backward_weights disagree"
+    return (d_feat, d_op, d_uv, bw), e
 
 
 def full_parity(wl, backward=True, g_alpha=True):
@@ -179,7 +189,7 @@ def full_parity(wl, backward=True, g_alpha=True):
     img_r, alpha_r, nb_r = oracle_reference(wl, A, ref, report)
     check_transmittance_drift(A, ref, report)
     report["fwd_max_err"] = check_image(A, img_r, alpha_r, "run A (dump)")
-    ref_grads = ref.backward(wl.g_img, wl.g_alpha if g_alpha else None) if backward else None
+    ref_grads = ref.backward(wl.g_img, wl.g_alpha if g_alpha else None) + (ref.blend_weights(),) if backward else None
     if backward:
         gA, report["grad_err_over_tol"] = check_backward(wl, A, ref_grads, g_alpha, "run A: ")
 

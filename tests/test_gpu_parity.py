@@ -218,6 +218,67 @@ def test_forward_is_repeatable_and_workspace_reusable():
         assert torch.equal(a, b)
 
 
+def _carve(nbytes, canary=0xA5, pad=1 << 16):
+    """A buffer of nbytes in the middle of a larger canary-filled allocation (256-byte aligned start)."""
+    whole = torch.full((nbytes + 2 * pad,), canary, dtype=torch.uint8, device="cuda")
+    return whole, whole[pad:pad + nbytes]
+
+
+def _intact(whole, nbytes, canary=0xA5, pad=1 << 16):
+    return bool((whole[:pad] == canary).all()) and bool((whole[pad + nbytes:] == canary).all())
+
+
+@pytest.mark.parametrize("name,kw", [("tiny", {}), ("tiny", {"D": 8}), ("stress", {"n_points": 1 << 18})])
+def test_guard_bands_around_every_buffer(name, kw):
+    """Stand-in for compute-sanitizer memcheck (closed on this pool, profiles/r02_sanitizer.md): nothing outside
+    the caller's buffers -- and nothing beyond inpc_raster_workspace_bytes -- is written."""
+    wl = make_workload(name, **kw)
+    N, D, W, H = wl.N, wl.D, wl.cam.width, wl.cam.height
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    pos, op, feat, g_img, g_alpha = t(wl.pos), t(wl.opacity), t(wl.feat), t(wl.g_img), t(wl.g_alpha)
+    for flags in (raster.SAVE_FOR_BACKWARD | raster.SAVE_SORTED, raster.SAVE_FOR_BACKWARD, 0):
+        sizes = dict(ws=raster.inpc_raster_workspace_bytes(N, D, W, H, flags), img=H * W * D * 4, alpha=H * W * 4,
+                     d_feat=N * D * 4, d_op=N * 4, d_uv=N * 8)
+        bufs = {k: _carve(v) for k, v in sizes.items()}
+        view = lambda k, shape: bufs[k][1].view(torch.float32).view(shape)
+        raster.inpc_raster_forward(pos, op, feat, wl.cam, out_feat=view("img", (H, W, D)), out_alpha=view("alpha", (H, W)),
+                                   workspace=bufs["ws"][1], flags=flags)
+        if flags & raster.SAVE_FOR_BACKWARD:
+            raster.inpc_raster_backward(pos, op, feat, wl.cam, g_img, g_alpha, bufs["ws"][1],
+                                        grad_feat=view("d_feat", (N, D)), grad_opacity=view("d_op", (N,)),
+                                        grad_uv=view("d_uv", (N, 2)))
+        torch.cuda.synchronize()
+        for k, (whole, _) in bufs.items():
+            assert _intact(whole, sizes[k]), f"{k}: bytes outside the buffer were written (flags {flags})"
+
+
+def test_results_do_not_depend_on_workspace_contents():
+    """Stand-in for compute-sanitizer initcheck: whatever the workspace held before the call, the results are
+    bit-identical (no read of memory the call itself has not written reaches a result)."""
+    wl = make_workload("stress", n_points=1 << 18)
+    N, D, W, H = wl.N, wl.D, wl.cam.width, wl.cam.height
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    pos, op, feat, g_img, g_alpha = t(wl.pos), t(wl.opacity), t(wl.feat), t(wl.g_img), t(wl.g_alpha)
+    nbytes = raster.inpc_raster_workspace_bytes(N, D, W, H, raster.SAVE_FOR_BACKWARD)
+    results = []
+    for fill in ("zero", "ff", "random"):
+        ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        if fill == "zero":
+            ws.zero_()
+        elif fill == "ff":
+            ws.fill_(0xFF)
+        else:
+            ws.copy_(torch.randint(0, 256, (nbytes,), dtype=torch.uint8, device="cuda"))
+        img, alpha, _ = raster.inpc_raster_forward(pos, op, feat, wl.cam, workspace=ws, flags=raster.SAVE_FOR_BACKWARD)
+        nb = raster.inpc_raster_get_blended_counts(ws, W, H)
+        grads = raster.inpc_raster_backward(pos, op, feat, wl.cam, g_img, g_alpha, ws)
+        torch.cuda.synchronize()
+        results.append((img, alpha, nb) + tuple(grads))
+    for other in results[1:]:
+        for a, b in zip(results[0], other):
+            assert torch.equal(a, b)
+
+
 def test_error_codes():
     wl = make_workload("tiny")
     st = gpu_forward(wl, flags=0)

@@ -255,6 +255,40 @@ def test_forced_blend_count_and_sorted_T():
     np.testing.assert_array_equal(d_op[20:], 0.0)
 
 
+def test_blend_weights_golden():
+    """NEXT row f1 (Eq. 3 input): hand-derived values of tests/golden/blend_weight.txt."""
+    gold = {}
+    for line in open(os.path.join(GOLDEN, "blend_weight.txt")):
+        if line.strip() and not line.startswith("#"):
+            c, i, v = line.split()
+            gold[(c, int(i))] = float(v)
+    p = [0.53125, -0.46875, 4.0]                                   # u = 40.5, v = 24.5: a pixel centre
+    n = 16
+    z = 4.0 + 0.25 * np.arange(n)                                  # depth order = index order
+    pos = np.stack([0.53125 / 4 * z, -0.46875 / 4 * z, z], 1)
+    r = _one(pos, [0.5] * n, [[1, 1, 1, 1]] * n)
+    r.blend()
+    bw = r.blend_weights()
+    for (c, i), v in gold.items():
+        if c == "A":
+            assert bw[i] == v, (i, bw[i], v)                       # powers of two: exact
+    np.testing.assert_array_equal(bw[:14], 0.5 ** (np.arange(14) + 1))
+    # case B: A on the centre of pixel (36, 28) at depth 3, B at (36.8, 28.8) depth 4
+    A = [(36.5 - 32) / 64 * 3.0, (28.5 - 32) / 64 * 3.0, 3.0]
+    B = [0.3, -0.2, 4.0]
+    r = _one([A, B], [0.8, 0.5], [[1, 1, 1, 1]] * 2)
+    r.blend()
+    bw = r.blend_weights()
+    # fp32 inputs: opacity 0.8f, and u = 36.8 carries an fp32 ulp of 3.8e-6 into tx = ty = 0.3
+    assert abs(bw[0] - gold[("B", 0)]) < 1e-7 and abs(bw[1] - gold[("B", 1)]) < 2e-6
+    # culled / zero-opacity points get exactly 0; a weight never exceeds the opacity
+    w = make_workload("tiny")
+    r = oracle.Raster.from_points(w.pos, w.opacity, w.feat, w.cam)
+    r.blend()
+    bw = r.blend_weights()
+    assert (bw >= 0).all() and (bw <= w.opacity.astype(np.float64) + 1e-15).all() and bw.max() > 0.3
+
+
 def test_general_stack_formula():
     rng = np.random.default_rng(5)
     n = 12
