@@ -41,7 +41,7 @@ if ROOT not in sys.path:
 FLAGS_STEP = 1      # INPC_SAVE_FOR_BACKWARD: the forward of the fwd+bwd step
 FLAGS_FWD = 0       # forward only (inference)
 
-METRIC = "fragments/sec (fwd+bwd step; ms/frame fwd and fwd+bwd beside it)"
+METRIC = "fragments/sec (fwd+bwd step, forward only for the inference config; ms/frame fwd and fwd+bwd beside it)"
 UNIT = "fragments/s"
 L2_BYTES = 126 * 1024 * 1024
 
@@ -167,12 +167,14 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # the oracle leg (cpu_baseline at N = 1, and --impl reference)
 def oracle_step(wl, n_sample: int) -> tuple[float, int]:
-    """One fwd+bwd of the oracle on the first n_sample points of the workload -> (seconds, fragments)."""
+    """One step (fwd+bwd; forward only for the inference config) of the oracle on the first n_sample points of the
+    workload -> (seconds, fragments)."""
     import oracle
     t0 = time.perf_counter()
     ref = oracle.Raster.from_points(wl.pos[:n_sample], wl.opacity[:n_sample], wl.feat[:n_sample], wl.cam)
     ref.blend()
-    ref.backward(wl.g_img, wl.g_alpha)
+    if wl.backward:
+        ref.backward(wl.g_img, wl.g_alpha)
     dt = time.perf_counter() - t0
     frags = ref.total
     del ref
@@ -244,7 +246,7 @@ def workload_config(wl, args, n_sets: int = 1) -> dict:
     return {"workload": f"{wl.name}: BASELINE.json config '{args.workload}', N={wl.N} points, "
                         f"{wl.cam.width}x{wl.cam.height}, D={wl.D}, seed {wl.seed}",
             "n_points": wl.N, "width": wl.cam.width, "height": wl.cam.height, "D": wl.D,
-            "pass": "forward + backward (grad_feat, grad_opacity, grad_uv)",
+            "pass": "forward + backward (grad_feat, grad_opacity, grad_uv)" if wl.backward else "forward only (feature image + alpha)",
             "parallelism": "replicas only (one cloud per GPU, no data-path collective)",
             "l2_hygiene": "inputs + records larger than L2 (see l2 key)" if n_sets == 1 else
                           f"working set fits L2: {n_sets} independent buffer sets rotated (see l2 key)"}
@@ -330,10 +332,17 @@ def ncu_traffic(workload: str) -> dict:
     return out
 
 
-def traffic_of_stage(traffic: dict, stage: str):
-    """Stage names carry no template arguments; the capture's kernel names do (k_blend<4, 1, 0>)."""
-    vals = [v for k, v in traffic.items() if not k.startswith("_") and k.split("<")[0] == stage]
-    return sum(vals) / len(vals) if vals else None
+def traffic_of_stage(traffic: dict, stage: str, D: int = 4, save: bool = True):
+    """Stage names carry no template arguments; the capture's kernel names do: k_blend<D, SAVE, DUMP>,
+    k_big<D, MODE> (0 forward, 2 backward), k_cellsort_big<D, THREADS, CHUNK> (two launches per stage: summed)."""
+    want = {"k_blend": f"k_blend<{D}, {1 if save else 0}, 0>", "k_big_fwd": f"k_big<{D}, 0>", "k_big_bwd": f"k_big<{D}, 2>"}
+    if stage in want:
+        return traffic.get(want[stage])
+    vals = [v for k, v in traffic.items() if not k.startswith("_") and k.split("<")[0] == stage
+            and ("<" not in k or k.split("<")[1].split(",")[0].strip(" >") == str(D))]
+    if not vals:
+        return None
+    return sum(vals) if stage == "k_cellsort_big" else sum(vals) / len(vals)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -418,9 +427,14 @@ def run_ours(args) -> int:
     def bwd():
         sets[turn[0] % n_sets][1]()
 
+    do_bwd = bool(wl.backward)          # BASELINE.json: the inference config is forward only
+
     def step():
-        fwd()
-        bwd()
+        if do_bwd:
+            fwd()
+            bwd()
+        else:
+            fwd(FLAGS_FWD)
         turn[0] += 1
 
     def fwd_only():
@@ -489,11 +503,13 @@ def run_ours(args) -> int:
     # ---- end to end: host buffers in, host buffers out, copies inside the timed region ----------------
     pos, op, feat, g_img, g_alpha = T["pos"], T["op"], T["feat"], T["g_img"], T["g_alpha"]
     img, alpha, d_feat, d_op, d_uv = T["img"], T["alpha"], T["d_feat"], T["d_op"], T["d_uv"]
-    flags = FLAGS_STEP
+    flags = FLAGS_STEP if do_bwd else FLAGS_FWD
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_in = [pin(wl.pos), pin(wl.opacity), pin(wl.feat), pin(wl.g_img), pin(wl.g_alpha)]
     d_in = [pos, op, feat, g_img, g_alpha]
     d_out = [img, alpha, d_feat, d_op, d_uv]
+    if not do_bwd:                                        # forward only: no output gradients in, no gradients out
+        h_in, d_in, d_out = h_in[:3], d_in[:3], d_out[:2]
     h_out = [torch.empty(t.shape, dtype=t.dtype).pin_memory() for t in d_out]
     h2d = sum(t.numel() * t.element_size() for t in h_in)
     d2h = sum(t.numel() * t.element_size() for t in h_out)
@@ -527,12 +543,15 @@ def run_ours(args) -> int:
             stream.wait_event(S["in_ready"])
             if i >= 2:
                 stream.wait_event(S["out_free"])         # step i-2's results have left the device
-            p_, o_, f_, gi_, ga_ = S["d_in"]
-            im_, al_, df_, dop_, du_ = S["d_out"]
+            p_, o_, f_ = S["d_in"][:3]
+            gi_, ga_ = S["d_in"][3:] if do_bwd else (None, None)
+            im_, al_ = S["d_out"][:2]
+            df_, dop_, du_ = S["d_out"][2:] if do_bwd else (None, None, None)
             raster.inpc_raster_forward(p_, o_, f_, cam, out_feat=im_, out_alpha=al_, workspace=S["ws"], flags=flags,
                                        stream=stream)
-            raster.inpc_raster_backward(p_, o_, f_, cam, gi_, ga_, S["ws"], grad_feat=df_, grad_opacity=dop_,
-                                        grad_uv=du_, stream=stream)
+            if do_bwd:
+                raster.inpc_raster_backward(p_, o_, f_, cam, gi_, ga_, S["ws"], grad_feat=df_, grad_opacity=dop_,
+                                            grad_uv=du_, stream=stream)
             S["done"].record(stream)
             s_out.wait_event(S["done"])
             with torch.cuda.stream(s_out):
@@ -547,8 +566,9 @@ def run_ours(args) -> int:
     def e2e_step():                                       # the same, one stream, nothing overlapped
         for h, d in zip(h_in, d_in):
             d.copy_(h, non_blocking=True)
-        fwd0()
-        bwd0()
+        fwd0(flags)
+        if do_bwd:
+            bwd0()
         for d, h in zip(d_out, h_out):
             h.copy_(d, non_blocking=True)
 
@@ -585,7 +605,7 @@ def run_ours(args) -> int:
         g_ms = sum(v for k, v in step_stage_ms.items() if STAGE_ROWS.get(k) == g)
         if g_ms <= 0:
             continue
-        tr = [traffic_of_stage(traffic, k) for k in step_stage_ms if STAGE_ROWS.get(k) == g and k.startswith("k_")]
+        tr = [traffic_of_stage(traffic, k, D, do_bwd) for k in step_stage_ms if STAGE_ROWS.get(k) == g and k.startswith("k_")]
         tr = [t for t in tr if t is not None]
         ach = alg[g] / (g_ms * 1e-3) / 1e9
         groups[g] = {"algorithmic_bytes": alg[g], "ms": g_ms, "achieved": ach, "frac": ach / peak,
@@ -599,17 +619,19 @@ def run_ours(args) -> int:
                 "algorithmic_bytes_per_launch": alg[rows], "ms_per_launch": per_stage[dom], "ms_rows": groups[rows]["ms"],
                 "kernels_of_rows": groups[rows]["kernels"],
                 "share_of_step": kernels[dom] / sum(step_stage_ms.values()),
-                "traffic": traffic_of_stage(traffic, dom), "traffic_source": traffic.get("_note"),
+                "traffic": traffic_of_stage(traffic, dom, D, do_bwd), "traffic_source": traffic.get("_note"),
                 "furthest_below_roof": {"rows": worst, "frac": groups[worst]["frac"], "ms": groups[worst]["ms"],
                                         "kernels": groups[worst]["kernels"]},
                 "note": "achieved = SURVEY 8d algorithmic bytes of the rows the dominant kernel implements / summed launch "
                         "time of the kernels implementing those rows (each timed alone); every group is in roofline_groups, "
                         "the whole step in roofline_step"}
-    ach_step = alg["fwd_bwd"] / (ms_step * 1e-3) / 1e9
+    step_key = "fwd_bwd" if do_bwd else "fwd"
+    ach_step = alg[step_key] / (ms_step * 1e-3) / 1e9
     ach_fwd = alg["fwd"] / (ms_fwd * 1e-3) / 1e9
-    roofline_step = {"bound": "hbm", "algorithmic_bytes_fwd_bwd": alg["fwd_bwd"], "achieved": ach_step,
+    roofline_step = {"bound": "hbm", "pass": "forward + backward" if do_bwd else "forward only",
+                     "algorithmic_bytes": alg[step_key], "achieved": ach_step,
                      "peak": peak, "unit": "GB/s", "frac": ach_step / peak, "frac_of_8TBps_nominal": ach_step / 8000.0,
-                     "target_ms_for_50pct_of_8TBps": alg["fwd_bwd"] / 4000.0 / 1e6,
+                     "target_ms_for_50pct_of_8TBps": alg[step_key] / 4000.0 / 1e6,
                      "fwd_only": {"algorithmic_bytes": alg["fwd"], "achieved": ach_fwd, "frac": ach_fwd / peak}}
 
     line = {

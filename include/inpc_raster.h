@@ -68,6 +68,9 @@ typedef enum inpc_status {
 /* flags of inpc_raster_forward / inpc_raster_workspace_bytes */
 #define INPC_SAVE_FOR_BACKWARD 1u  /* keep what inpc_raster_backward needs in the workspace                 */
 #define INPC_SAVE_SORTED       2u  /* also materialise every pixel's sorted fragment list (for get_sorted)  */
+/* flags of the _ex / _levels / _multisample entry points only (NEXT row f3 of the scope table) */
+#define INPC_OUT_PLANAR        4u  /* feature image (and its gradient) as [D][H][W] instead of [H][W][D]     */
+#define INPC_ACCUMULATE        8u  /* forward: out += out_scale * result (out holds an earlier call's image) */
 
 typedef struct inpc_stats {          /* host struct filled by inpc_raster_get_stats                          */
     uint64_t n_points;               /* N of the last forward                                                 */
@@ -100,6 +103,49 @@ int inpc_raster_backward(const float* pos, const float* opacity, const float* fe
                          const float* grad_out_feat, const float* grad_out_alpha,
                          float* grad_feat, float* grad_opacity, float* grad_uv,
                          void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- NEXT row f3: the paper's real call pattern -- several resolution levels per call, several point clouds
+ * averaged per pixel, [D][H][W] output (PAPER.md:100 "multisampling"; :126, :372 "multiple resolutions of feature
+ * maps ... multiple instances of our rasterization module for each resolution level"; :130 CNN input). ----------
+ *
+ * inpc_raster_forward_ex = inpc_raster_forward plus
+ *   flags INPC_OUT_PLANAR : out_feat is [D][H][W];
+ *   flags INPC_ACCUMULATE : out_feat / out_alpha already hold an image and the new one is ADDED to it;
+ *   out_scale             : factor on the image and on alpha (1/S for the average of S clouds).
+ *   With flags <= 3 and out_scale = 1 it is bit-identical to inpc_raster_forward.
+ * inpc_raster_backward_ex: grad_out_feat read as [D][H][W] with INPC_OUT_PLANAR, both output gradients multiplied
+ *   by grad_scale; blend_weight may be NULL. */
+int inpc_raster_forward_ex(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                           const inpc_camera* cam, float* out_feat, float* out_alpha,
+                           void* workspace, size_t workspace_bytes, uint32_t flags, float out_scale, void* cuda_stream);
+int inpc_raster_backward_ex(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                            const inpc_camera* cam,
+                            const float* grad_out_feat, const float* grad_out_alpha,
+                            float* grad_feat, float* grad_opacity, float* grad_uv, float* blend_weight,
+                            void* workspace, size_t workspace_bytes, uint32_t flags, float grad_scale, void* cuda_stream);
+
+/* Camera of resolution level l (host only, no device work): the image is halved l times,
+ *   width_l = ceil(width / 2^l), height_l = ceil(height / 2^l), fx, fy, cx, cy multiplied by 2^-l (exact in fp32),
+ * so a point that projects to (u, v) at level 0 projects to (u, v) / 2^l: pixel centres stay at (i+0.5, j+0.5). */
+int inpc_raster_level_camera(const inpc_camera* cam, int32_t level, inpc_camera* out);
+
+/* One point cloud rasterised at n_levels (<= 8) resolution levels: level l uses inpc_raster_level_camera(cam, l),
+ * out_feat[l] / out_alpha[l] / workspaces[l] / workspace_bytes[l] are HOST arrays of n_levels device pointers /
+ * sizes (workspace l sized for the level-l image; each keeps its own state for a later backward with that level's
+ * camera).  flags / out_scale as for inpc_raster_forward_ex. */
+int inpc_raster_forward_levels(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                               const inpc_camera* cam, int32_t n_levels, float* const* out_feat, float* const* out_alpha,
+                               void* const* workspaces, const size_t* workspace_bytes, uint32_t flags, float out_scale,
+                               void* cuda_stream);
+
+/* Inference multisampling: n_clouds (<= 64) independently sampled point clouds (HOST arrays of device pointers and
+ * of point counts) are each rasterised at n_levels levels and averaged per pixel, out[l] = (1/S) sum_s image_s[l],
+ * in cloud order (so the result is bit-reproducible).  Forward only: ONE workspace, sized for the largest cloud at
+ * level 0, is reused; flags may only hold INPC_OUT_PLANAR. */
+int inpc_raster_forward_multisample(int32_t n_clouds, const float* const* pos, const float* const* opacity,
+                                    const float* const* feat, const int64_t* N, int32_t D, const inpc_camera* cam,
+                                    int32_t n_levels, float* const* out_feat, float* const* out_alpha, void* workspace,
+                                    size_t workspace_bytes, uint32_t flags, void* cuda_stream);
 
 /* The same backward pass with the per-point BLENDING WEIGHT fused in (NEXT row f1 of the scope table):
  *   blend_weight[N] = max over the point's blended fragments of alpha_c T_c, alpha_c = opacity w_c (Eq. 7) and

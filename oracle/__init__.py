@@ -206,3 +206,51 @@ def fp64_projection_changes(pos, cam) -> int:
     pos = np.ascontiguousarray(pos, dtype=np.float32).reshape(-1, 3)
     cs = _cam_struct(cam)
     return int(lib.oracle_count_fp64_projection_changes(_p(pos), pos.shape[0], C.byref(cs)))
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT row f3 -- the paper's call pattern, as plain compositions of the oracle above (test infrastructure):
+# several resolution levels of one cloud, the per-pixel average of several clouds
+# ("multisampling"), and the [D,H,W] layout the CNN reads.
+
+class _LevelCamera:
+    pass
+
+
+def level_camera(cam, level: int):
+    """Camera of resolution level l: the image halved l times.  width_l = ceil(width / 2^l), likewise height;
+    fx, fy, cx, cy times 2^-l (a power of two: exact in fp32), so (u, v) becomes (u, v) / 2^l and pixel centres stay
+    at (i + 0.5, j + 0.5).  Reading: the paper only says "progressively lower resolution"; halving
+    matches the 2x average pooling between the U-Net's levels."""
+    c = _LevelCamera()
+    s = np.float32(1.0) / np.float32(2 ** level)
+    c.fx, c.fy = np.float32(cam.fx) * s, np.float32(cam.fy) * s
+    c.cx, c.cy = np.float32(cam.cx) * s, np.float32(cam.cy) * s
+    c.R, c.t, c.near_z, c.far_z = cam.R, cam.t, cam.near_z, cam.far_z
+    c.width = -(-int(cam.width) // 2 ** level)
+    c.height = -(-int(cam.height) // 2 ** level)
+    return c
+
+
+def rasterize_levels(pos, opacity, feat, cam, n_levels: int):
+    """-> [Raster of level 0, ..., Raster of level n_levels - 1]."""
+    return [Raster.from_points(pos, opacity, feat, level_camera(cam, l)) for l in range(n_levels)]
+
+
+def multisample(clouds, cam, n_levels: int = 1):
+    """clouds: list of (pos, opacity, feat).  -> per level (img[H,W,D], alpha[H,W]): the plain per-pixel mean of the
+    clouds' images (PAPER.md:100: "rasterize multiple point clouds ... and average the results")."""
+    out = []
+    for l in range(n_levels):
+        cl = level_camera(cam, l)
+        imgs, alphas = [], []
+        for pos, op, feat in clouds:
+            img, alpha, _, _ = Raster.from_points(pos, op, feat, cl).blend()
+            imgs.append(img); alphas.append(alpha)
+        out.append((np.mean(imgs, axis=0), np.mean(alphas, axis=0)))
+    return out
+
+
+def to_planar(img):
+    """[H,W,D] -> [D,H,W]."""
+    return np.ascontiguousarray(np.transpose(img, (2, 0, 1)))

@@ -32,6 +32,7 @@ struct BackArgs {
     const uint4* pcur;
     const float* g_feat;
     const float* g_alpha;
+    ImageIO io;
     float* gD;
 };
 
@@ -174,13 +175,8 @@ __global__ void __launch_bounds__(kTileThreads) k_back(BackArgs A) {
         // global float index of (slot, corner) = (cursor >> 2) + 4 * (slot - smem record)
         float* gDtop = A.gD + 4 * ((ptrdiff_t)(int32_t)(0u - bt));
         float* gDbot = A.gD + 4 * ((ptrdiff_t)(int32_t)(0u - bb));
-        float g[D];
-#pragma unroll
-        for (int v = 0; v < FV; ++v) {
-            const float4 t = __ldg(reinterpret_cast<const float4*>(A.g_feat + pix * D) + v);
-            g[4 * v] = t.x; g[4 * v + 1] = t.y; g[4 * v + 2] = t.z; g[4 * v + 3] = t.w;
-        }
-        const float gA = A.g_alpha ? __ldg(A.g_alpha + pix) : 0.f;
+        float g[D], gA;
+        load_pixel_grad<D>(A.io, A.g_feat, A.g_alpha, pix, g, gA);
 
         float B = 0.f;
         float pa = 0.f, pT = 0.f;                         // pending fragment: alpha, transmittance, features, gD address

@@ -32,6 +32,7 @@ struct BigArgs {
     const float* g_feat;
     const float* g_alpha;
     float* gD;
+    ImageIO io;
 };
 
 template <int D, int MODE>
@@ -52,21 +53,13 @@ __global__ void __launch_bounds__(kLongThreads) k_big(BigArgs A) {
             const uint32_t obase = (MODE == kFwdDump) ? A.pixoff[pix] : 0u;
             blend_pixel<D, MODE == kFwdDump, double>(A.dk, A.Ra, A.Rf, L, 0u, 0u, A.gT, acc, accA, consumed, A.sorted_idx,
                                                      A.sorted_depth, A.sorted_T, obase);
-#pragma unroll
-            for (int v = 0; v < D / 4; ++v)
-                reinterpret_cast<float4*>(A.out_feat + (size_t)pix * D)[v] = make_float4(acc[4 * v], acc[4 * v + 1], acc[4 * v + 2], acc[4 * v + 3]);
-            A.out_alpha[pix] = accA;
+            store_pixel<D>(A.io, A.out_feat, A.out_alpha, (size_t)pix, acc, accA);
             if (A.gT) A.pcur[pix] = consumed;
         } else {
             const uint4 consumed = A.pcur[pix];
             L.e0 = L.c0 + consumed.x; L.e1 = L.c1 + consumed.y; L.e2 = L.c2 + consumed.z; L.e3 = L.c3 + consumed.w;
-            float g[D];
-#pragma unroll
-            for (int v = 0; v < D / 4; ++v) {
-                const float4 t = __ldg(reinterpret_cast<const float4*>(A.g_feat + (size_t)pix * D) + v);
-                g[4 * v] = t.x; g[4 * v + 1] = t.y; g[4 * v + 2] = t.z; g[4 * v + 3] = t.w;
-            }
-            const float gA = A.g_alpha ? __ldg(A.g_alpha + pix) : 0.f;
+            float g[D], gA;
+            load_pixel_grad<D>(A.io, A.g_feat, A.g_alpha, (size_t)pix, g, gA);
             backward_pixel<D, double>(A.dk, A.Ra, A.Rf, A.gT, L, 0u, 0u, g, gA, A.gD);
         }
     }

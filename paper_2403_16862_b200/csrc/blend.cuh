@@ -32,6 +32,7 @@ struct BlendArgs {
     int W, H;
     float* out_feat;
     float* out_alpha;
+    ImageIO io;
     float* gT;               // NULL unless INPC_SAVE_FOR_BACKWARD
     uint4* pcur;
     // dump (INPC_SAVE_SORTED)
@@ -317,10 +318,7 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
             }
         }
 #undef INPC_PICK
-#pragma unroll
-        for (int v = 0; v < FV; ++v)
-            reinterpret_cast<float4*>(A.out_feat + pix * D)[v] = make_float4(acc[4 * v], acc[4 * v + 1], acc[4 * v + 2], acc[4 * v + 3]);
-        A.out_alpha[pix] = accA;
+        store_pixel<D>(A.io, A.out_feat, A.out_alpha, pix, acc, accA);
         if constexpr (SAVE) A.pcur[pix] = consumed;
     }
 }

@@ -167,6 +167,56 @@ __device__ __forceinline__ Proj project_point(const Camera& c, float x, float y,
     return p;
 }
 
+// ---- how a feature image (forward) or its gradient (backward) is laid out and combined (NEXT row f3) ------------
+// planar 0: [H][W][D] pixel-interleaved (one 16-byte store per pixel and four channels); 1: [D][H][W], what a CNN
+// wants.  Forward: out = (accumulate ? out : 0) + scale * result -- the per-pixel average of several
+// point clouds ("multisampling") is S calls with scale 1/S.  Backward: grad_out is read through the same
+// layout and multiplied by scale.  scale = 1 and accumulate = 0 reproduce the plain result bit for bit.
+struct ImageIO {
+    int planar, accumulate;
+    float scale;
+    uint32_t P;                // W * H
+};
+template <int D>
+__device__ __forceinline__ void store_pixel(const ImageIO& io, float* __restrict__ out_feat, float* __restrict__ out_alpha,
+                                            size_t pix, const float (&acc)[D], float accA) {
+    if (!io.planar) {
+        float4* o = reinterpret_cast<float4*>(out_feat + pix * D);
+#pragma unroll
+        for (int v = 0; v < D / 4; ++v) {
+            float4 r = make_float4(io.scale * acc[4 * v], io.scale * acc[4 * v + 1], io.scale * acc[4 * v + 2], io.scale * acc[4 * v + 3]);
+            if (io.accumulate) { const float4 b = o[v]; r.x += b.x; r.y += b.y; r.z += b.z; r.w += b.w; }
+            o[v] = r;
+        }
+    } else {
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+            float* o = out_feat + (size_t)d * io.P + pix;
+            float r = io.scale * acc[d];
+            if (io.accumulate) r += *o;
+            *o = r;
+        }
+    }
+    float a = io.scale * accA;
+    if (io.accumulate) a += out_alpha[pix];
+    out_alpha[pix] = a;
+}
+template <int D>
+__device__ __forceinline__ void load_pixel_grad(const ImageIO& io, const float* __restrict__ g_feat,
+                                                const float* __restrict__ g_alpha, size_t pix, float (&g)[D], float& gA) {
+    if (!io.planar) {
+#pragma unroll
+        for (int v = 0; v < D / 4; ++v) {
+            const float4 t = __ldg(reinterpret_cast<const float4*>(g_feat + pix * D) + v);
+            g[4 * v] = io.scale * t.x; g[4 * v + 1] = io.scale * t.y; g[4 * v + 2] = io.scale * t.z; g[4 * v + 3] = io.scale * t.w;
+        }
+    } else {
+#pragma unroll
+        for (int d = 0; d < D; ++d) g[d] = io.scale * __ldg(g_feat + (size_t)d * io.P + pix);
+    }
+    gA = g_alpha ? io.scale * __ldg(g_alpha + pix) : 0.f;
+}
+
 // Work-item encoding for the tile kernel: X (12 bits) | Y (12) | log2 tw (3) | log2 th (2)
 __host__ __device__ __forceinline__ uint32_t encode_item(int X, int Y, int lw, int lh) {
     return (uint32_t)X | ((uint32_t)Y << 12) | ((uint32_t)lw << 24) | ((uint32_t)lh << 27);

@@ -31,7 +31,8 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                                                            int H, const float4* __restrict__ Ra,
                                                            const float4* __restrict__ gT, const float4* __restrict__ gD,
                                                            const uint4* __restrict__ pcur,
-                                                           const float* __restrict__ g_feat, float* __restrict__ gpt) {
+                                                           const float* __restrict__ g_feat, ImageIO io,
+                                                           float* __restrict__ gpt) {
     constexpr int GP = gpt_floats<D>();
     __shared__ uint32_t s_off[kGradCells + 1];
     const int tid = threadIdx.x;
@@ -58,7 +59,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
             const int x0 = i - 1, y0 = j - 1;
             // every gather of the four corner pixels is issued before any of them is used
             uint4 cur[4];
-            float4 gp[4][D / 4];
+            float gp[4][D];
             bool in[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -66,9 +67,12 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                 in[c] = px >= 0 && px < W && py >= 0 && py < H;               // else: fragment does not exist
                 const size_t pp = in[c] ? (size_t)py * W + px : 0;
                 cur[c] = in[c] ? __ldg(&pcur[pp]) : make_uint4(0, 0, 0, 0);
+                float unused;
+                if (in[c]) load_pixel_grad<D>(io, g_feat, nullptr, pp, gp[c], unused);
+                else {
 #pragma unroll
-                for (int v = 0; v < D / 4; ++v)
-                    gp[c][v] = in[c] ? __ldg(reinterpret_cast<const float4*>(g_feat + pp * D) + v) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int d = 0; d < D; ++d) gp[c][d] = 0.f;
+                }
             }
             const float tc[4] = {t4.x, t4.y, t4.z, t4.w}, dc[4] = {d4.x, d4.y, d4.z, d4.w};
             float df[D];
@@ -88,10 +92,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                 du += (dx ? wy : -wy) * dl;
                 dv += (dy ? wx : -wx) * dl;
 #pragma unroll
-                for (int v = 0; v < D / 4; ++v) {
-                    const float4 t = gp[c][v];
-                    df[4 * v] += Ta * t.x; df[4 * v + 1] += Ta * t.y; df[4 * v + 2] += Ta * t.z; df[4 * v + 3] += Ta * t.w;
-                }
+                for (int d = 0; d < D; ++d) df[d] += Ta * gp[c][d];
             }
             du *= r0.z; dv *= r0.z;
             float4* out = reinterpret_cast<float4*>(gpt + (size_t)__float_as_uint(r0.w) * GP);

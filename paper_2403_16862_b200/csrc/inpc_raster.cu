@@ -330,10 +330,13 @@ static Side* side_for(const DeviceInfo& di) {
 template <int D>
 static int forward_impl(const float* pos, const float* opacity, const float* feat, int64_t N, const inpc_camera* cam,
                         float* out_feat, float* out_alpha, unsigned char* ws, const Layout& L, uint32_t flags,
-                        cudaStream_t st) {
+                        float out_scale, cudaStream_t st) {
     const DeviceInfo di = device_info();
     if (!di.ok) return cuda_fail(cudaErrorNoDevice);
     const Camera camk = to_camera(cam);
+    ImageIO io{};
+    io.planar = (flags & INPC_OUT_PLANAR) ? 1 : 0; io.accumulate = (flags & INPC_ACCUMULATE) ? 1 : 0;
+    io.scale = out_scale; io.P = L.P;
     const int W = cam->width, H = cam->height;
     Header* hdr = reinterpret_cast<Header*>(ws + L.header);
     uint32_t* cellcnt = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
@@ -413,10 +416,10 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
 
     BlendArgs A{};
     A.hdr = hdr; A.celloff = cellcnt; A.dk = dk; A.Ra = Ra; A.Rf = Rf;
-    A.W = W; A.H = H; A.out_feat = out_feat; A.out_alpha = out_alpha;
+    A.W = W; A.H = H; A.out_feat = out_feat; A.out_alpha = out_alpha; A.io = io;
     BigArgs Bg{};
     Bg.hdr = hdr; Bg.bigpix = bigpix; Bg.celloff = cellcnt; Bg.dk = dk; Bg.Ra = Ra; Bg.Rf = Rf;
-    Bg.W = W; Bg.H = H; Bg.out_feat = out_feat; Bg.out_alpha = out_alpha;
+    Bg.W = W; Bg.H = H; Bg.out_feat = out_feat; Bg.out_alpha = out_alpha; Bg.io = io;
     if (save) {
         A.gT = Bg.gT = reinterpret_cast<float*>(ws + L.gT);
         A.pcur = Bg.pcur = reinterpret_cast<uint4*>(ws + L.pcur);
@@ -452,10 +455,12 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
 template <int D>
 static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat, const float* g_alpha, float* d_feat,
                          float* d_opacity, float* d_uv, float* blend_weight, unsigned char* ws, const Layout& L,
-                         cudaStream_t st) {
+                         uint32_t flags, float grad_scale, cudaStream_t st) {
     const DeviceInfo di = device_info();
     if (!di.ok) return cuda_fail(cudaErrorNoDevice);
     const int W = cam->width, H = cam->height;
+    ImageIO io{};
+    io.planar = (flags & INPC_OUT_PLANAR) ? 1 : 0; io.accumulate = 0; io.scale = grad_scale; io.P = L.P;
     Header* hdr = reinterpret_cast<Header*>(ws + L.header);
     { StageTimer tm(kStZeroBwd, st);
       k_check_backward<<<1, 1, 0, st>>>(hdr, W, H, D, (uint32_t)N); }
@@ -484,12 +489,12 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     BigArgs Bg{};
     Bg.hdr = hdr; Bg.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); Bg.celloff = celloff;
     Bg.dk = reinterpret_cast<uint32_t*>(ws + L.dk); Bg.Ra = Ra; Bg.Rf = Rf;
-    Bg.W = W; Bg.H = H; Bg.gT = gT; Bg.pcur = pcur; Bg.g_feat = g_feat; Bg.g_alpha = g_alpha; Bg.gD = gD;
+    Bg.W = W; Bg.H = H; Bg.gT = gT; Bg.pcur = pcur; Bg.g_feat = g_feat; Bg.g_alpha = g_alpha; Bg.gD = gD; Bg.io = io;
     int rc = launch_big<D, kBwd>(Bg, di.sms, st);
     if (rc != INPC_OK) return rc;
     BackArgs A{};
     A.hdr = hdr; A.celloff = celloff; A.dk = Bg.dk; A.Ra = Ra; A.Rf = Rf;
-    A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD;
+    A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD; A.io = io;
     const Bands Bf = make_bands(W, H, L.C, kDefaultBands);     // the plan the forward built the item lists with
     uint32_t u0 = 0;
     for (int b = 0; b < Bf.plan.n_bands; ++b) {
@@ -502,7 +507,7 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
             { StageTimer tm(kStCombine, s2);
               k_combine<D><<<(int)std::min<uint32_t>(u1 - u0, (uint32_t)di.sms * 8), kGradThreads, 0, s2>>>(
                   hdr, celloff, L.C, u0, u1, W, H, Ra, reinterpret_cast<const float4*>(gT),
-                  reinterpret_cast<const float4*>(gD), pcur, g_feat, gpt); }
+                  reinterpret_cast<const float4*>(gD), pcur, g_feat, io, gpt); }
             INPC_LAUNCHED(kname<D>("k_combine"));
             u0 = u1;
         }
@@ -526,13 +531,14 @@ size_t inpc_raster_workspace_bytes(int64_t n_points, int32_t D, int32_t W, int32
     return make_layout(n_points, D, W, H, flags).total;
 }
 
-int inpc_raster_forward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
-                        const inpc_camera* cam, float* out_feat, float* out_alpha, void* workspace,
-                        size_t workspace_bytes, uint32_t flags, void* cuda_stream) {
+static int forward_entry(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                         const inpc_camera* cam, float* out_feat, float* out_alpha, void* workspace,
+                         size_t workspace_bytes, uint32_t flags, float out_scale, void* cuda_stream) {
     int rc = check_common(N, D, cam);
     if (rc != INPC_OK) return rc;
     if (!out_feat || !out_alpha || !workspace) return INPC_ERR_INVALID_ARG;
     if (N > 0 && (!pos || !opacity || !feat)) return INPC_ERR_INVALID_ARG;
+    if (flags & ~(INPC_SAVE_FOR_BACKWARD | INPC_SAVE_SORTED | INPC_OUT_PLANAR | INPC_ACCUMULATE)) return INPC_ERR_INVALID_ARG;
     if (!aligned16(pos) || !aligned16(opacity) || !aligned16(feat) || !aligned16(out_feat) || !aligned16(out_alpha) ||
         (reinterpret_cast<uintptr_t>(workspace) & 255u))
         return INPC_ERR_INVALID_ARG;
@@ -540,17 +546,80 @@ int inpc_raster_forward(const float* pos, const float* opacity, const float* fea
     if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     unsigned char* ws = static_cast<unsigned char*>(workspace);
-    return D == 4 ? forward_impl<4>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st)
-                  : forward_impl<8>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, st);
+    return D == 4 ? forward_impl<4>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, out_scale, st)
+                  : forward_impl<8>(pos, opacity, feat, N, cam, out_feat, out_alpha, ws, L, flags, out_scale, st);
+}
+
+int inpc_raster_forward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                        const inpc_camera* cam, float* out_feat, float* out_alpha, void* workspace,
+                        size_t workspace_bytes, uint32_t flags, void* cuda_stream) {
+    if (flags & ~(INPC_SAVE_FOR_BACKWARD | INPC_SAVE_SORTED)) return INPC_ERR_INVALID_ARG;   // layout flags: _ex
+    return forward_entry(pos, opacity, feat, N, D, cam, out_feat, out_alpha, workspace, workspace_bytes, flags, 1.0f,
+                         cuda_stream);
+}
+
+int inpc_raster_forward_ex(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                           const inpc_camera* cam, float* out_feat, float* out_alpha, void* workspace,
+                           size_t workspace_bytes, uint32_t flags, float out_scale, void* cuda_stream) {
+    return forward_entry(pos, opacity, feat, N, D, cam, out_feat, out_alpha, workspace, workspace_bytes, flags, out_scale,
+                         cuda_stream);
+}
+
+int inpc_raster_level_camera(const inpc_camera* cam, int32_t level, inpc_camera* out) {
+    if (!cam || !out || level < 0 || level > 8) return INPC_ERR_INVALID_ARG;
+    *out = *cam;
+    const float s = 1.0f / (float)(1 << level);              // a power of two: every product below is exact
+    out->fx = cam->fx * s; out->fy = cam->fy * s; out->cx = cam->cx * s; out->cy = cam->cy * s;
+    out->width = (cam->width + (1 << level) - 1) >> level;
+    out->height = (cam->height + (1 << level) - 1) >> level;
+    return INPC_OK;
+}
+
+int inpc_raster_forward_levels(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                               const inpc_camera* cam, int32_t n_levels, float* const* out_feat, float* const* out_alpha,
+                               void* const* workspaces, const size_t* workspace_bytes, uint32_t flags, float out_scale,
+                               void* cuda_stream) {
+    if (n_levels < 1 || n_levels > 8 || !out_feat || !out_alpha || !workspaces || !workspace_bytes) return INPC_ERR_INVALID_ARG;
+    for (int32_t l = 0; l < n_levels; ++l) {
+        inpc_camera c;
+        int rc = inpc_raster_level_camera(cam, l, &c);
+        if (rc == INPC_OK)
+            rc = forward_entry(pos, opacity, feat, N, D, &c, out_feat[l], out_alpha[l], workspaces[l], workspace_bytes[l],
+                               flags, out_scale, cuda_stream);
+        if (rc != INPC_OK) return rc;
+    }
+    return INPC_OK;
+}
+
+int inpc_raster_forward_multisample(int32_t n_clouds, const float* const* pos, const float* const* opacity,
+                                    const float* const* feat, const int64_t* N, int32_t D, const inpc_camera* cam,
+                                    int32_t n_levels, float* const* out_feat, float* const* out_alpha, void* workspace,
+                                    size_t workspace_bytes, uint32_t flags, void* cuda_stream) {
+    if (n_clouds < 1 || n_clouds > 64 || !pos || !opacity || !feat || !N) return INPC_ERR_INVALID_ARG;
+    if (n_levels < 1 || n_levels > 8 || !out_feat || !out_alpha) return INPC_ERR_INVALID_ARG;
+    if (flags & ~INPC_OUT_PLANAR) return INPC_ERR_INVALID_ARG;     // inference path: one workspace, nothing is saved
+    const float scale = 1.0f / (float)n_clouds;
+    for (int32_t s = 0; s < n_clouds; ++s)
+        for (int32_t l = 0; l < n_levels; ++l) {
+            inpc_camera c;
+            int rc = inpc_raster_level_camera(cam, l, &c);
+            if (rc == INPC_OK)
+                rc = forward_entry(pos[s], opacity[s], feat[s], N[s], D, &c, out_feat[l], out_alpha[l], workspace,
+                                   workspace_bytes, flags | (s > 0 ? INPC_ACCUMULATE : 0u), scale, cuda_stream);
+            if (rc != INPC_OK) return rc;
+        }
+    return INPC_OK;
 }
 
 static int backward_entry(int64_t N, int32_t D, const inpc_camera* cam, const float* grad_out_feat,
                           const float* grad_out_alpha, float* grad_feat, float* grad_opacity, float* grad_uv,
-                          float* blend_weight, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+                          float* blend_weight, void* workspace, size_t workspace_bytes, uint32_t flags, float grad_scale,
+                          void* cuda_stream) {
     int rc = check_common(N, D, cam);
     if (rc != INPC_OK) return rc;
     if (!grad_out_feat || !workspace) return INPC_ERR_INVALID_ARG;
     if (N > 0 && (!grad_feat || !grad_opacity || !grad_uv)) return INPC_ERR_INVALID_ARG;
+    if (flags & ~INPC_OUT_PLANAR) return INPC_ERR_INVALID_ARG;
     if (!aligned16(grad_out_feat) || !aligned16(grad_out_alpha) || !aligned16(grad_feat) || !aligned16(grad_opacity) ||
         !aligned16(grad_uv) || !aligned16(blend_weight) || (reinterpret_cast<uintptr_t>(workspace) & 255u))
         return INPC_ERR_INVALID_ARG;
@@ -561,8 +630,8 @@ static int backward_entry(int64_t N, int32_t D, const inpc_camera* cam, const fl
     if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     unsigned char* ws = static_cast<unsigned char*>(workspace);
-    return D == 4 ? backward_impl<4>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight, ws, L, st)
-                  : backward_impl<8>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight, ws, L, st);
+    return D == 4 ? backward_impl<4>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight, ws, L, flags, grad_scale, st)
+                  : backward_impl<8>(N, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight, ws, L, flags, grad_scale, st);
 }
 
 int inpc_raster_backward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
@@ -571,7 +640,7 @@ int inpc_raster_backward(const float* pos, const float* opacity, const float* fe
                          size_t workspace_bytes, void* cuda_stream) {
     (void)pos; (void)opacity; (void)feat;   // the records saved by the forward hold what the backward needs
     return backward_entry(N, D, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, nullptr, workspace,
-                          workspace_bytes, cuda_stream);
+                          workspace_bytes, 0u, 1.0f, cuda_stream);
 }
 
 int inpc_raster_backward_weights(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
@@ -581,7 +650,16 @@ int inpc_raster_backward_weights(const float* pos, const float* opacity, const f
     (void)pos; (void)opacity; (void)feat;
     if (N > 0 && !blend_weight) return INPC_ERR_INVALID_ARG;
     return backward_entry(N, D, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight,
-                          workspace, workspace_bytes, cuda_stream);
+                          workspace, workspace_bytes, 0u, 1.0f, cuda_stream);
+}
+
+int inpc_raster_backward_ex(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
+                            const inpc_camera* cam, const float* grad_out_feat, const float* grad_out_alpha,
+                            float* grad_feat, float* grad_opacity, float* grad_uv, float* blend_weight,
+                            void* workspace, size_t workspace_bytes, uint32_t flags, float grad_scale, void* cuda_stream) {
+    (void)pos; (void)opacity; (void)feat;
+    return backward_entry(N, D, cam, grad_out_feat, grad_out_alpha, grad_feat, grad_opacity, grad_uv, blend_weight,
+                          workspace, workspace_bytes, flags, grad_scale, cuda_stream);
 }
 
 // The introspection calls synchronise: they read the workspace's Header back and take shape, D and flags from it.

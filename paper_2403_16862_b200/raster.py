@@ -16,9 +16,13 @@ LIB_PATH = os.path.join(_HERE, "libinpc_raster.so")
 
 SAVE_FOR_BACKWARD = 1
 SAVE_SORTED = 2
+OUT_PLANAR = 4          # _ex / _levels / _multisample entry points: feature image as [D][H][W]
+ACCUMULATE = 8          # _ex: add to the image already in the output buffers
 
 EXPORTS = (
     "inpc_raster_workspace_bytes", "inpc_raster_forward", "inpc_raster_backward", "inpc_raster_backward_weights",
+    "inpc_raster_forward_ex", "inpc_raster_backward_ex", "inpc_raster_level_camera", "inpc_raster_forward_levels",
+    "inpc_raster_forward_multisample",
     "inpc_raster_get_counts", "inpc_raster_get_blended_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
     "inpc_raster_get_status",
     "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count", "inpc_raster_launched_kernels",
@@ -67,6 +71,18 @@ def load() -> C.CDLL:
         lib.inpc_raster_forward.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, C.c_size_t, u32, vp]
         lib.inpc_raster_backward.restype = C.c_int
         lib.inpc_raster_backward.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        lib.inpc_raster_forward_ex.restype = C.c_int
+        lib.inpc_raster_forward_ex.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, C.c_size_t, u32, C.c_float, vp]
+        lib.inpc_raster_backward_ex.restype = C.c_int
+        lib.inpc_raster_backward_ex.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, vp, C.c_size_t, u32, C.c_float, vp]
+        lib.inpc_raster_level_camera.restype = C.c_int
+        lib.inpc_raster_level_camera.argtypes = [C.POINTER(InpcCamera), i32, C.POINTER(InpcCamera)]
+        lib.inpc_raster_forward_levels.restype = C.c_int
+        lib.inpc_raster_forward_levels.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), i32, C.POINTER(vp), C.POINTER(vp),
+                                                   C.POINTER(vp), C.POINTER(C.c_size_t), u32, C.c_float, vp]
+        lib.inpc_raster_forward_multisample.restype = C.c_int
+        lib.inpc_raster_forward_multisample.argtypes = [i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64), i32,
+                                                        C.POINTER(InpcCamera), i32, C.POINTER(vp), C.POINTER(vp), vp, C.c_size_t, u32, vp]
         lib.inpc_raster_backward_weights.restype = C.c_int
         lib.inpc_raster_backward_weights.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
         lib.inpc_raster_get_counts.restype = C.c_int
@@ -133,29 +149,94 @@ def alloc_workspace(N: int, D: int, W: int, H: int, flags: int = SAVE_FOR_BACKWA
     return torch.empty(nbytes, dtype=torch.uint8, device=device)
 
 
+def _img_shape(H, W, D, flags):
+    return (D, H, W) if flags & OUT_PLANAR else (H, W, D)
+
+
+def inpc_raster_level_camera(cam, level: int) -> InpcCamera:
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    out = InpcCamera()
+    rc = load().inpc_raster_level_camera(C.byref(cs), level, C.byref(out))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_level_camera")
+    return out
+
+
+def _ptr_array(tensors):
+    return (C.c_void_p * len(tensors))(*[t.data_ptr() for t in tensors])
+
+
+def inpc_raster_forward_levels(pos, opacity, feat, cam, n_levels: int, flags: int = SAVE_FOR_BACKWARD, out_scale: float = 1.0,
+                               stream=None):
+    """One cloud at n_levels resolution levels -> (list of out_feat, list of out_alpha, list of workspaces, list of
+    level cameras)."""
+    lib = load()
+    _check(pos, torch.float32, "pos"); _check(opacity, torch.float32, "opacity"); _check(feat, torch.float32, "feat")
+    N, D = int(pos.shape[0]), int(feat.shape[1])
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    cams = [inpc_raster_level_camera(cs, l) for l in range(n_levels)]
+    dev = pos.device
+    imgs = [torch.empty(_img_shape(c.height, c.width, D, flags), dtype=torch.float32, device=dev) for c in cams]
+    alphas = [torch.empty((c.height, c.width), dtype=torch.float32, device=dev) for c in cams]
+    wss = [alloc_workspace(N, D, c.width, c.height, flags & 3, dev) for c in cams]
+    sizes = (C.c_size_t * n_levels)(*[w.numel() for w in wss])
+    rc = lib.inpc_raster_forward_levels(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), n_levels, _ptr_array(imgs),
+                                        _ptr_array(alphas), _ptr_array(wss), sizes, flags, out_scale, _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_forward_levels")
+    return imgs, alphas, wss, cams
+
+
+def inpc_raster_forward_multisample(clouds, cam, n_levels: int = 1, flags: int = 0, stream=None):
+    """clouds: list of (pos, opacity, feat) device tensors.  -> (list of averaged out_feat per level, list of alpha)."""
+    lib = load()
+    D = int(clouds[0][2].shape[1])
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    cams = [inpc_raster_level_camera(cs, l) for l in range(n_levels)]
+    dev = clouds[0][0].device
+    imgs = [torch.empty(_img_shape(c.height, c.width, D, flags), dtype=torch.float32, device=dev) for c in cams]
+    alphas = [torch.empty((c.height, c.width), dtype=torch.float32, device=dev) for c in cams]
+    Ns = [int(c[0].shape[0]) for c in clouds]
+    ws = alloc_workspace(max(Ns), D, cs.width, cs.height, 0, dev)
+    S = len(clouds)
+    rc = lib.inpc_raster_forward_multisample(S, _ptr_array([c[0] for c in clouds]), _ptr_array([c[1] for c in clouds]),
+                                             _ptr_array([c[2] for c in clouds]), (C.c_int64 * S)(*Ns), D, C.byref(cs),
+                                             n_levels, _ptr_array(imgs), _ptr_array(alphas), _ptr(ws), ws.numel(), flags,
+                                             _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_forward_multisample")
+    return imgs, alphas
+
+
 def inpc_raster_forward(pos, opacity, feat, cam, out_feat=None, out_alpha=None, workspace=None,
-                        flags: int = SAVE_FOR_BACKWARD, stream=None):
-    """-> (out_feat[H,W,D], out_alpha[H,W], workspace).  Enqueues on the current stream; no sync."""
+                        flags: int = SAVE_FOR_BACKWARD, stream=None, out_scale: float = 1.0):
+    """-> (out_feat[H,W,D] ([D,H,W] with OUT_PLANAR), out_alpha[H,W], workspace).  Enqueues on the current stream;
+    no sync.  OUT_PLANAR / ACCUMULATE / out_scale != 1 go through inpc_raster_forward_ex."""
     lib = load()
     _check(pos, torch.float32, "pos"); _check(opacity, torch.float32, "opacity"); _check(feat, torch.float32, "feat")
     N, D = int(pos.shape[0]), int(feat.shape[1])
     cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
     W, H = cs.width, cs.height
     if workspace is None:
-        workspace = alloc_workspace(N, D, W, H, flags, pos.device)
+        workspace = alloc_workspace(N, D, W, H, flags & 3, pos.device)
     if out_feat is None:
-        out_feat = torch.empty((H, W, D), dtype=torch.float32, device=pos.device)
+        out_feat = torch.empty(_img_shape(H, W, D, flags), dtype=torch.float32, device=pos.device)
     if out_alpha is None:
         out_alpha = torch.empty((H, W), dtype=torch.float32, device=pos.device)
-    rc = lib.inpc_raster_forward(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(out_feat),
-                                 _ptr(out_alpha), _ptr(workspace), workspace.numel(), flags, _stream(stream))
+    if (flags & ~3) or out_scale != 1.0:
+        rc = lib.inpc_raster_forward_ex(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(out_feat),
+                                        _ptr(out_alpha), _ptr(workspace), workspace.numel(), flags, out_scale, _stream(stream))
+    else:
+        rc = lib.inpc_raster_forward(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(out_feat),
+                                     _ptr(out_alpha), _ptr(workspace), workspace.numel(), flags, _stream(stream))
     if rc != 0:
         raise InpcError(rc, "inpc_raster_forward")
     return out_feat, out_alpha, workspace
 
 
 def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha, workspace,
-                         grad_feat=None, grad_opacity=None, grad_uv=None, stream=None, blend_weight=None):
+                         grad_feat=None, grad_opacity=None, grad_uv=None, stream=None, blend_weight=None,
+                         flags: int = 0, grad_scale: float = 1.0):
     """-> (grad_feat[N,D], grad_opacity[N], grad_uv[N,2]).  Enqueues on the current stream; no sync.
     With blend_weight (True, or a float32 tensor [N]) the fused per-point blending weights (Eq. 3) come back
     as a fourth result (inpc_raster_backward_weights)."""
@@ -172,9 +253,19 @@ def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha,
         grad_opacity = torch.empty((N,), dtype=torch.float32, device=dev)
     if grad_uv is None:
         grad_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
-    if blend_weight is not None and blend_weight is not False:
-        if blend_weight is True:
-            blend_weight = torch.empty((N,), dtype=torch.float32, device=dev)
+    if blend_weight is True:
+        blend_weight = torch.empty((N,), dtype=torch.float32, device=dev)
+    elif blend_weight is False:
+        blend_weight = None
+    if flags or grad_scale != 1.0:
+        rc = lib.inpc_raster_backward_ex(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(grad_out_feat),
+                                         _ptr(grad_out_alpha), _ptr(grad_feat), _ptr(grad_opacity), _ptr(grad_uv),
+                                         _ptr(blend_weight), _ptr(workspace), workspace.numel(), flags, grad_scale,
+                                         _stream(stream))
+        if rc != 0:
+            raise InpcError(rc, "inpc_raster_backward_ex")
+        return (grad_feat, grad_opacity, grad_uv) + ((blend_weight,) if blend_weight is not None else ())
+    if blend_weight is not None:
         rc = lib.inpc_raster_backward_weights(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(grad_out_feat),
                                               _ptr(grad_out_alpha), _ptr(grad_feat), _ptr(grad_opacity), _ptr(grad_uv),
                                               _ptr(blend_weight), _ptr(workspace), workspace.numel(), _stream(stream))

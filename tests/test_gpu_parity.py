@@ -200,6 +200,119 @@ def test_single_pixel_image():
     full_parity(_wl(pos, rng.uniform(0, 0.05, n), rng.uniform(0, 1, (n, 4)), cam))
 
 
+# ------------------------------------------------------------------------------ NEXT row f3: levels, multisampling, [D,H,W]
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _reference_with_gpu_counts(ref, ws, W, H):
+    """Oracle image / alpha with the termination-ambiguous pixels resolved as in harness.oracle_reference."""
+    img_r, alpha_r, nb_r, margin = ref.blend()
+    amb = margin < harness.MARGIN
+    if amb.any():
+        nb = raster.inpc_raster_get_blended_counts(ws, W, H).cpu().numpy().view(np.uint32)
+        assert np.array_equal(nb[~amb], nb_r[~amb])
+        force = np.full((H, W), oracle.NO_FORCE, dtype=np.uint32)
+        force[amb] = nb[amb]
+        img_r, alpha_r, _, _ = ref.blend(force_nb=force)
+    return img_r, alpha_r
+
+
+@pytest.mark.parametrize("name,kw,planar", [("tiny", {}, False), ("tiny", {"D": 8}, True),
+                                            ("train", {"n_points": 1 << 19}, True), ("1m", {}, False)])
+def test_three_resolution_levels_forward_and_backward(name, kw, planar):
+    """One cloud at three resolution levels, each level against the oracle run with that
+    level's camera -- forward, and backward through inpc_raster_backward_ex with the level's own gradient images;
+    [D,H,W] layout on request."""
+    wl = make_workload(name, **kw)
+    D = wl.D
+    flags = raster.SAVE_FOR_BACKWARD | (raster.OUT_PLANAR if planar else 0)
+    pos, op, feat = _dev(wl.pos), _dev(wl.opacity), _dev(wl.feat)
+    imgs, alphas, wss, cams = raster.inpc_raster_forward_levels(pos, op, feat, wl.cam, 3, flags=flags)
+    torch.cuda.synchronize()
+    refs = oracle.rasterize_levels(wl.pos, wl.opacity, wl.feat, wl.cam, 3)
+    rng = np.random.Generator(np.random.PCG64(77))
+    for l in range(3):
+        oc = oracle.level_camera(wl.cam, l)
+        W, H = cams[l].width, cams[l].height
+        assert (W, H) == (oc.width, oc.height) and cams[l].fx == float(oc.fx) and cams[l].cx == float(oc.cx)
+        cnt = raster.inpc_raster_get_counts(wss[l], W, H).cpu().numpy().view(np.uint32)
+        assert np.array_equal(cnt, refs[l].counts()), f"level {l}: per-pixel counts differ"
+        img_r, alpha_r = _reference_with_gpu_counts(refs[l], wss[l], W, H)
+        img = imgs[l].cpu().numpy().astype(np.float64)
+        if planar:
+            assert img.shape == (D, H, W)
+            img_cmp = oracle.to_planar(img_r)
+        else:
+            img_cmp = img_r
+        assert np.abs(img - img_cmp).max() <= harness.FWD_ATOL, f"level {l}"
+        assert np.abs(alphas[l].cpu().numpy() - alpha_r).max() <= harness.FWD_ATOL
+        # backward of this level
+        g_img = rng.standard_normal((H, W, D)).astype(np.float32)
+        g_alpha = rng.standard_normal((H, W)).astype(np.float32)
+        g_dev = _dev(oracle.to_planar(g_img) if planar else g_img)
+        out = raster.inpc_raster_backward(pos, op, feat, cams[l], g_dev, _dev(g_alpha), wss[l],
+                                          flags=raster.OUT_PLANAR if planar else 0, grad_scale=0.5, blend_weight=True)
+        torch.cuda.synchronize()
+        assert raster.inpc_raster_get_status(wss[l]) == 0
+        rf, ro, ru = refs[l].backward(0.5 * g_img.astype(np.float64), 0.5 * g_alpha.astype(np.float64))
+        harness.check_grads(f"level {l} grad_feat", out[0], rf)
+        harness.check_grads(f"level {l} grad_opacity", out[1], ro)
+        harness.check_grads(f"level {l} grad_uv", out[2], ru)
+        assert np.abs(out[3].cpu().numpy() - refs[l].blend_weights()).max() <= harness.BW_ATOL
+
+
+@pytest.mark.parametrize("planar", [False, True])
+def test_multisample_average_of_four_clouds(planar):
+    """Inference multisampling: four independently drawn clouds, per-pixel mean, two levels."""
+    clouds_np, clouds = [], []
+    for s in range(4):
+        wl = make_workload("train", n_points=1 << 18, seed=40 + s)
+        clouds_np.append((wl.pos, wl.opacity, wl.feat))
+        clouds.append((_dev(wl.pos), _dev(wl.opacity), _dev(wl.feat)))
+    cam = wl.cam
+    imgs, alphas = raster.inpc_raster_forward_multisample(clouds, cam, n_levels=2, flags=raster.OUT_PLANAR if planar else 0)
+    torch.cuda.synchronize()
+    ref = oracle.multisample(clouds_np, cam, n_levels=2)
+    for l in range(2):
+        img = imgs[l].cpu().numpy().astype(np.float64)
+        img_r = oracle.to_planar(ref[l][0]) if planar else ref[l][0]
+        # each cloud's image is within 1e-4 (termination-ambiguous pixels included: one fragment more or less at
+        # T ~ 1e-4 moves a pixel by < 1e-4), so is their mean
+        assert np.abs(img - img_r).max() <= harness.FWD_ATOL
+        assert np.abs(alphas[l].cpu().numpy() - ref[l][1]).max() <= harness.FWD_ATOL
+    # bit-reproducible, and equal to accumulating by hand through inpc_raster_forward_ex
+    imgs2, alphas2 = raster.inpc_raster_forward_multisample(clouds, cam, n_levels=2, flags=raster.OUT_PLANAR if planar else 0)
+    assert torch.equal(imgs[0], imgs2[0]) and torch.equal(alphas[1], alphas2[1])
+    fl = raster.OUT_PLANAR if planar else 0
+    out_f, out_a, ws = raster.inpc_raster_forward(*clouds[0], cam, flags=fl, out_scale=0.25)
+    for c in clouds[1:]:
+        raster.inpc_raster_forward(*c, cam, out_feat=out_f, out_alpha=out_a, workspace=ws, flags=fl | raster.ACCUMULATE,
+                                   out_scale=0.25)
+    assert torch.equal(out_f, imgs[0]) and torch.equal(out_a, alphas[0])
+
+
+def test_forward_ex_defaults_are_bit_identical_to_forward():
+    wl = make_workload("tiny")
+    pos, op, feat = _dev(wl.pos), _dev(wl.opacity), _dev(wl.feat)
+    a = raster.inpc_raster_forward(pos, op, feat, wl.cam, flags=raster.SAVE_FOR_BACKWARD)
+    lib = raster.load()
+    img = torch.empty_like(a[0]); alpha = torch.empty_like(a[1])
+    cs = raster.camera_struct(wl.cam)
+    rc = lib.inpc_raster_forward_ex(pos.data_ptr(), op.data_ptr(), feat.data_ptr(), wl.N, 4, ctypes.byref(cs), img.data_ptr(),
+                                    alpha.data_ptr(), a[2].data_ptr(), a[2].numel(), raster.SAVE_FOR_BACKWARD, 1.0, None)
+    torch.cuda.synchronize()
+    assert rc == 0 and torch.equal(img, a[0]) and torch.equal(alpha, a[1])
+    with pytest.raises(raster.InpcError) as e:                  # the plain entry point refuses the layout flags
+        lib2 = raster.load()
+        rc = lib2.inpc_raster_forward(pos.data_ptr(), op.data_ptr(), feat.data_ptr(), wl.N, 4, ctypes.byref(cs), img.data_ptr(),
+                                      alpha.data_ptr(), a[2].data_ptr(), a[2].numel(), raster.OUT_PLANAR, None)
+        if rc != 0:
+            raise raster.InpcError(rc, "inpc_raster_forward")
+    assert e.value.status == -1
+
+
 # ------------------------------------------------------------------------------ API behaviour
 
 def test_forward_is_repeatable_and_workspace_reusable():

@@ -289,6 +289,42 @@ def test_blend_weights_golden():
     assert (bw >= 0).all() and (bw <= w.opacity.astype(np.float64) + 1e-15).all() and bw.max() > 0.3
 
 
+def test_level_camera_golden_and_multisample_mean():
+    """NEXT row f3: the level camera against a hand-derived footprint (tests/golden/level1_point.txt); the
+    multisample image is the plain mean; the planar layout is a transposition."""
+    cam = Camera(**TINY)
+    c1 = oracle.level_camera(cam, 1)
+    assert (c1.width, c1.height, float(c1.fx), float(c1.cx)) == (32, 32, 32.0, 16.0)
+    c2 = oracle.level_camera(Camera(fx=1100.0, fy=1100.0, cx=648.5, cy=420.0, width=1297, height=840), 2)
+    assert (c2.width, c2.height, float(c2.fx), float(c2.cx), float(c2.cy)) == (325, 210, 275.0, 162.125, 105.0)
+    f = np.array([[0.25, 0.5, 0.75, 1.0]], np.float32)
+    r0, r1 = oracle.rasterize_levels([[0.3, -0.2, 4.0]], [0.5], f, cam, 2)
+    img, alpha, _, _ = r1.blend()
+    assert img.shape == (32, 32, 4)
+    total = 0.0
+    for x, y, w in _golden("level1_point.txt"):
+        assert abs(alpha[int(y), int(x)] - 0.5 * w) < 2e-6            # fp32 u carries an ulp of 2e-6 into tx
+        np.testing.assert_allclose(img[int(y), int(x)], 0.5 * w * f[0], atol=2e-6)
+        total += alpha[int(y), int(x)]
+    assert abs(total - 0.5) < 1e-12 and abs(alpha.sum() - 0.5) < 1e-12
+    # the same point at level 0 keeps the single_point.txt footprint
+    a0 = r0.blend()[1]
+    assert abs(a0[28, 36] - 0.5 * 0.49) < 2e-6
+    # multisample: mean of the clouds' images; two single-point clouds on different pixels -> half of each
+    A = ([[0.3, -0.2, 4.0]], [0.5], f)
+    B = ([[-0.4, 0.1, 2.0]], [0.8], f * 0.5)
+    (m_img, m_alpha), = oracle.multisample([A, B], cam)
+    ia = oracle.Raster.from_points(*A, cam).blend()
+    ib = oracle.Raster.from_points(*B, cam).blend()
+    np.testing.assert_array_equal(m_img, (ia[0] + ib[0]) / 2)
+    np.testing.assert_array_equal(m_alpha, (ia[1] + ib[1]) / 2)
+    assert abs(m_alpha.sum() - (0.5 + float(np.float32(0.8))) / 2) < 1e-12       # opacities are fp32 inputs
+    (s_img, s_alpha), = oracle.multisample([A, A, A, A], cam)            # identical clouds: the mean is the image
+    np.testing.assert_allclose(s_img, ia[0], atol=1e-16)
+    pl = oracle.to_planar(m_img)
+    assert pl.shape == (4, 64, 64) and pl[2, 28, 36] == m_img[28, 36, 2]
+
+
 def test_general_stack_formula():
     rng = np.random.default_rng(5)
     n = 12
