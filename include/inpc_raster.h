@@ -71,6 +71,7 @@ typedef enum inpc_status {
 /* flags of the _ex / _levels / _multisample entry points only (NEXT row f3 of the scope table) */
 #define INPC_OUT_PLANAR        4u  /* feature image (and its gradient) as [D][H][W] instead of [H][W][D]     */
 #define INPC_ACCUMULATE        8u  /* forward: out += out_scale * result (out holds an earlier call's image) */
+#define INPC_FUSED_SH         16u  /* workspace sizing for inpc_raster_forward_sh / _backward_sh (NEXT row f2)  */
 
 typedef struct inpc_stats {          /* host struct filled by inpc_raster_get_stats                          */
     uint64_t n_points;               /* N of the last forward                                                 */
@@ -122,6 +123,22 @@ int inpc_raster_backward_ex(const float* pos, const float* opacity, const float*
                             const inpc_camera* cam,
                             const float* grad_out_feat, const float* grad_out_alpha,
                             float* grad_feat, float* grad_opacity, float* grad_uv, float* blend_weight,
+                            void* workspace, size_t workspace_bytes, uint32_t flags, float grad_scale, void* cuda_stream);
+
+/* ---- NEXT row f2: spherical harmonics fused into the rasterizer. ------------------------
+ * sh_coeff[N][36] replaces feat: the 4-D feature of a point is  f[d] = sum_{b<9} Y_b(dir) sh_coeff[4 b + d]  with
+ * Y_0..Y_8 the real SH basis of degree <= 2 (Condon-Shortley phase; reading R18) of the unit direction
+ * from the camera centre (-R^T t) to the point.  D is 4.  The workspace must be sized with
+ * inpc_raster_workspace_bytes(N, 4, W, H, flags | INPC_FUSED_SH).  Other arguments as inpc_raster_forward_ex /
+ * inpc_raster_backward_ex; grad_sh_coeff[N][36] = Y_b dL/df[d] (exact zeros for culled points).  No gradient is
+ * propagated into the position through the direction. */
+int inpc_raster_forward_sh(const float* pos, const float* opacity, const float* sh_coeff, int64_t N,
+                           const inpc_camera* cam, float* out_feat, float* out_alpha,
+                           void* workspace, size_t workspace_bytes, uint32_t flags, float out_scale, void* cuda_stream);
+int inpc_raster_backward_sh(const float* pos, const float* opacity, const float* sh_coeff, int64_t N,
+                            const inpc_camera* cam,
+                            const float* grad_out_feat, const float* grad_out_alpha,
+                            float* grad_sh_coeff, float* grad_opacity, float* grad_uv, float* blend_weight,
                             void* workspace, size_t workspace_bytes, uint32_t flags, float grad_scale, void* cuda_stream);
 
 /* Camera of resolution level l (host only, no device work): the image is halved l times,

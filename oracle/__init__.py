@@ -254,3 +254,50 @@ def multisample(clouds, cam, n_levels: int = 1):
 def to_planar(img):
     """[H,W,D] -> [D,H,W]."""
     return np.ascontiguousarray(np.transpose(img, (2, 0, 1)))
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT row f2 -- view-dependent features from spherical harmonics (PAPER.md:112: SH of degree 2, 4-D output,
+# M = 36 coefficients per point; "fused into this pipeline", PAPER.md:370).  Plain numpy, fp64.
+
+SH_C0 = 0.28209479177387814      # 1 / (2 sqrt(pi))
+SH_C1 = 0.4886025119029199       # sqrt(3 / (4 pi))
+SH_C2 = (1.0925484305920792,     # sqrt(15 / (4 pi))
+         0.31539156525252005,    # sqrt(5 / (16 pi))
+         0.5462742152960396)     # sqrt(15 / (16 pi))
+
+
+def sh_basis(d):
+    """Real SH basis of degree 0..2 at unit directions d[...,3] -> [...,9], in the order (l, m) = (0,0), (1,-1), (1,0),
+    (1,1), (2,-2), (2,-1), (2,0), (2,1), (2,2), with the Condon-Shortley phase (-1)^m (reading R18: the paper names no
+    convention; this is the one of the common graphics code bases).  Pinned against scipy.special in the tests."""
+    d = np.asarray(d, dtype=np.float64)
+    x, y, z = d[..., 0], d[..., 1], d[..., 2]
+    return np.stack([np.full_like(x, SH_C0), -SH_C1 * y, SH_C1 * z, -SH_C1 * x,
+                     SH_C2[0] * x * y, -SH_C2[0] * y * z, SH_C2[1] * (2 * z * z - x * x - y * y),
+                     -SH_C2[0] * x * z, SH_C2[2] * (x * x - y * y)], axis=-1)
+
+
+def view_directions(pos, cam):
+    """Unit vectors from the camera centre (-R^T t) to the points (zero vector for a point on the centre)."""
+    R = np.asarray(cam.R, dtype=np.float64).reshape(3, 3)
+    t = np.asarray(cam.t, dtype=np.float64).reshape(3)
+    v = np.asarray(pos, dtype=np.float64).reshape(-1, 3) - (-R.T @ t)
+    n = np.linalg.norm(v, axis=1, keepdims=True)
+    return np.divide(v, n, out=np.zeros_like(v), where=n > 0)
+
+
+def sh_features(pos, coeff, cam):
+    """coeff[N,36] (basis-major: coefficient 4 b + d belongs to basis b, channel d) -> feat[N,4] f64."""
+    Y = sh_basis(view_directions(pos, cam))                                   # [N,9]
+    Y = np.where(np.linalg.norm(view_directions(pos, cam), axis=1, keepdims=True) > 0, Y, np.array([SH_C0] + [0.0] * 8))
+    c = np.asarray(coeff, dtype=np.float64).reshape(-1, 9, 4)
+    return np.einsum("nb,nbd->nd", Y, c)
+
+
+def sh_backward(pos, cam, d_feat):
+    """dL/dcoeff[N,36] = Y_b dL/dfeat[d] (the feature is linear in the coefficients)."""
+    dirs = view_directions(pos, cam)
+    Y = sh_basis(dirs)
+    Y = np.where(np.linalg.norm(dirs, axis=1, keepdims=True) > 0, Y, np.array([SH_C0] + [0.0] * 8))
+    return np.einsum("nb,nd->nbd", Y, np.asarray(d_feat, dtype=np.float64)).reshape(-1, 36)

@@ -7,6 +7,7 @@
 //       k_classify (per-pixel fragment counts = 2x2 box sum of the cell counts)
 #pragma once
 #include "common.cuh"
+#include "sh.cuh"
 
 namespace inpc {
 
@@ -65,9 +66,14 @@ __global__ void __launch_bounds__(kBinThreads) k_project_count(const float* __re
 // { depth_bits, idx, tx, ty | opacity, cell, 0, 0 }.  (Anything narrower than a sector scattered by slot costs a
 // DRAM read-modify-write: profiles/r01_v1_baseline.md.)  All of a thread's atomics and opacity loads are
 // issued before the first store.
+// SH (NEXT row f2, sh.cuh): the pass also evaluates every kept point's view-dependent feature from its 36 SH
+// coefficients (read once, here, coalesced) and leaves it in shfeat[point] for the cell sort to pick up.
+template <bool SH>
 __global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict__ pos,
                                                           const float* __restrict__ opacity, long long N, Camera cam,
-                                                          uint32_t* __restrict__ cursor, float4* __restrict__ A) {
+                                                          uint32_t* __restrict__ cursor, float4* __restrict__ A,
+                                                          const float4* __restrict__ sh_coeff, ViewPoint view,
+                                                          float4* __restrict__ shfeat) {
     __shared__ __align__(16) float s_pos[kBinChunk * 3];
     for (long long base = (long long)blockIdx.x * kBinChunk; base < N; base += (long long)gridDim.x * kBinChunk) {
         __syncthreads();
@@ -100,6 +106,11 @@ __global__ void __launch_bounds__(kBinThreads) k_scatter(const float* __restrict
             a1.y = __uint_as_float((uint32_t)p[k].cell);
             a1.z = 0.f; a1.w = 0.f;
             st_sector(A + 2 * (size_t)slot[k], a0, a1);         // one 256-bit store = the whole 32-byte sector
+            if (SH) {
+                const int l = k * kBinThreads + threadIdx.x;
+                shfeat[i] = sh_feature(sh_coeff + (size_t)i * kShBasis, s_pos[3 * l] - view.cx, s_pos[3 * l + 1] - view.cy,
+                                       s_pos[3 * l + 2] - view.cz);
+            }
         }
     }
 }

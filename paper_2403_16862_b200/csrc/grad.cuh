@@ -16,6 +16,7 @@
 //              blend_weight[N] (coalesced); culled points (their bit of the kept mask is 0) get exact zeros.
 #pragma once
 #include "common.cuh"
+#include "sh.cuh"
 
 namespace inpc {
 
@@ -106,11 +107,14 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
     }
 }
 
-template <int D>
+// SH (NEXT row f2): d_feat is dL/dcoeff[N][36] = Y_b(dir) dL/dfeature[d] instead of dL/dfeature[N][4]; pos / view give
+// the direction (no gradient flows into the position through it: the paper's positions are sampled, not optimised).
+template <int D, bool SH>
 __global__ void __launch_bounds__(256) k_split(const Header* __restrict__ hdr, const float* __restrict__ gpt,
                                                 const uint32_t* __restrict__ kept,
                                                 long long N, float* __restrict__ d_feat, float* __restrict__ d_opacity,
-                                                float* __restrict__ d_uv, float* __restrict__ blend_weight) {
+                                                float* __restrict__ d_uv, float* __restrict__ blend_weight,
+                                                const float* __restrict__ pos, ViewPoint view) {
     constexpr int GP = gpt_floats<D>();
     if (!hdr->bwd_ok) return;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
@@ -123,8 +127,17 @@ __global__ void __launch_bounds__(256) k_split(const Header* __restrict__ hdr, c
             for (int v = 0; v < D / 4; ++v) f[v] = __ldcs(&in[v]);
             o = __ldcs(&in[D / 4]);
         }
+        if (SH) {
+            float Y[kShBasis];
+            sh_basis9(__ldg(&pos[3 * i]) - view.cx, __ldg(&pos[3 * i + 1]) - view.cy, __ldg(&pos[3 * i + 2]) - view.cz, Y);
 #pragma unroll
-        for (int v = 0; v < D / 4; ++v) __stcs(reinterpret_cast<float4*>(d_feat + (size_t)i * D) + v, f[v]);
+            for (int b = 0; b < kShBasis; ++b)
+                __stcs(reinterpret_cast<float4*>(d_feat + (size_t)i * kShCoeffs) + b,
+                       make_float4(Y[b] * f[0].x, Y[b] * f[0].y, Y[b] * f[0].z, Y[b] * f[0].w));
+        } else {
+#pragma unroll
+            for (int v = 0; v < D / 4; ++v) __stcs(reinterpret_cast<float4*>(d_feat + (size_t)i * D) + v, f[v]);
+        }
         __stcs(&d_opacity[i], o.x);
         __stcs(reinterpret_cast<float2*>(d_uv) + i, make_float2(o.y, o.z));
         if (blend_weight) __stcs(&blend_weight[i], o.w);

@@ -87,6 +87,7 @@ struct Layout {
     size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
     size_t kept, cursor, A, gT, gD, dk, Ra, Rf, items, bigpix, bigcells, bigkeys;
     size_t pcur, gpt;                                     // only with INPC_SAVE_FOR_BACKWARD
+    size_t shfeat;                                        // only with INPC_FUSED_SH: per-point features out of the SH pass
     size_t pixoff, sorted_idx, sorted_depth, sorted_T;    // only with INPC_SAVE_SORTED
     size_t total;
     uint32_t C, P, max_big_cells, n_status;
@@ -123,6 +124,7 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
         L.pcur = o; o = align_up(o + (size_t)L.P * 16);
         L.gpt = o;  o = align_up(o + n * (size_t)(D == 4 ? 32 : 64) + 64);
     }
+    if (flags & INPC_FUSED_SH) { L.shfeat = o; o = align_up(o + (n + 8) * 16); }
     if (flags & INPC_SAVE_SORTED) {
         L.pixoff = o;       o = align_up(o + ((size_t)L.P + 1) * 4);
         L.sorted_idx = o;   o = align_up(o + (4 * n + 8) * 4);
@@ -165,6 +167,14 @@ static int check_common(int64_t N, int D, const inpc_camera* cam) {
     if (D != 4 && D != 8) return INPC_ERR_UNSUPPORTED;
     if (cam->width > 4095 || cam->height > 4095) return INPC_ERR_UNSUPPORTED;
     return INPC_OK;
+}
+
+static ViewPoint view_point(const inpc_camera* c) {       // camera centre in world space: -R^T t
+    ViewPoint v;
+    v.cx = -(c->R[0] * c->t[0] + c->R[3] * c->t[1] + c->R[6] * c->t[2]);
+    v.cy = -(c->R[1] * c->t[0] + c->R[4] * c->t[1] + c->R[7] * c->t[2]);
+    v.cz = -(c->R[2] * c->t[0] + c->R[5] * c->t[1] + c->R[8] * c->t[2]);
+    return v;
 }
 
 static Camera to_camera(const inpc_camera* c) {
@@ -330,7 +340,7 @@ static Side* side_for(const DeviceInfo& di) {
 template <int D>
 static int forward_impl(const float* pos, const float* opacity, const float* feat, int64_t N, const inpc_camera* cam,
                         float* out_feat, float* out_alpha, unsigned char* ws, const Layout& L, uint32_t flags,
-                        float out_scale, cudaStream_t st) {
+                        float out_scale, cudaStream_t st, const float* sh_coeff = nullptr) {
     const DeviceInfo di = device_info();
     if (!di.ok) return cuda_fail(cudaErrorNoDevice);
     const Camera camk = to_camera(cam);
@@ -405,8 +415,16 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     // caller's stream: scatter, then the cell sort band by band
     if (N > 0) {
         { StageTimer tm(kStScatter, st);
-          k_scatter<<<scatter_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cursor, Arec); }
-        INPC_LAUNCHED("k_scatter");
+          if (sh_coeff) {
+              feat = reinterpret_cast<const float*>(ws + L.shfeat);       // from here on the features are the SH pass's
+              k_scatter<true><<<scatter_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cursor, Arec,
+                                                                    reinterpret_cast<const float4*>(sh_coeff), view_point(cam),
+                                                                    reinterpret_cast<float4*>(ws + L.shfeat));
+          } else {
+              k_scatter<false><<<scatter_grid, kBinThreads, 0, st>>>(pos, opacity, (long long)N, camk, cursor, Arec, nullptr,
+                                                                     ViewPoint{}, nullptr);
+          } }
+        INPC_LAUNCHED(sh_coeff ? "k_scatter<1>" : "k_scatter<0>");
         INPC_CUDA(fork(s2, st));                                              // the large-cell list
         int rc = launch_cellsort_big<D>(hdr, bigcells, Arec,
                                         reinterpret_cast<unsigned long long*>(ws + L.bigkeys), feat, dk, Ra, Rf, di,
@@ -455,7 +473,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
 template <int D>
 static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat, const float* g_alpha, float* d_feat,
                          float* d_opacity, float* d_uv, float* blend_weight, unsigned char* ws, const Layout& L,
-                         uint32_t flags, float grad_scale, cudaStream_t st) {
+                         uint32_t flags, float grad_scale, cudaStream_t st, const float* sh_pos = nullptr) {
     const DeviceInfo di = device_info();
     if (!di.ok) return cuda_fail(cudaErrorNoDevice);
     const int W = cam->width, H = cam->height;
@@ -514,9 +532,13 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     }
     INPC_CUDA(fork(s2, st));                                                  // join
     { StageTimer tm(kStSplit, st);
-      k_split<D><<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16), 256, 0, st>>>(
-          hdr, gpt, reinterpret_cast<const uint32_t*>(ws + L.kept), (long long)N, d_feat, d_opacity, d_uv, blend_weight); }
-    INPC_LAUNCHED(kname<D>("k_split"));
+      const int grid = (int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16);
+      const uint32_t* kept = reinterpret_cast<const uint32_t*>(ws + L.kept);
+      if (sh_pos) k_split<D, true><<<grid, 256, 0, st>>>(hdr, gpt, kept, (long long)N, d_feat, d_opacity, d_uv, blend_weight,
+                                                         sh_pos, view_point(cam));
+      else k_split<D, false><<<grid, 256, 0, st>>>(hdr, gpt, kept, (long long)N, d_feat, d_opacity, d_uv, blend_weight,
+                                                   nullptr, ViewPoint{}); }
+    INPC_LAUNCHED(sh_pos ? kname<D, 1>("k_split") : kname<D, 0>("k_split"));
     return INPC_OK;
 }
 
@@ -563,6 +585,45 @@ int inpc_raster_forward_ex(const float* pos, const float* opacity, const float* 
                            size_t workspace_bytes, uint32_t flags, float out_scale, void* cuda_stream) {
     return forward_entry(pos, opacity, feat, N, D, cam, out_feat, out_alpha, workspace, workspace_bytes, flags, out_scale,
                          cuda_stream);
+}
+
+int inpc_raster_forward_sh(const float* pos, const float* opacity, const float* sh_coeff, int64_t N,
+                           const inpc_camera* cam, float* out_feat, float* out_alpha, void* workspace,
+                           size_t workspace_bytes, uint32_t flags, float out_scale, void* cuda_stream) {
+    int rc = check_common(N, 4, cam);
+    if (rc != INPC_OK) return rc;
+    if (!out_feat || !out_alpha || !workspace) return INPC_ERR_INVALID_ARG;
+    if (N > 0 && (!pos || !opacity || !sh_coeff)) return INPC_ERR_INVALID_ARG;
+    if (flags & ~(INPC_SAVE_FOR_BACKWARD | INPC_SAVE_SORTED | INPC_OUT_PLANAR | INPC_ACCUMULATE | INPC_FUSED_SH)) return INPC_ERR_INVALID_ARG;
+    flags |= INPC_FUSED_SH;
+    if (!aligned16(pos) || !aligned16(opacity) || !aligned16(sh_coeff) || !aligned16(out_feat) || !aligned16(out_alpha) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 255u))
+        return INPC_ERR_INVALID_ARG;
+    const Layout L = make_layout(N, 4, cam->width, cam->height, flags);
+    if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
+    return forward_impl<4>(pos, opacity, nullptr, N, cam, out_feat, out_alpha, static_cast<unsigned char*>(workspace), L, flags,
+                           out_scale, static_cast<cudaStream_t>(cuda_stream), N > 0 ? sh_coeff : nullptr);
+}
+
+int inpc_raster_backward_sh(const float* pos, const float* opacity, const float* sh_coeff, int64_t N,
+                            const inpc_camera* cam, const float* grad_out_feat, const float* grad_out_alpha,
+                            float* grad_sh_coeff, float* grad_opacity, float* grad_uv, float* blend_weight,
+                            void* workspace, size_t workspace_bytes, uint32_t flags, float grad_scale, void* cuda_stream) {
+    (void)opacity; (void)sh_coeff;
+    int rc = check_common(N, 4, cam);
+    if (rc != INPC_OK) return rc;
+    if (!grad_out_feat || !workspace) return INPC_ERR_INVALID_ARG;
+    if (N > 0 && (!pos || !grad_sh_coeff || !grad_opacity || !grad_uv)) return INPC_ERR_INVALID_ARG;
+    if (flags & ~INPC_OUT_PLANAR) return INPC_ERR_INVALID_ARG;
+    if (!aligned16(pos) || !aligned16(grad_out_feat) || !aligned16(grad_out_alpha) || !aligned16(grad_sh_coeff) ||
+        !aligned16(grad_opacity) || !aligned16(grad_uv) || !aligned16(blend_weight) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 255u))
+        return INPC_ERR_INVALID_ARG;
+    const Layout L = make_layout(N, 4, cam->width, cam->height, INPC_SAVE_FOR_BACKWARD | INPC_FUSED_SH);
+    if (workspace_bytes < L.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
+    return backward_impl<4>(N, cam, grad_out_feat, grad_out_alpha, grad_sh_coeff, grad_opacity, grad_uv, blend_weight,
+                            static_cast<unsigned char*>(workspace), L, flags, grad_scale,
+                            static_cast<cudaStream_t>(cuda_stream), N > 0 ? pos : nullptr);
 }
 
 int inpc_raster_level_camera(const inpc_camera* cam, int32_t level, inpc_camera* out) {

@@ -18,11 +18,13 @@ SAVE_FOR_BACKWARD = 1
 SAVE_SORTED = 2
 OUT_PLANAR = 4          # _ex / _levels / _multisample entry points: feature image as [D][H][W]
 ACCUMULATE = 8          # _ex: add to the image already in the output buffers
+FUSED_SH = 16           # workspace sizing of the _sh entry points
+SH_COEFFS = 36          # M: 9 basis functions x 4 channels, basis-major
 
 EXPORTS = (
     "inpc_raster_workspace_bytes", "inpc_raster_forward", "inpc_raster_backward", "inpc_raster_backward_weights",
     "inpc_raster_forward_ex", "inpc_raster_backward_ex", "inpc_raster_level_camera", "inpc_raster_forward_levels",
-    "inpc_raster_forward_multisample",
+    "inpc_raster_forward_multisample", "inpc_raster_forward_sh", "inpc_raster_backward_sh",
     "inpc_raster_get_counts", "inpc_raster_get_blended_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
     "inpc_raster_get_status",
     "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count", "inpc_raster_launched_kernels",
@@ -75,6 +77,10 @@ def load() -> C.CDLL:
         lib.inpc_raster_forward_ex.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, C.c_size_t, u32, C.c_float, vp]
         lib.inpc_raster_backward_ex.restype = C.c_int
         lib.inpc_raster_backward_ex.argtypes = [vp, vp, vp, i64, i32, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, vp, C.c_size_t, u32, C.c_float, vp]
+        lib.inpc_raster_forward_sh.restype = C.c_int
+        lib.inpc_raster_forward_sh.argtypes = [vp, vp, vp, i64, C.POINTER(InpcCamera), vp, vp, vp, C.c_size_t, u32, C.c_float, vp]
+        lib.inpc_raster_backward_sh.restype = C.c_int
+        lib.inpc_raster_backward_sh.argtypes = [vp, vp, vp, i64, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, vp, C.c_size_t, u32, C.c_float, vp]
         lib.inpc_raster_level_camera.restype = C.c_int
         lib.inpc_raster_level_camera.argtypes = [C.POINTER(InpcCamera), i32, C.POINTER(InpcCamera)]
         lib.inpc_raster_forward_levels.restype = C.c_int
@@ -206,6 +212,42 @@ def inpc_raster_forward_multisample(clouds, cam, n_levels: int = 1, flags: int =
     if rc != 0:
         raise InpcError(rc, "inpc_raster_forward_multisample")
     return imgs, alphas
+
+
+def inpc_raster_forward_sh(pos, opacity, sh_coeff, cam, flags: int = SAVE_FOR_BACKWARD, out_scale: float = 1.0, stream=None):
+    """Forward with the SH evaluation fused in: sh_coeff[N,36] instead of feat.  -> (out_feat, out_alpha, workspace)."""
+    lib = load()
+    _check(pos, torch.float32, "pos"); _check(opacity, torch.float32, "opacity"); _check(sh_coeff, torch.float32, "sh_coeff")
+    N = int(pos.shape[0])
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    W, H = cs.width, cs.height
+    ws = alloc_workspace(N, 4, W, H, (flags & 3) | FUSED_SH, pos.device)
+    out_feat = torch.empty(_img_shape(H, W, 4, flags), dtype=torch.float32, device=pos.device)
+    out_alpha = torch.empty((H, W), dtype=torch.float32, device=pos.device)
+    rc = lib.inpc_raster_forward_sh(_ptr(pos), _ptr(opacity), _ptr(sh_coeff), N, C.byref(cs), _ptr(out_feat), _ptr(out_alpha),
+                                    _ptr(ws), ws.numel(), flags, out_scale, _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_forward_sh")
+    return out_feat, out_alpha, ws
+
+
+def inpc_raster_backward_sh(pos, opacity, sh_coeff, cam, grad_out_feat, grad_out_alpha, workspace, flags: int = 0,
+                            grad_scale: float = 1.0, blend_weight: bool = False, stream=None):
+    """-> (grad_sh_coeff[N,36], grad_opacity[N], grad_uv[N,2][, blend_weight[N]])."""
+    lib = load()
+    N = int(pos.shape[0])
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    dev = pos.device
+    g_c = torch.empty((N, SH_COEFFS), dtype=torch.float32, device=dev)
+    g_o = torch.empty((N,), dtype=torch.float32, device=dev)
+    g_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
+    bw = torch.empty((N,), dtype=torch.float32, device=dev) if blend_weight else None
+    rc = lib.inpc_raster_backward_sh(_ptr(pos), _ptr(opacity), _ptr(sh_coeff), N, C.byref(cs), _ptr(grad_out_feat),
+                                     _ptr(grad_out_alpha), _ptr(g_c), _ptr(g_o), _ptr(g_uv), _ptr(bw), _ptr(workspace),
+                                     workspace.numel(), flags, grad_scale, _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_raster_backward_sh")
+    return (g_c, g_o, g_uv) + ((bw,) if blend_weight else ())
 
 
 def inpc_raster_forward(pos, opacity, feat, cam, out_feat=None, out_alpha=None, workspace=None,

@@ -313,6 +313,48 @@ def test_forward_ex_defaults_are_bit_identical_to_forward():
     assert e.value.status == -1
 
 
+# ------------------------------------------------------------------------------ NEXT row f2: fused spherical harmonics
+
+@pytest.mark.parametrize("name,kw,pose", [("tiny", {}, False), ("tiny", {}, True), ("train", {"n_points": 1 << 20}, False)])
+def test_fused_sh_forward_and_backward(name, kw, pose):
+    """36 SH coefficients per point instead of a feature: forward image / alpha and the gradients
+    w.r.t. the coefficients, opacity and screen position against the oracle (numpy SH in fp64 + the plain oracle)."""
+    wl = make_workload(name, **kw)
+    if pose:
+        R, t = second_pose()
+        wl.cam = wl.cam.with_pose(R, t)
+    W, H, N = wl.cam.width, wl.cam.height, wl.N
+    rng = np.random.Generator(np.random.PCG64(123))
+    coeff = (rng.standard_normal((N, 36)) * 0.5).astype(np.float32)
+    pos, op, cf = _dev(wl.pos), _dev(wl.opacity), _dev(coeff)
+    img, alpha, ws = raster.inpc_raster_forward_sh(pos, op, cf, wl.cam, flags=raster.SAVE_FOR_BACKWARD)
+    torch.cuda.synchronize()
+    feat_r = oracle.sh_features(wl.pos, coeff, wl.cam)
+    ref = oracle.Raster.from_points(wl.pos, wl.opacity, feat_r.astype(np.float32), wl.cam)
+    cnt = raster.inpc_raster_get_counts(ws, W, H).cpu().numpy().view(np.uint32)
+    assert np.array_equal(cnt, ref.counts())
+    img_r, alpha_r = _reference_with_gpu_counts(ref, ws, W, H)
+    scale = max(1.0, float(np.abs(feat_r).max()))              # the image is linear in the features
+    assert np.abs(img.cpu().numpy() - img_r).max() <= harness.FWD_ATOL * scale
+    assert np.abs(alpha.cpu().numpy() - alpha_r).max() <= harness.FWD_ATOL
+    g_c, g_o, g_uv, bw = raster.inpc_raster_backward_sh(pos, op, cf, wl.cam, _dev(wl.g_img), _dev(wl.g_alpha), ws,
+                                                        blend_weight=True)
+    torch.cuda.synchronize()
+    assert raster.inpc_raster_get_status(ws) == 0
+    rf, ro, ru = ref.backward(wl.g_img, wl.g_alpha)
+    harness.check_grads("grad_sh_coeff", g_c, oracle.sh_backward(wl.pos, wl.cam, rf))
+    # opacity / uv gradients carry the feature magnitude: same relative tolerance, the absolute floor scaled with it
+    for name_, got, want in (("grad_opacity", g_o, ro), ("grad_uv", g_uv, ru)):
+        got = got.cpu().numpy().astype(np.float64).reshape(want.shape)
+        tol = np.maximum(harness.GRAD_RTOL * np.abs(want), harness.GRAD_ATOL * scale)
+        assert (np.abs(got - want) <= tol).all(), name_
+    assert np.abs(bw.cpu().numpy() - ref.blend_weights()).max() <= harness.BW_ATOL
+    # culled points: exact zeros in all 36 coefficient gradients
+    dead = ~np.isin(np.arange(N), ref.sorted_fragments()[1])
+    if dead.any():
+        assert float(g_c.cpu().numpy()[dead].__abs__().max()) == 0.0
+
+
 # ------------------------------------------------------------------------------ API behaviour
 
 def test_forward_is_repeatable_and_workspace_reusable():

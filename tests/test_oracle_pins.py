@@ -325,6 +325,58 @@ def test_level_camera_golden_and_multisample_mean():
     assert pl.shape == (4, 64, 64) and pl[2, 28, 36] == m_img[28, 36, 2]
 
 
+def test_sh_basis_against_scipy_and_closed_forms():
+    """NEXT row f2: the oracle's real SH basis (degree <= 2) against a LIBRARY routine -- the complex spherical
+    harmonics of scipy.special -- and against closed forms on the axes."""
+    from scipy import special
+    rng = np.random.default_rng(11)
+    d = rng.standard_normal((200, 3)); d /= np.linalg.norm(d, axis=1, keepdims=True)
+    theta = np.arctan2(d[:, 1], d[:, 0])            # azimuth
+    phi = np.arccos(d[:, 2])                        # polar angle
+    if hasattr(special, "sph_harm_y"):
+        Ylm = lambda l, m: special.sph_harm_y(l, m, phi, theta)
+    else:
+        Ylm = lambda l, m: special.sph_harm(m, l, theta, phi)
+    ref = []
+    for l in range(3):
+        for m in range(-l, l + 1):
+            if m == 0:
+                ref.append(Ylm(l, 0).real)
+            elif m > 0:
+                ref.append(np.sqrt(2) * Ylm(l, m).real)       # scipy includes the Condon-Shortley phase: the real
+            else:                                             # combination is sqrt(2) Re / Im of Y_l^|m|, no extra sign
+                ref.append(np.sqrt(2) * Ylm(l, -m).imag)
+    np.testing.assert_allclose(oracle.sh_basis(d), np.stack(ref, 1), atol=1e-12)
+    # closed forms: +z sees Y = (C0, 0, C1, 0, 0, 0, 2 * 0.3154, 0, 0)
+    np.testing.assert_allclose(oracle.sh_basis([0, 0, 1.0]), [0.28209479177387814, 0, 0.4886025119029199, 0, 0, 0,
+                                                             0.6307831305050401, 0, 0], atol=1e-15)
+    np.testing.assert_allclose(oracle.sh_basis([1.0, 0, 0]), [0.28209479177387814, 0, 0, -0.4886025119029199, 0, 0,
+                                                             -0.31539156525252005, 0, 0.5462742152960396], atol=1e-15)
+    # orthonormality on the sphere (Monte Carlo): (4 pi / n) sum Y_a Y_b ~ delta_ab
+    dd = rng.standard_normal((400000, 3)); dd /= np.linalg.norm(dd, axis=1, keepdims=True)
+    Y = oracle.sh_basis(dd)
+    np.testing.assert_allclose(4 * np.pi * (Y.T @ Y) / len(dd), np.eye(9), atol=0.02)
+
+
+def test_sh_features_and_adjoint():
+    cam = Camera(**TINY)
+    R, t = second_pose()
+    cam = cam.with_pose(R, t)
+    rng = np.random.default_rng(12)
+    pos = rng.uniform(-1, 1, (50, 3)) + [0, 0, 4]
+    coeff = rng.standard_normal((50, 36))
+    f = oracle.sh_features(pos, coeff, cam)
+    # a coefficient vector that is non-zero only in the constant term gives C0 * that term, whatever the direction
+    c0 = np.zeros((50, 36)); c0[:, :4] = coeff[:, :4]
+    np.testing.assert_allclose(oracle.sh_features(pos, c0, cam), 0.28209479177387814 * coeff[:, :4], atol=1e-15)
+    # the camera centre is -R^T t: a point there sees the constant term only
+    centre = -np.asarray(R, np.float64).T @ np.asarray(t, np.float64)
+    np.testing.assert_allclose(oracle.sh_features([centre], coeff[:1], cam), 0.28209479177387814 * coeff[:1, :4], atol=1e-12)
+    # linear in the coefficients; sh_backward is the exact adjoint
+    g = rng.standard_normal((50, 4))
+    assert abs((f * g).sum() - (oracle.sh_backward(pos, cam, g) * coeff).sum()) < 1e-10
+
+
 def test_general_stack_formula():
     rng = np.random.default_rng(5)
     n = 12
