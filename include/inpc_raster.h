@@ -205,6 +205,25 @@ int inpc_raster_get_sorted(const void* workspace, int32_t W, int32_t H, uint32_t
 /* Fills *stats (host) from the workspace of the last forward; synchronises the stream. */
 int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_stream);
 
+/* ---- NEXT row f4: view-specific sampling of the implicit point cloud, the rasterizer's upstream neighbour
+ * (Sec. 3.2, Eq. 4; depth Eq. 9; frustum re-sampling PAPER.md:322). -------------
+ * Leaves of the probability octree: leaf_centre[L][3] (world), leaf_level[L] (side = root_side / 2^level),
+ * leaf_prob[L] in [0,1]; L <= 2^24 (the paper's 256^3 cap).  Each leaf gets the weight
+ *   p^ = visible * p / (d * 2^(level * 0.5)),   d = max(|z_view - near| / (far - near), 1e-8)
+ * (visible: its centre or one of its corners is inside the view frustum), N leaves are drawn with replacement
+ * from p^ / sum p^ (inverse CDF), each draw is offset uniformly inside its leaf, and a position outside the
+ * frustum is drawn again (up to 8 times; then pos = NaN, leaf = -1: the rasterizer culls it).
+ * pos[N][3] and leaf[N] are outputs; the result is a pure function of the inputs and `seed` (counter-based
+ * SplitMix64, integer CDF; csrc/sampler.cuh states the exact arithmetic), bit-reproducible on any device.
+ * workspace: inpc_sample_workspace_bytes(L) bytes, 256-byte aligned.  inpc_sample_get_stats synchronises and
+ * returns how many samples are valid, the integer CDF total and max p^ of the last call on that workspace. */
+size_t inpc_sample_workspace_bytes(int64_t n_leaves);
+int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
+                     float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+int inpc_sample_get_stats(const void* workspace, uint64_t* n_valid, uint64_t* cdf_total, double* max_weight,
+                          void* cuda_stream);
+
 const char* inpc_raster_strerror(int status);
 /* CUDA error string of the last INPC_ERR_CUDA on this thread ("" if none). */
 const char* inpc_raster_last_cuda_error(void);

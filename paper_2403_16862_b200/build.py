@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libinpc_raster.so")
 SOURCES = ["inpc_raster.cu"]
-HEADERS = ["common.cuh", "bin.cuh", "cellsort.cuh", "tile.cuh", "blend.cuh", "back.cuh", "big.cuh", "grad.cuh", os.path.join("..", "..", "include", "inpc_raster.h")]
+HEADERS = ["common.cuh", "bin.cuh", "cellsort.cuh", "tile.cuh", "blend.cuh", "back.cuh", "big.cuh", "grad.cuh", "sh.cuh", "sampler.cuh", os.path.join("..", "..", "include", "inpc_raster.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

@@ -23,6 +23,7 @@
 #include "cellsort.cuh"
 #include "common.cuh"
 #include "grad.cuh"
+#include "sampler.cuh"
 #include "tile.cuh"
 
 namespace inpc {
@@ -803,6 +804,75 @@ int inpc_raster_get_sorted(const void* workspace, int32_t W, int32_t H, uint32_t
             INPC_CUDA(cudaMemcpyAsync(transmittance, ws + L.sorted_T, (size_t)h.n_fragments * 4, cudaMemcpyDeviceToDevice, st));
     }
     INPC_CUDA(cudaStreamSynchronize(st));
+    return INPC_OK;
+}
+
+// ---- NEXT row f4: view-specific sampling (sampler.cuh) ---------------------------------------------------------------
+struct SampleLayout { size_t head, phat, cdf, tiles, total; uint32_t n_tiles; };
+static SampleLayout sample_layout(int64_t L) {
+    SampleLayout S{};
+    S.n_tiles = (uint32_t)((L + kScan64Tile - 1) / kScan64Tile);
+    size_t o = 0;
+    S.head = o;  o = align_up(o + 64);                       // max_bits, total, n_valid
+    S.phat = o;  o = align_up(o + (size_t)L * 8);
+    S.cdf = o;   o = align_up(o + (size_t)L * 8);
+    S.tiles = o; o = align_up(o + ((size_t)S.n_tiles + 1) * 8);
+    S.total = o;
+    return S;
+}
+
+size_t inpc_sample_workspace_bytes(int64_t n_leaves) {
+    if (n_leaves < 1 || n_leaves > (1ll << 24)) return 0;
+    return sample_layout(n_leaves).total;
+}
+
+int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
+                     float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!cam || !leaf_centre || !leaf_level || !leaf_prob || !workspace || N < 0 || N >= (1ll << 31)) return INPC_ERR_INVALID_ARG;
+    if (n_leaves < 1 || n_leaves > (1ll << 24) || !(root_side > 0.f)) return INPC_ERR_INVALID_ARG;
+    if (cam->width <= 0 || cam->height <= 0 || !(cam->near_z < cam->far_z)) return INPC_ERR_INVALID_ARG;
+    if (N > 0 && (!pos || !leaf)) return INPC_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(workspace) & 255u) return INPC_ERR_INVALID_ARG;
+    const SampleLayout S = sample_layout(n_leaves);
+    if (workspace_bytes < S.total) return INPC_ERR_WORKSPACE_TOO_SMALL;
+    const DeviceInfo di = device_info();
+    if (!di.ok) return cuda_fail(cudaErrorNoDevice);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    unsigned long long* head = reinterpret_cast<unsigned long long*>(ws + S.head);
+    double* phat = reinterpret_cast<double*>(ws + S.phat);
+    unsigned long long* cdf = reinterpret_cast<unsigned long long*>(ws + S.cdf);
+    unsigned long long* tiles = reinterpret_cast<unsigned long long*>(ws + S.tiles);
+    const Camera camk = to_camera(cam);
+    const uint32_t L = (uint32_t)n_leaves;
+    INPC_CUDA(cudaMemsetAsync(head, 0, 64, st));
+    k_leaf_weight<<<std::min<uint32_t>((L + 255) / 256, (uint32_t)di.sms * 8), 256, 0, st>>>(leaf_centre, leaf_level, leaf_prob, L,
+                                                                                            root_side, camk, phat, head);
+    INPC_LAUNCHED("k_leaf_weight");
+    k_cdf_local<<<S.n_tiles, kScan64Threads, 0, st>>>(phat, L, head, cdf, tiles);
+    INPC_LAUNCHED("k_cdf_local");
+    k_cdf_tiles<<<1, 1024, 0, st>>>(tiles, S.n_tiles, head + 1);
+    INPC_LAUNCHED("k_cdf_tiles");
+    k_cdf_add<<<S.n_tiles, kScan64Threads, 0, st>>>(cdf, L, tiles);
+    INPC_LAUNCHED("k_cdf_add");
+    if (N > 0) {
+        k_sample<<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 8), 256, 0, st>>>(
+            cdf, L, head + 1, leaf_centre, leaf_level, root_side, camk, (unsigned long long)seed, (long long)N, pos, leaf, head + 2);
+        INPC_LAUNCHED("k_sample");
+    }
+    return INPC_OK;
+}
+
+int inpc_sample_get_stats(const void* workspace, uint64_t* n_valid, uint64_t* cdf_total, double* max_weight, void* cuda_stream) {
+    if (!workspace) return INPC_ERR_INVALID_ARG;
+    unsigned long long h[3];
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    INPC_CUDA(cudaMemcpyAsync(h, workspace, sizeof(h), cudaMemcpyDeviceToHost, st));
+    INPC_CUDA(cudaStreamSynchronize(st));
+    if (max_weight) { double m; std::memcpy(&m, &h[0], 8); *max_weight = m; }
+    if (cdf_total) *cdf_total = h[1];
+    if (n_valid) *n_valid = h[2];
     return INPC_OK;
 }
 

@@ -25,6 +25,7 @@ EXPORTS = (
     "inpc_raster_workspace_bytes", "inpc_raster_forward", "inpc_raster_backward", "inpc_raster_backward_weights",
     "inpc_raster_forward_ex", "inpc_raster_backward_ex", "inpc_raster_level_camera", "inpc_raster_forward_levels",
     "inpc_raster_forward_multisample", "inpc_raster_forward_sh", "inpc_raster_backward_sh",
+    "inpc_sample_workspace_bytes", "inpc_sample_view", "inpc_sample_get_stats",
     "inpc_raster_get_counts", "inpc_raster_get_blended_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
     "inpc_raster_get_status",
     "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count", "inpc_raster_launched_kernels",
@@ -81,6 +82,12 @@ def load() -> C.CDLL:
         lib.inpc_raster_forward_sh.argtypes = [vp, vp, vp, i64, C.POINTER(InpcCamera), vp, vp, vp, C.c_size_t, u32, C.c_float, vp]
         lib.inpc_raster_backward_sh.restype = C.c_int
         lib.inpc_raster_backward_sh.argtypes = [vp, vp, vp, i64, C.POINTER(InpcCamera), vp, vp, vp, vp, vp, vp, vp, C.c_size_t, u32, C.c_float, vp]
+        lib.inpc_sample_workspace_bytes.restype = C.c_size_t
+        lib.inpc_sample_workspace_bytes.argtypes = [i64]
+        lib.inpc_sample_view.restype = C.c_int
+        lib.inpc_sample_view.argtypes = [vp, vp, vp, i64, C.c_float, C.POINTER(InpcCamera), C.c_uint64, i64, vp, vp, vp, C.c_size_t, vp]
+        lib.inpc_sample_get_stats.restype = C.c_int
+        lib.inpc_sample_get_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_double), vp]
         lib.inpc_raster_level_camera.restype = C.c_int
         lib.inpc_raster_level_camera.argtypes = [C.POINTER(InpcCamera), i32, C.POINTER(InpcCamera)]
         lib.inpc_raster_forward_levels.restype = C.c_int
@@ -212,6 +219,33 @@ def inpc_raster_forward_multisample(clouds, cam, n_levels: int = 1, flags: int =
     if rc != 0:
         raise InpcError(rc, "inpc_raster_forward_multisample")
     return imgs, alphas
+
+
+def inpc_sample_view(leaf_centre, leaf_level, leaf_prob, root_side: float, cam, seed: int, N: int, workspace=None, stream=None):
+    """View-specific sampling (Eq. 4): -> (pos[N,3] float32, leaf[N] int32, workspace).  No sync."""
+    lib = load()
+    _check(leaf_centre, torch.float32, "leaf_centre"); _check(leaf_level, torch.int32, "leaf_level")
+    _check(leaf_prob, torch.float32, "leaf_prob")
+    L = int(leaf_level.shape[0])
+    dev = leaf_centre.device
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    if workspace is None:
+        workspace = torch.empty(int(lib.inpc_sample_workspace_bytes(L)), dtype=torch.uint8, device=dev)
+    pos = torch.empty((N, 3), dtype=torch.float32, device=dev)
+    leaf = torch.empty((N,), dtype=torch.int32, device=dev)
+    rc = lib.inpc_sample_view(_ptr(leaf_centre), _ptr(leaf_level), _ptr(leaf_prob), L, float(root_side), C.byref(cs),
+                              C.c_uint64(seed), N, _ptr(pos), _ptr(leaf), _ptr(workspace), workspace.numel(), _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_sample_view")
+    return pos, leaf, workspace
+
+
+def inpc_sample_get_stats(workspace, stream=None) -> dict:
+    nv, tot, mx = C.c_uint64(0), C.c_uint64(0), C.c_double(0.0)
+    rc = load().inpc_sample_get_stats(_ptr(workspace), C.byref(nv), C.byref(tot), C.byref(mx), _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_sample_get_stats")
+    return {"n_valid": int(nv.value), "cdf_total": int(tot.value), "max_weight": float(mx.value)}
 
 
 def inpc_raster_forward_sh(pos, opacity, sh_coeff, cam, flags: int = SAVE_FOR_BACKWARD, out_scale: float = 1.0, stream=None):

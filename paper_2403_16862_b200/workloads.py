@@ -210,3 +210,23 @@ def make_workload(name: str, n_points: int | None = None, seed: int | None = Non
                     feat=np.ascontiguousarray(feat, dtype=np.float32),
                     cam=cam, g_img=g_img, g_alpha=g_alpha,
                     backward=bool(cfg["backward"]), seed=seed)
+
+
+def make_octree(n_leaves: int = 1 << 16, seed: int = 7, cam: dict = CAM_1297, root_side: float = 64.0):
+    """Synthetic probability octree for the view-specific sampler (NEXT row f4; PAPER.md:62-84 describes the real
+    one, which needs the optimisation loop): leaves of levels 4..12 of the root cube [-32,32]^2 x [0,64] placed on
+    the surface generator (so most are in front of the camera), a tenth of them mirrored behind the camera or pushed
+    out of the frustum (to exercise the visibility indicator), probabilities U[0.02, 1].
+    -> (centre[L,3] f32, level[L] i32, prob[L] f32, root_side)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    s = _rejection(_surface_once, rng, n_leaves, cam, 0.5, 50.0)
+    out = rng.uniform(0, 1, n_leaves) < 0.1
+    s[out, 2] *= np.where(rng.uniform(0, 1, out.sum()) < 0.5, -1.0, 1.0)      # behind the camera ...
+    s[out, 0] += np.where(s[out, 2] > 0, 40.0, 0.0)                            # ... or far off to the side
+    level = rng.integers(4, 13, n_leaves)
+    side = root_side / np.exp2(level)
+    origin = np.array([-root_side / 2, -root_side / 2, 0.0])
+    centre = (np.floor((s - origin) / side[:, None]) + 0.5) * side[:, None] + origin
+    prob = rng.uniform(0.02, 1.0, n_leaves)
+    return (np.ascontiguousarray(centre, dtype=np.float32), np.ascontiguousarray(level, dtype=np.int32),
+            np.ascontiguousarray(prob, dtype=np.float32), float(root_side))

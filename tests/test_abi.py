@@ -26,7 +26,7 @@ def _declared_symbols():
         if fn.endswith(".h"):
             src = open(os.path.join(inc, fn)).read()
             src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-            names |= set(re.findall(r"\b(inpc_raster_\w+)\s*\(", src))
+            names |= set(re.findall(r"\b(inpc_(?:raster|sample)_\w+)\s*\(", src))
     return names
 
 

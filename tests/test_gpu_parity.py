@@ -355,6 +355,50 @@ def test_fused_sh_forward_and_backward(name, kw, pose):
         assert float(g_c.cpu().numpy()[dead].__abs__().max()) == 0.0
 
 
+# ------------------------------------------------------------------------------ NEXT row f4: view-specific sampler
+
+@pytest.mark.parametrize("n_leaves,N,pose", [(4096, 100_000, False), (1 << 16, 1 << 20, True), (1 << 20, 1 << 22, False)])
+def test_view_specific_sampler_is_bit_exact(n_leaves, N, pose):
+    """Eq. 4 re-weighting, multinomial with replacement, in-leaf jitter, frustum re-sampling:
+    the drawn leaf indices and the fp32 positions against oracle/sampler.py, bit for bit."""
+    from oracle import sampler as osampler
+    from paper_2403_16862_b200.workloads import make_octree
+    centre, level, prob, root = make_octree(n_leaves, seed=21)
+    cam = make_workload("tiny").cam.__class__(fx=1100.0, fy=1100.0, cx=648.5, cy=420.0, width=1297, height=840)
+    if pose:
+        cam = cam.with_pose(*second_pose())
+    pos, leaf, ws = raster.inpc_sample_view(_dev(centre), _dev(level), _dev(prob), root, cam, seed=2024, N=N)
+    torch.cuda.synchronize()
+    rpos, rleaf = osampler.sample_view(centre, level, prob, root, cam, seed=2024, N=N)
+    assert np.array_equal(leaf.cpu().numpy(), rleaf), "drawn leaf indices differ"
+    assert np.array_equal(pos.cpu().numpy().view(np.uint32)[rleaf >= 0], rpos.view(np.uint32)[rleaf >= 0]), "positions differ"
+    assert np.isnan(pos.cpu().numpy()[rleaf < 0]).all()
+    st = raster.inpc_sample_get_stats(ws)
+    cdf = osampler.integer_cdf(osampler.leaf_weights(centre, level, prob, root, cam))
+    assert st["n_valid"] == int((rleaf >= 0).sum()) and st["cdf_total"] == int(cdf[-1])
+    assert st["max_weight"] == float(osampler.leaf_weights(centre, level, prob, root, cam).max())
+    # the sampled cloud goes straight into the rasterizer: every valid sample lands in the image
+    n = min(N, 1 << 20)
+    op = torch.full((n,), 0.3, device="cuda"); feat = torch.rand((n, 4), device="cuda")
+    _, alpha, rws = raster.inpc_raster_forward(pos[:n].contiguous(), op, feat, cam, flags=0)
+    assert raster.inpc_raster_get_stats(rws)["n_kept"] == int((rleaf[:n] >= 0).sum())
+
+
+def test_sampler_edge_cases():
+    from paper_2403_16862_b200.workloads import make_octree
+    cam = make_workload("tiny").cam
+    centre = torch.tensor([[0.0, 0.0, -5.0]], device="cuda"); level = torch.tensor([8], dtype=torch.int32, device="cuda")
+    prob = torch.tensor([1.0], device="cuda")
+    pos, leaf, ws = raster.inpc_sample_view(centre, level, prob, 64.0, cam, seed=1, N=100)      # nothing visible
+    torch.cuda.synchronize()
+    assert (leaf == -1).all() and torch.isnan(pos).all() and raster.inpc_sample_get_stats(ws)["cdf_total"] == 0
+    pos, leaf, ws = raster.inpc_sample_view(centre, level, prob, 64.0, cam, seed=1, N=0)        # N = 0
+    assert pos.shape == (0, 3)
+    with pytest.raises(raster.InpcError) as e:
+        raster.inpc_sample_view(centre, level, prob, -1.0, cam, seed=1, N=10)
+    assert e.value.status == -1
+
+
 # ------------------------------------------------------------------------------ API behaviour
 
 def test_forward_is_repeatable_and_workspace_reusable():
