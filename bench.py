@@ -388,6 +388,73 @@ def workload_statistics(raster, wl, T, dev) -> dict:
 
 
 # ------------------------------------------------------------------------------------------------
+def next_rows(raster, wl, T, dev, stream, reps: int = 10) -> dict:
+    """Timings of the NEXT rows of the scope table on the same workload, outside the headline:
+    f1 blending weights fused into the backward pass, f2 SH fused into the emission pass, f3 three resolution levels
+    and four-cloud multisampling, f4 the view-specific sampler.  CUDA events, 3 warm-ups, mean of `reps`."""
+    import numpy as np
+    import torch
+    from paper_2403_16862_b200.workloads import make_octree
+    N, D, W, H = wl.N, wl.D, wl.cam.width, wl.cam.height
+    cam = T["cam"]
+
+    def ms(fn):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    out = {}
+    pos, op, feat, g_img, g_alpha, ws = T["pos"], T["op"], T["feat"], T["g_img"], T["g_alpha"], T["ws"]
+    raster.inpc_raster_forward(pos, op, feat, cam, out_feat=T["img"], out_alpha=T["alpha"], workspace=ws, flags=FLAGS_STEP)
+    bw = torch.empty((N,), dtype=torch.float32, device=dev)
+    t_plain = ms(lambda: raster.inpc_raster_backward(pos, op, feat, cam, g_img, g_alpha, ws, grad_feat=T["d_feat"],
+                                                     grad_opacity=T["d_op"], grad_uv=T["d_uv"]))
+    t_w = ms(lambda: raster.inpc_raster_backward(pos, op, feat, cam, g_img, g_alpha, ws, grad_feat=T["d_feat"],
+                                                 grad_opacity=T["d_op"], grad_uv=T["d_uv"], blend_weight=bw))
+    out["f1_blend_weights"] = {"ms_backward": t_plain, "ms_backward_with_weights": t_w, "extra_bytes_per_point": 4}
+    if D == 4:
+        coeff = torch.randn((N, 36), dtype=torch.float32, device=dev) * 0.5
+        st = {}
+
+        def f_sh():
+            st["o"] = raster.inpc_raster_forward_sh(pos, op, coeff, cam, flags=FLAGS_STEP)
+
+        def b_sh():
+            raster.inpc_raster_backward_sh(pos, op, coeff, cam, g_img, g_alpha, st["o"][2])
+
+        t_f = ms(f_sh)
+        t_b = ms(b_sh)
+        out["f2_fused_sh"] = {"ms_forward": t_f, "ms_backward": t_b, "coefficient_bytes_per_point": 144,
+                              "note": "includes the allocation of outputs / workspace by the binding in every call"}
+        del coeff, st
+    t_l = ms(lambda: raster.inpc_raster_forward_levels(pos, op, feat, cam, 3, flags=FLAGS_FWD))
+    out["f3_three_levels_forward"] = {"ms": t_l, "note": "levels 0, 1, 2 of one cloud, forward only (binding allocates per call)"}
+    clouds = [(pos, op, feat)] * 4
+    t_m = ms(lambda: raster.inpc_raster_forward_multisample(clouds, cam, n_levels=1, flags=raster.OUT_PLANAR))
+    out["f3_multisample_4_clouds"] = {"ms": t_m, "splats": 16 * N,
+                                      "note": "four clouds of N points averaged per pixel, [D,H,W] output (PAPER.md:172: 8M x 4 x 4 = 128 M splats)"}
+    centre, level, prob, root = make_octree(1 << 20, seed=21)
+    dc, dl, dp = (torch.from_numpy(a).to(dev) for a in (centre, level, prob))
+    sws = {}
+
+    def f_s():
+        sws["o"] = raster.inpc_sample_view(dc, dl, dp, root, cam, seed=7, N=N, workspace=sws.get("w"))
+        sws["w"] = sws["o"][2]
+
+    t_s = ms(f_s)
+    out["f4_sampler"] = {"ms": t_s, "leaves": 1 << 20, "samples": N, "samples_per_sec": N / (t_s * 1e-3),
+                         "valid": raster.inpc_sample_get_stats(sws["w"])["n_valid"]}
+    return out
+
+
+# ------------------------------------------------------------------------------------------------
 def run_ours(args) -> int:
     import numpy as np
     import torch
@@ -658,6 +725,8 @@ def run_ours(args) -> int:
                          f"inputs fit L2: {n_sets} independent buffer sets ({n_sets * set_bytes >> 20} MiB) rotated, one per step"},
         "clocks": clock_info,
     }
+    if world == 1 and wl.backward and not args.no_next_rows:
+        line["next_rows"] = next_rows(raster, wl, T, dev, stream)
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(wl)
         line["cpu_baseline_all_cores"] = cpu_baseline(wl, openmp=True)
@@ -677,6 +746,7 @@ def main(argv=None) -> int:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle leg (profiling runs)")
     ap.add_argument("--no-stats", action="store_true", help="skip the workload statistics (profiling runs)")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the timings of the NEXT rows f1-f4 (profiling runs)")
     ap.add_argument("--print-source-hash", action="store_true", help="print the kernel-source hash a traffic capture is recorded with")
     args = ap.parse_args(argv)
     if args.print_source_hash:

@@ -292,43 +292,74 @@ struct BandPlan {
     uint32_t item_base[kMaxBands];       // start of the band's item list inside items[]
 };
 
+// Two passes over the same DFS: the first counts what the thread's base tile will emit, the warp then reserves the
+// slots of all its lanes with ONE atomic per list (thousands of single-slot atomics on one address serialise:
+// 122 us on the stress workload), the second writes.
 __global__ void __launch_bounds__(128) k_build_items(const uint32_t* __restrict__ celloff, int W, int H, int cap,
                                                       BandPlan plan, Header* __restrict__ hdr,
                                                       uint32_t* __restrict__ items_all, uint32_t* __restrict__ bigpix) {
     const int ntx = (W + kTileW - 1) / kTileW, nty = (H + kTileH - 1) / kTileH;
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= ntx * nty) return;
-    const int X0 = (t % ntx) * kTileW, Y0 = (t / ntx) * kTileH;
-    const int band = min((t / ntx) / plan.rows_per_band, plan.n_bands - 1);
+    const bool live = t < ntx * nty;
+    const int tt = live ? t : 0;
+    const int X0 = (tt % ntx) * kTileW, Y0 = (tt / ntx) * kTileH;
+    const int band = min((tt / ntx) / plan.rows_per_band, plan.n_bands - 1);
     uint32_t* items = items_all + plan.item_base[band];
-    uint32_t* n_items = &hdr->band_items[band];
-    uint32_t stack[12];                                  // binary DFS: depth <= 7, one sibling pending per level
-    int sp = 0;
-    stack[sp++] = encode_item(X0, Y0, kTileLW, kTileLH);
-    while (sp > 0) {
-        const uint32_t it = stack[--sp];
-        const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
-        if (X >= W || Y >= H) continue;
-        const int tw = 1 << lw, th = 1 << lh;
-        const uint32_t n = tile_padded_records(celloff, W, H, X, Y, tw, th);
-        if (n <= (uint32_t)cap) {
-            items[atomicAdd(n_items, 1u)] = it;          // empty tiles too: their pixels must be zeroed
-            continue;
+    uint32_t n_it = 0, n_bp = 0, at_it = 0, at_bp = 0;
+    unsigned long long n_bf = 0;
+    const int lane = threadIdx.x & 31;
+    for (int pass = 0; pass < 2; ++pass) {
+        uint32_t stack[12];                              // binary DFS: depth <= 7, one sibling pending per level
+        int sp = 0;
+        if (live) stack[sp++] = encode_item(X0, Y0, kTileLW, kTileLH);
+        while (sp > 0) {
+            const uint32_t it = stack[--sp];
+            const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
+            if (X >= W || Y >= H) continue;
+            const int tw = 1 << lw, th = 1 << lh;
+            const uint32_t n = tile_padded_records(celloff, W, H, X, Y, tw, th);
+            if (n <= (uint32_t)cap) {                    // empty tiles too: their pixels must be zeroed
+                if (pass == 0) ++n_it; else items[at_it++] = it;
+                continue;
+            }
+            if (tw * th <= kMinTilePix) {
+                for (int y = Y; y < min(Y + th, H); ++y)
+                    for (int x = X; x < min(X + tw, W); ++x) {
+                        if (pass == 0) { ++n_bp; n_bf += pixel_count(celloff, W, x, y); }
+                        else bigpix[at_bp++] = (uint32_t)(y * W + x);
+                    }
+                continue;
+            }
+            if (lw >= lh + 1 || lh == 0) {               // split the wider side (tiles are kept ~2:1)
+                stack[sp++] = encode_item(X + (tw >> 1), Y, lw - 1, lh);
+                stack[sp++] = encode_item(X, Y, lw - 1, lh);
+            } else {
+                stack[sp++] = encode_item(X, Y + (th >> 1), lw, lh - 1);
+                stack[sp++] = encode_item(X, Y, lw, lh - 1);
+            }
         }
-        if (tw * th <= kMinTilePix) {
-            for (int y = Y; y < min(Y + th, H); ++y)
-                for (int x = X; x < min(X + tw, W); ++x) {
-                    bigpix[atomicAdd(&hdr->n_big_pixels, 1u)] = (uint32_t)(y * W + x);
-                    atomicAdd(&hdr->n_big_fragments, (unsigned long long)pixel_count(celloff, W, x, y));
+        if (pass == 0) {
+            // warp-wide reservation; lanes of one warp may belong to different bands (a warp spans at most two tile rows
+            // worth of base tiles only when ntx < 32): reserve per band among the lanes that share it
+            const uint32_t peers = __match_any_sync(0xffffffffu, band);
+            uint32_t inc_it = 0, inc_bp = 0, tot_it = 0, tot_bp = 0;
+            unsigned long long tot_bf = 0;
+            for (int l = 0; l < 32; ++l) {
+                const uint32_t a = __shfl_sync(0xffffffffu, n_it, l), b = __shfl_sync(0xffffffffu, n_bp, l);
+                const unsigned long long c = __shfl_sync(0xffffffffu, n_bf, l);
+                if ((peers >> l) & 1u) {
+                    if (l < lane) { inc_it += a; inc_bp += b; }
+                    tot_it += a; tot_bp += b; tot_bf += c;
                 }
-            continue;
-        }
-        if (lw >= lh + 1 || lh == 0) {                   // split the wider side (tiles are kept ~2:1)
-            stack[sp++] = encode_item(X + (tw >> 1), Y, lw - 1, lh);
-            stack[sp++] = encode_item(X, Y, lw - 1, lh);
-        } else {
-            stack[sp++] = encode_item(X, Y + (th >> 1), lw, lh - 1);
-            stack[sp++] = encode_item(X, Y, lw, lh - 1);
+            }
+            const int leader = __ffs(peers) - 1;
+            uint32_t base_it = 0, base_bp = 0;
+            if (lane == leader) {
+                if (tot_it) base_it = atomicAdd(&hdr->band_items[band], tot_it);
+                if (tot_bp) { base_bp = atomicAdd(&hdr->n_big_pixels, tot_bp); atomicAdd(&hdr->n_big_fragments, tot_bf); }
+            }
+            at_it = __shfl_sync(0xffffffffu, base_it, leader) + inc_it;
+            at_bp = __shfl_sync(0xffffffffu, base_bp, leader) + inc_bp;
         }
     }
 }

@@ -21,7 +21,7 @@
 namespace inpc {
 
 constexpr int kGradThreads = 256;
-constexpr int kGradCells   = 1024;
+constexpr int kGradCells   = 128;      // cells per work unit: small, so that a unit full of deep cells does not become one CTA's tail
 
 template <int D> __host__ __device__ constexpr int gpt_floats() { return D == 4 ? 8 : 16; }
 
@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
             const int x0 = i - 1, y0 = j - 1;
             // every gather of the four corner pixels is issued before any of them is used
             uint4 cur[4];
-            float gp[4][D];
+            float4 gp[4][D / 4];
             bool in[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -68,11 +68,12 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                 in[c] = px >= 0 && px < W && py >= 0 && py < H;               // else: fragment does not exist
                 const size_t pp = in[c] ? (size_t)py * W + px : 0;
                 cur[c] = in[c] ? __ldg(&pcur[pp]) : make_uint4(0, 0, 0, 0);
-                float unused;
-                if (in[c]) load_pixel_grad<D>(io, g_feat, nullptr, pp, gp[c], unused);
-                else {
 #pragma unroll
-                    for (int d = 0; d < D; ++d) gp[c][d] = 0.f;
+                for (int v = 0; v < D / 4; ++v) {
+                    if (!in[c]) gp[c][v] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    else if (!io.planar) gp[c][v] = __ldg(reinterpret_cast<const float4*>(g_feat + pp * D) + v);
+                    else gp[c][v] = make_float4(__ldg(g_feat + (size_t)(4 * v) * io.P + pp), __ldg(g_feat + (size_t)(4 * v + 1) * io.P + pp),
+                                                __ldg(g_feat + (size_t)(4 * v + 2) * io.P + pp), __ldg(g_feat + (size_t)(4 * v + 3) * io.P + pp));
                 }
             }
             const float tc[4] = {t4.x, t4.y, t4.z, t4.w}, dc[4] = {d4.x, d4.y, d4.z, d4.w};
@@ -92,8 +93,12 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                 dop += wx * wy * dl;
                 du += (dx ? wy : -wy) * dl;
                 dv += (dy ? wx : -wx) * dl;
+                const float Tg = io.scale * Ta;                            // the gradient image's scale, applied once (1: exact)
 #pragma unroll
-                for (int d = 0; d < D; ++d) df[d] += Ta * gp[c][d];
+                for (int v = 0; v < D / 4; ++v) {
+                    const float4 t = gp[c][v];
+                    df[4 * v] += Tg * t.x; df[4 * v + 1] += Tg * t.y; df[4 * v + 2] += Tg * t.z; df[4 * v + 3] += Tg * t.w;
+                }
             }
             du *= r0.z; dv *= r0.z;
             float4* out = reinterpret_cast<float4*>(gpt + (size_t)__float_as_uint(r0.w) * GP);

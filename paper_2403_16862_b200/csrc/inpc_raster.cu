@@ -524,8 +524,10 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
         if (u1 > u0) {
             INPC_CUDA(fork(st, s2));                                          // band b is walked: combine its cells
             { StageTimer tm(kStCombine, s2);
-              k_combine<D><<<(int)std::min<uint32_t>(u1 - u0, (uint32_t)di.sms * 8), kGradThreads, 0, s2>>>(
-                  hdr, celloff, L.C, u0, u1, W, H, Ra, reinterpret_cast<const float4*>(gT),
+              constexpr uint32_t kSub = kCsCells / kGradCells;               // the band plan counts kCsCells-cell units
+              const uint32_t g0 = u0 * kSub, g1 = std::min<uint32_t>(u1 * kSub, (L.C + kGradCells - 1) / kGradCells);
+              k_combine<D><<<(int)std::min<uint32_t>(g1 - g0, (uint32_t)di.sms * 8), kGradThreads, 0, s2>>>(
+                  hdr, celloff, L.C, g0, g1, W, H, Ra, reinterpret_cast<const float4*>(gT),
                   reinterpret_cast<const float4*>(gD), pcur, g_feat, io, gpt); }
             INPC_LAUNCHED(kname<D>("k_combine"));
             u0 = u1;
