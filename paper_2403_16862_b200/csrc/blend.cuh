@@ -14,7 +14,10 @@
 //      head key selects the list with predicates, and only "two heads with equal depth bits" (ascending
 //      point index decides, read from global memory) and the two loop exits are branches.
 // With INPC_SAVE_FOR_BACKWARD the transmittance in front of every blended fragment goes to
-// gT[(slot, corner)] and the four list positions at the stop to pcur[pixel].
+// gT[(slot, corner)], the four list positions at the stop to pcur[pixel], and the ORDER itself to
+// ord[pixoff[pixel] + k] = which staged (record, corner) was blended k-th (16 bits: the fragment's byte offset
+// record * 16 + 4 * corner inside the tile's staged records) -- the backward pass stages the same tile the same
+// way and walks that list backwards without merging anything again (back.cuh).
 #pragma once
 #include "common.cuh"
 
@@ -35,15 +38,17 @@ struct BlendArgs {
     ImageIO io;
     float* gT;               // NULL unless INPC_SAVE_FOR_BACKWARD
     uint4* pcur;
+    uint16_t* ord;           // blend order of every pixel (INPC_SAVE_FOR_BACKWARD), indexed through pixoff
+    const uint32_t* pixoff;  // exclusive scan of the per-pixel fragment counts (save or dump)
     // dump (INPC_SAVE_SORTED)
-    const uint32_t* pixoff;
     uint32_t* sorted_idx;
     uint32_t* sorted_depth;
     float* sorted_T;         // transmittance in front of every blended fragment, -1 behind the cut-off
 };
 
-template <int D> __host__ __device__ constexpr size_t blend_smem_bytes() {
-    return (size_t)TileCfg<D>::kCap * (4 + 16 + 4 * D);
+// per staged record: depth key, alphas, features; with SAVE also the tile's order lists (2 bytes per fragment)
+template <int D, bool SAVE> __host__ __device__ constexpr size_t blend_smem_bytes() {
+    return (size_t)TileCfg<D>::kCap * (4 + 16 + 4 * D + (SAVE ? 8 : 0));
 }
 
 // Packed list state: low 16 bits = byte offset of the head fragment's alpha inside s_a (record * 16 +
@@ -66,6 +71,11 @@ __device__ __forceinline__ uint32_t pack_list(uint32_t start_rec, uint32_t end_r
         p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;                                                           \
     } while (0)
 
+#ifdef INPC_EXP_NO_STS
+#define INPC_EXP_STS(a, v)
+#else
+#define INPC_EXP_STS(a, v) sts_u16(a, v)
+#endif
 template <int D, bool SAVE, bool DUMP>
 __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
     constexpr int FV  = D / 4;                     // float4 of features per record
@@ -75,6 +85,9 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
     float4*   s_a4 = reinterpret_cast<float4*>(smem + (size_t)CAP * 4);
     float4*   s_f  = reinterpret_cast<float4*>(smem + (size_t)CAP * 20);
     const unsigned char* s_ab = smem + (size_t)CAP * 4;
+    uint16_t* s_ord = reinterpret_cast<uint16_t*>(smem + (size_t)CAP * (20 + 16 * FV));   // SAVE only
+    __shared__ uint32_t s_pixbase[kTileThreads], s_wsum[kTileThreads / 32], s_ordtot;     // SAVE: starts of the tile's order lists
+    __shared__ uint32_t s_rowg[kTileH];                                                   // ... and of its pixel rows' runs in ord[]
 
     __shared__ uint32_t s_off[kTileH + 1][kTileW + 2];
     __shared__ uint32_t s_sbase[kTileH + 1], s_a4row[kTileH + 1];
@@ -93,15 +106,32 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
         s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
     }
     uint32_t parity = 0;
+    bool have_prev = false;                               // SAVE: the previous item's order lists still sit in shared memory
+    int pX = 0, pY = 0, plw = 0, pth = 0;
 
     while (true) {
         __syncthreads();                                  // everyone is done with the previous item's smem
+        if constexpr (SAVE) {
+            // The previous tile's order lists go out to ord[], coalesced: pixel row r of the tile is one contiguous run
+            // both in shared memory (pixels in natural order) and in the global array (pixoff is row-major).
+#ifndef INPC_EXP_NO_COPYOUT
+            if (have_prev) {
+                for (int r = 0; r < pth && pY + r < H; ++r) {
+                    const uint32_t s0 = s_pixbase[r << plw], s1 = r + 1 < pth ? s_pixbase[(r + 1) << plw] : s_ordtot;
+                    uint16_t* dst = A.ord + s_rowg[r];
+                    for (uint32_t i = tid; i < s1 - s0; i += kTileThreads) dst[i] = s_ord[s0 + i];
+                }
+            }
+#endif
+        }
         const uint32_t item_i = s_next;
         if (item_i >= n_items) break;
         const uint32_t it = s_next_code;
         const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
         const int tw = 1 << lw, th = 1 << lh;
 
+        uint32_t rowg = 0;                                // SAVE: where pixel row `tid - 64` of this tile starts in ord[]
+        if constexpr (SAVE) { if (tid >= 64 && tid - 64 < th && Y + tid - 64 < H) rowg = __ldg(&A.pixoff[(size_t)(Y + tid - 64) * W + X]); }
         // cell offsets of the tile's (th+1) x (tw+2) window
         for (int e = tid; e < (th + 1) * (tw + 2); e += kTileThreads) {
             const int r = e / (tw + 2), c = e - r * (tw + 2);
@@ -112,6 +142,7 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
         }
         if (tid < 64) s_hist[tid] = 0;
         __syncthreads();
+        if constexpr (SAVE) { if (tid >= 64 && tid - 64 < th) s_rowg[tid - 64] = rowg; }
         if (tid == 32) {                                  // fetch the next work item while this one is processed
             const uint32_t nx = atomicAdd(A.item_cursor, 1u);
             s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
@@ -150,7 +181,21 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
             n_mine = (s_off[ly0][lx0 + 2] - s_off[ly0][lx0]) + (s_off[ly0 + 1][lx0 + 2] - s_off[ly0 + 1][lx0]);
         const uint32_t bucket = 63u - min(n_mine >> 2, 63u);          // descending count
         const uint32_t rank_in_bucket = atomicAdd(&s_hist[bucket], 1u);
+        uint32_t inc_mine = n_mine;                                    // SAVE: scan of the counts in natural pixel order
+        if constexpr (SAVE) {
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc_mine, d); if ((tid & 31) >= d) inc_mine += t; }
+            if ((tid & 31) == 31) s_wsum[tid >> 5] = inc_mine;
+        }
         __syncthreads();
+        if constexpr (SAVE) {
+            uint32_t before = 0;
+#pragma unroll
+            for (int w = 0; w < kTileThreads / 32; ++w) before += w < (tid >> 5) ? s_wsum[w] : 0u;
+            s_pixbase[tid] = before + inc_mine - n_mine;
+            if (tid == kTileThreads - 1) s_ordtot = before + inc_mine;
+            have_prev = true; pX = X; pY = Y; plw = lw; pth = th;
+        }
         if (tid < 32) {                                                // exclusive scan of the 64 buckets
             const uint32_t h0 = s_hist[2 * tid], h1 = s_hist[2 * tid + 1];
             uint32_t inc = h0 + h1;
@@ -214,6 +259,8 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
         const uint32_t sa = smem_u32(s_ab), sf = smem_u32(s_f), sk = smem_u32(s_dk);
         uint32_t kd = 0;                              // DUMP: position of the next fragment in the pixel's sorted list
         const uint32_t obase = DUMP ? A.pixoff[pix] : 0u;
+        uint32_t so = SAVE ? smem_u32(s_ord) + 2u * s_pixbase[q] : 0u;   // next entry of this pixel's order list
+        (void)so;
         uint32_t m = min(min(h0, h1), min(h2, h3));
         bool p0, p1, p2, p3;
         float aA = 0.f, aB = 0.f;
@@ -258,7 +305,7 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
                 acc[4 * v] += c * f##X[v].x; acc[4 * v + 1] += c * f##X[v].y;                                             \
                 acc[4 * v + 2] += c * f##X[v].z; acc[4 * v + 3] += c * f##X[v].w;                                         \
             }                                                                                                             \
-            if constexpr (SAVE) ((cur##X & 8u) ? gTtop : gTbot)[cur##X >> 2] = T;                                         \
+            if constexpr (SAVE) { ((cur##X & 8u) ? gTtop : gTbot)[cur##X >> 2] = T; INPC_EXP_STS(so, cur##X); so += 2u; }        \
             if constexpr (DUMP) A.sorted_T[obase + kd##X] = T;                                                            \
             T *= (1.f - a##X);                                                                                            \
         }

@@ -41,7 +41,7 @@ constexpr float kTMin      = 1e-4f; // transmittance cut-off (BASELINE.json nort
 constexpr uint32_t kSentHi = 0xFFFFFFFFu;   // "list exhausted" for the ascending merge (depth bits < 0x7F800000)
 
 template <int D> struct TileCfg;
-template <> struct TileCfg<4> { static constexpr int kCap = 1344; };   // records per tile item
+template <> struct TileCfg<4> { static constexpr int kCap = 1216; };   // records per tile item
 template <> struct TileCfg<8> { static constexpr int kCap = 1024; };
 
 struct Camera {
@@ -119,6 +119,12 @@ __device__ __forceinline__ float lds_f32(uint32_t a) {
 }
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
     uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v;
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a) {
+    uint16_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a)); return v;
+}
+__device__ __forceinline__ void sts_u16(uint32_t a, uint32_t v) {
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((uint16_t)v) : "memory");
 }
 __device__ __forceinline__ float4 lds_v4(uint32_t a) {
     float4 v; asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a)); return v;

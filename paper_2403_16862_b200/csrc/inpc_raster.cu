@@ -87,9 +87,10 @@ struct StageTimer {                       // RAII: start event now, stop event a
 struct Layout {
     size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
     size_t kept, cursor, A, gT, gD, dk, Ra, Rf, items, bigpix, bigcells, bigkeys;
-    size_t pcur, gpt;                                     // only with INPC_SAVE_FOR_BACKWARD
+    size_t pixoff;                                        // per-pixel list offsets (order lists, sorted dump)
+    size_t pcur, gpt, ord;                                // only with INPC_SAVE_FOR_BACKWARD
     size_t shfeat;                                        // only with INPC_FUSED_SH: per-point features out of the SH pass
-    size_t pixoff, sorted_idx, sorted_depth, sorted_T;    // only with INPC_SAVE_SORTED
+    size_t sorted_idx, sorted_depth, sorted_T;            // only with INPC_SAVE_SORTED
     size_t total;
     uint32_t C, P, max_big_cells, n_status;
 };
@@ -121,13 +122,14 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     L.bigpix = o;  o = align_up(o + ((size_t)L.P + 16) * 4);
     L.bigcells = o; o = align_up(o + ((size_t)L.max_big_cells + 1) * sizeof(BigCell));
     L.bigkeys = o; o = align_up(o + (n + 8) * 8);
+    L.pixoff = o;  o = align_up(o + ((size_t)L.P + 1) * 4);
     if (flags & INPC_SAVE_FOR_BACKWARD) {
         L.pcur = o; o = align_up(o + (size_t)L.P * 16);
         L.gpt = o;  o = align_up(o + n * (size_t)(D == 4 ? 32 : 64) + 64);
+        L.ord = o;  o = align_up(o + (4 * n + 64) * 2);
     }
     if (flags & INPC_FUSED_SH) { L.shfeat = o; o = align_up(o + (n + 8) * 16); }
     if (flags & INPC_SAVE_SORTED) {
-        L.pixoff = o;       o = align_up(o + ((size_t)L.P + 1) * 4);
         L.sorted_idx = o;   o = align_up(o + (4 * n + 8) * 4);
         L.sorted_depth = o; o = align_up(o + (4 * n + 8) * 4);
         L.sorted_T = o;     o = align_up(o + (4 * n + 8) * 4);
@@ -221,7 +223,7 @@ static int launch_back(const BackArgs& A, const DeviceInfo& di, cudaStream_t st)
 
 template <int D, bool SAVE, bool DUMP>
 static int launch_blend(const BlendArgs& A, const DeviceInfo& di, cudaStream_t st) {
-    constexpr size_t smem = blend_smem_bytes<D>();
+    constexpr size_t smem = blend_smem_bytes<D, SAVE>();
     static int grid_by_dev[kMaxDevices] = {};
     int grid = 0;
     int rc = persistent_grid(k_blend<D, SAVE, DUMP>, kTileThreads, smem, di, grid_by_dev, &grid);
@@ -362,7 +364,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     BigCell* bigcells = reinterpret_cast<BigCell*>(ws + L.bigcells);
     const bool dump = (flags & INPC_SAVE_SORTED) != 0;
     const bool save = (flags & INPC_SAVE_FOR_BACKWARD) != 0;
-    uint32_t* pixoff = dump ? reinterpret_cast<uint32_t*>(ws + L.pixoff) : nullptr;
+    uint32_t* pixoff = (dump || save) ? reinterpret_cast<uint32_t*>(ws + L.pixoff) : nullptr;
 
     // two streams unless per-stage timing wants every kernel alone
     std::unique_lock<std::mutex> side_lock(g_side_mu, std::defer_lock);
@@ -402,7 +404,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     { StageTimer tm(kStClassify, s2);
       k_classify<<<(L.C + 255) / 256, 256, 0, s2>>>(cellcnt, W, H, hdr, bigcells, pixoff); }
     INPC_LAUNCHED("k_classify");
-    if (dump) {
+    if (pixoff) {                                         // starts of the per-pixel lists (saved blend order, sorted dump)
         { StageTimer tm(kStOther, s2);
           k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, s2>>>(
               pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr, nullptr); }
@@ -442,9 +444,10 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     if (save) {
         A.gT = Bg.gT = reinterpret_cast<float*>(ws + L.gT);
         A.pcur = Bg.pcur = reinterpret_cast<uint4*>(ws + L.pcur);
+        A.ord = reinterpret_cast<uint16_t*>(ws + L.ord);
     }
+    Bg.pixoff = A.pixoff = pixoff;
     if (dump) {
-        Bg.pixoff = A.pixoff = pixoff;
         Bg.sorted_idx = A.sorted_idx = reinterpret_cast<uint32_t*>(ws + L.sorted_idx);
         Bg.sorted_depth = A.sorted_depth = reinterpret_cast<uint32_t*>(ws + L.sorted_depth);
         Bg.sorted_T = A.sorted_T = reinterpret_cast<float*>(ws + L.sorted_T);
@@ -512,7 +515,8 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     int rc = launch_big<D, kBwd>(Bg, di.sms, st);
     if (rc != INPC_OK) return rc;
     BackArgs A{};
-    A.hdr = hdr; A.celloff = celloff; A.dk = Bg.dk; A.Ra = Ra; A.Rf = Rf;
+    A.hdr = hdr; A.celloff = celloff; A.Ra = Ra; A.Rf = Rf;
+    A.pixoff = reinterpret_cast<const uint32_t*>(ws + L.pixoff); A.ord = reinterpret_cast<const uint16_t*>(ws + L.ord);
     A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD; A.io = io;
     const Bands Bf = make_bands(W, H, L.C, kDefaultBands);     // the plan the forward built the item lists with
     uint32_t u0 = 0;
