@@ -5,14 +5,17 @@
 // staged exactly as the forward pass staged it (same cell rows, same 4-record alignment => the same shared-memory
 // record indices), with cp.async.bulk onto one mbarrier: per record the { tx, ty, opacity, idx } word (turned into
 // the four per-corner alphas in place), the features and the four transmittances gT the forward pass saved.
-// The depth order is NOT merged again: the forward pass left, for every pixel, the list of (record, corner) it
-// blended, in order (ord, 16 bits per fragment, blend.cuh); a tile's lists are th contiguous runs of that array
-// and are staged with the same bulk copies.  ONE THREAD PER PIXEL (lanes in descending order of the blended
-// count) walks its list from the last blended fragment to the first with the division-free recurrence
+// The depth order is NOT merged again: the forward pass left, for every tile item, one block of ord[] holding the
+// item's per-pixel lists of blended (record, corner) in blend order (16 bits per fragment, blend.cuh); the block
+// is staged by one more bulk copy.  ONE THREAD PER PIXEL (lanes in descending order of the blended count) walks
+// its list from the last blended fragment to the first with the division-free recurrence
 //     dL/da_k = T_k (G_k - B_k),    B_{k-1} = a_k G_k + (1 - a_k) B_k,    G_k = <feat_k, g_img[p]> + g_alpha[p]
 // and writes dL/da_k to gD[(slot, corner)]; grad.cuh combines the four corners of every record.  No address in
 // the loop depends on the recurrence, so the loads of four fragments are issued together and the only dependent
 // chain is B.
+// What bounds a tile is latency, not work, so everything a tile needs BEFORE its bulk copies can be issued (cell
+// offsets, block position) and everything its pixels need (blended counts, image gradients) is loaded into
+// registers one tile ahead, while the previous tile is walked.
 #pragma once
 #include "common.cuh"
 
@@ -29,7 +32,7 @@ struct BackArgs {
     int W, H;
     const float* gT;
     const uint4* pcur;
-    const uint32_t* pixoff;  // start of every pixel's order list
+    const uint2* ordinfo;    // per item of this band: { first entry of its block of ord[], entries }
     const uint16_t* ord;     // (record * 16 + 4 * corner) of the k-th blended fragment, tile-local (forward pass)
     const float* g_feat;
     const float* g_alpha;
@@ -37,29 +40,71 @@ struct BackArgs {
     float* gD;
 };
 
-constexpr int kOrdPad = 8 * 2 * kTileH;      // entries: every tile row's run is widened to 16-byte boundaries at both ends
-
 template <int D> __host__ __device__ constexpr size_t back_smem_bytes() {
-    return (size_t)TileCfg<D>::kCap * (16 + 4 * D + 16 + 8) + 2 * kOrdPad;     // alphas, features, gT, order lists
+    return (size_t)TileCfg<D>::kCap * (16 + 4 * D + 16 + 8) + 16;     // alphas, features, gT, order lists
+}
+
+// What a thread loads one tile ahead: up to two entries of the (th+1) x (tw+2) window of cell offsets, its pixel's
+// (natural order) blended counts and image gradient, and (thread 0) the tile's block of the saved order.
+template <int D> struct BackPrefetch {
+    uint32_t off0, off1;
+    uint4 cn;
+    float g[D], gA;
+    uint2 info;
+};
+
+template <int D>
+__device__ __forceinline__ void back_prefetch(const BackArgs& A, uint32_t item_i, uint32_t it, bool valid, BackPrefetch<D>& P) {
+    const int tid = threadIdx.x;
+    const int W = A.W, H = A.H;
+    const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
+    const int tw = 1 << lw, th = 1 << lh;
+    P.off0 = P.off1 = 0u;
+    P.cn = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int d = 0; d < D; ++d) P.g[d] = 0.f;
+    P.gA = 0.f;
+    P.info = make_uint2(0, 0);
+    if (!valid) return;
+    const int n_off = (th + 1) * (tw + 2);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int e = tid + h * kTileThreads;
+        if (e < n_off) {
+            const int r = e / (tw + 2), c = e - r * (tw + 2);
+            const int j = Y + r;
+            const uint32_t v = j <= H ? __ldg(&A.celloff[(uint32_t)j * (W + 1) + min(X + c, W + 1)]) : 0u;
+            if (h == 0) P.off0 = v; else P.off1 = v;
+        }
+    }
+    const int ly0 = tid >> lw, lx0 = tid & (tw - 1);
+    if (tid < tw * th && X + lx0 < W && Y + ly0 < H) {
+        const size_t p0 = (size_t)(Y + ly0) * W + X + lx0;
+        P.cn = __ldg(&A.pcur[p0]);
+        load_pixel_grad<D>(A.io, A.g_feat, A.g_alpha, p0, P.g, P.gA);
+    }
+    if (tid == 0) P.info = __ldg(&A.ordinfo[item_i]);
 }
 
 template <int D>
 __global__ void __launch_bounds__(kTileThreads, 3) k_back(BackArgs A) {
     constexpr int FV  = D / 4;
     constexpr int CAP = TileCfg<D>::kCap;
+    static_assert((kTileH + 1) * (kTileW + 2) <= 2 * kTileThreads, "two window entries per thread");
     extern __shared__ __align__(128) unsigned char smem[];
     float4*   s_a4  = reinterpret_cast<float4*>(smem);
     float4*   s_f   = reinterpret_cast<float4*>(smem + (size_t)CAP * 16);
     float4*   s_t4  = reinterpret_cast<float4*>(smem + (size_t)CAP * (16 + 16 * FV));
     uint16_t* s_ord = reinterpret_cast<uint16_t*>(smem + (size_t)CAP * (32 + 16 * FV));
 
-    __shared__ uint32_t s_off[kTileH + 1][kTileW + 2];
+    __shared__ uint32_t s_off[(kTileH + 1) * (kTileW + 2)];   // window of cell offsets, row stride tw + 2
     __shared__ uint32_t s_sbase[kTileH + 1], s_a4row[kTileH + 1];
-    __shared__ uint32_t s_rowblk[kTileH], s_rowg[kTileH];     // order-list run of pixel row r: smem entry s_rowblk[r] <-> global entry s_rowg[r]
     __shared__ uint32_t s_hist[64];
-    __shared__ uint32_t s_pixbase[kTileThreads];
+    __shared__ uint32_t s_pixbase[kTileThreads], s_wsum[kTileThreads / 32];
+    __shared__ uint4    s_cn[kTileThreads];                   // per pixel (natural order): blended records of its four lists
+    __shared__ float    s_g[kTileThreads][D + 1];             // ... and its image gradient (g_img[D], g_alpha)
     __shared__ uint8_t  s_perm[kTileThreads];
-    __shared__ uint32_t s_next, s_next_code, s_tot;
+    __shared__ uint32_t s_next, s_next_code, s_tot, s_ordn;
     __shared__ __align__(8) uint64_t s_bar;
 
     const int tid = threadIdx.x;
@@ -72,86 +117,78 @@ __global__ void __launch_bounds__(kTileThreads, 3) k_back(BackArgs A) {
         const uint32_t nx = atomicAdd(A.item_cursor, 1u);
         s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
     }
+    __syncthreads();
+    BackPrefetch<D> P;
+    back_prefetch<D>(A, s_next, s_next_code, s_next < n_items, P);
     uint32_t parity = 0;
 
     while (true) {
-        __syncthreads();                                  // everyone is done with the previous item's smem
+        __syncthreads();                                  // (A) everyone is done with the previous item's smem
         const uint32_t item_i = s_next;
         if (item_i >= n_items) break;
         const uint32_t it = s_next_code;
         const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
-        const int tw = 1 << lw, th = 1 << lh;
-
-        // this thread's pixel in natural order: its blended count and the start of its order list (loads in flight early)
-        const int ly0 = tid >> lw, lx0 = tid & (tw - 1);
-        const bool live0 = tid < tw * th && X + lx0 < W && Y + ly0 < H;
-        uint32_t n_mine = 0, po_mine = 0;
-        if (live0) {
-            const size_t p0 = (size_t)(Y + ly0) * W + X + lx0;
-            const uint4 cn = __ldg(&A.pcur[p0]);
-            n_mine = cn.x + cn.y + cn.z + cn.w;
-            po_mine = __ldg(&A.pixoff[p0]);
-        }
-        // cell offsets of the tile's (th+1) x (tw+2) window
-        for (int e = tid; e < (th + 1) * (tw + 2); e += kTileThreads) {
-            const int r = e / (tw + 2), c = e - r * (tw + 2);
-            const int j = Y + r;
-            uint32_t v = 0;
-            if (j <= H) v = __ldg(&A.celloff[(uint32_t)j * (W + 1) + min(X + c, W + 1)]);
-            s_off[r][c] = v;
-        }
+        const int tw = 1 << lw, th = 1 << lh, ws = tw + 2;
+        // what was loaded one tile ahead goes to shared memory
+        if (tid < (th + 1) * ws) s_off[tid] = P.off0;
+        if (tid + kTileThreads < (th + 1) * ws) s_off[tid + kTileThreads] = P.off1;
+        s_cn[tid] = P.cn;
+#pragma unroll
+        for (int d = 0; d < D; ++d) s_g[tid][d] = P.g[d];
+        s_g[tid][D] = P.gA;
+        if (tid == 0) s_ordn = P.info.y;
+        const uint32_t ord_base = P.info.x;               // (thread 0)
+        const uint32_t n_bl = P.cn.x + P.cn.y + P.cn.z + P.cn.w;
         if (tid < 64) s_hist[tid] = 0;
-        __syncthreads();
+        __syncthreads();                                  // (B)
         if (tid == 32) {                                  // fetch the next work item while this one is processed
             const uint32_t nx = atomicAdd(A.item_cursor, 1u);
             s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
         }
-        if (tid < 32) {                                   // warp 0: one lane per cell row / pixel row issues that row's copies
-            // order-list run of pixel row `tid`: global entries [g0, g1), widened to 8-entry (16-byte) boundaries
-            uint32_t gs = 0, olen = 0;
-            if (tid < th && Y + tid < H) {
-                const size_t pr = (size_t)(Y + tid) * W;
-                const uint32_t g0 = __ldg(&A.pixoff[pr + X]), g1 = __ldg(&A.pixoff[pr + min(X + tw, W)]);
-                gs = g0 & ~7u;
-                olen = g1 > g0 ? ((g1 + 7u) & ~7u) - gs : 0u;
-            }
+        if (tid < 32) {                                   // warp 0: one lane per cell row issues that row's copies
             const bool row = tid <= th;
             uint32_t a4 = 0, len = 0;
             if (row) {
-                const uint32_t a = s_off[tid][0], b = s_off[tid][tw + 1];
+                const uint32_t a = s_off[tid * ws], b = s_off[tid * ws + tw + 1];
                 a4 = a & ~3u;
                 len = b > a ? ((b + 3u) & ~3u) - a4 : 0u;
             }
-            uint32_t inc = len, oinc = olen;
+            uint32_t inc = len;
 #pragma unroll
-            for (int d = 1; d < 16; d <<= 1) {
-                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d), u = __shfl_up_sync(0xffffffffu, oinc, d);
-                if (tid >= d) { inc += t; oinc += u; }
-            }
-            const uint32_t sb = inc - len, ob = oinc - olen;
-            const uint32_t tot = __shfl_sync(0xffffffffu, inc, 15), otot = __shfl_sync(0xffffffffu, oinc, 15);
+            for (int d = 1; d < 16; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d); if (tid >= d) inc += t; }
+            const uint32_t sb = inc - len;
+            const uint32_t tot = __shfl_sync(0xffffffffu, inc, 15);
             if (row) { s_a4row[tid] = a4; s_sbase[tid] = sb; }
-            if (tid < th) { s_rowblk[tid] = ob; s_rowg[tid] = gs; }
+            const uint32_t n8 = (s_ordn + 7u) & ~7u;      // the forward pass wrote the block in 8-entry (16-byte) units
             fence_proxy_async();
             if (tid == 0) {
                 s_tot = tot;
-                if (tot > 0) mbar_arrive_expect_tx(&s_bar, tot * (uint32_t)(16 + 16 * FV + 16) + otot * 2u);
+                if (tot > 0) {
+                    mbar_arrive_expect_tx(&s_bar, tot * (uint32_t)(16 + 16 * FV + 16) + n8 * 2u);
+                    if (n8) bulk_g2s(s_ord, A.ord + ord_base, n8 * 2u, &s_bar);
+                }
             }
             __syncwarp();
-            if (tot > 0) {
-                if (len) {
-                    bulk_g2s(s_a4 + sb, A.Ra + a4, len * 16, &s_bar);
-                    bulk_g2s(s_f + (size_t)sb * FV, A.Rf + (size_t)a4 * FV, len * FV * 16, &s_bar);
-                    bulk_g2s(s_t4 + sb, reinterpret_cast<const float4*>(A.gT) + a4, len * 16, &s_bar);
-                }
-                if (olen) bulk_g2s(s_ord + ob, A.ord + gs, olen * 2, &s_bar);
+            if (tot > 0 && len) {
+                bulk_g2s(s_a4 + sb, A.Ra + a4, len * 16, &s_bar);
+                bulk_g2s(s_f + (size_t)sb * FV, A.Rf + (size_t)a4 * FV, len * FV * 16, &s_bar);
+                bulk_g2s(s_t4 + sb, reinterpret_cast<const float4*>(A.gT) + a4, len * 16, &s_bar);
             }
         }
-        // while the copies fly: the lane permutation by descending blended count
-        const uint32_t bucket = 63u - min(n_mine >> 2, 63u);
+        // while the copies fly: the lane permutation by descending blended count; the starts of the order lists are the
+        // exclusive scan of the pixels' fragment counts in natural order (exactly what the forward pass laid out)
+        const int ly0 = tid >> lw, lx0 = tid & (tw - 1);
+        uint32_t n_all = 0;
+        if (tid < tw * th && X + lx0 < W && Y + ly0 < H)
+            n_all = (s_off[ly0 * ws + lx0 + 2] - s_off[ly0 * ws + lx0]) + (s_off[(ly0 + 1) * ws + lx0 + 2] - s_off[(ly0 + 1) * ws + lx0]);
+        const uint32_t bucket = 63u - min(n_bl >> 2, 63u);
         const uint32_t rank_in_bucket = atomicAdd(&s_hist[bucket], 1u);
-        __syncthreads();
-        if (tid < 32) {                                                // exclusive scan of the 64 buckets
+        uint32_t inc_all = n_all;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc_all, d); if ((tid & 31) >= d) inc_all += t; }
+        if ((tid & 31) == 31) s_wsum[tid >> 5] = inc_all;
+        __syncthreads();                                  // (C)
+        if (tid < 32) {                                   // exclusive scan of the 64 buckets
             const uint32_t b0 = s_hist[2 * tid], b1 = s_hist[2 * tid + 1];
             uint32_t inc = b0 + b1;
 #pragma unroll
@@ -159,8 +196,13 @@ __global__ void __launch_bounds__(kTileThreads, 3) k_back(BackArgs A) {
             s_hist[2 * tid] = inc - b0 - b1;
             s_hist[2 * tid + 1] = inc - b1;
         }
-        if (live0) s_pixbase[tid] = s_rowblk[ly0] + (po_mine - s_rowg[ly0]);
-        __syncthreads();
+        {
+            uint32_t before = 0;
+#pragma unroll
+            for (int w = 0; w < kTileThreads / 32; ++w) before += w < (tid >> 5) ? s_wsum[w] : 0u;
+            s_pixbase[tid] = before + inc_all - n_all;
+        }
+        __syncthreads();                                  // (D)
         s_perm[s_hist[bucket] + rank_in_bucket] = (uint8_t)tid;
         const uint32_t tot = s_tot;
         if (tot > 0) { mbar_wait(&s_bar, parity); parity ^= 1u; }
@@ -170,23 +212,25 @@ __global__ void __launch_bounds__(kTileThreads, 3) k_back(BackArgs A) {
             const float wx0 = 1.f - q.x, wy0 = 1.f - q.y;
             s_a4[r] = make_float4(q.z * (wx0 * wy0), q.z * (q.x * wy0), q.z * (wx0 * q.y), q.z * (q.x * q.y));
         }
-        __syncthreads();
+        __syncthreads();                                  // (E)
+        // the next tile's metadata: in flight while this one is walked
+        { const uint32_t nx = s_next; back_prefetch<D>(A, nx, s_next_code, nx < n_items, P); }
 
         // ---------------------------------------------------------------- one thread per pixel
         const int q = s_perm[tid];
         const int ly = q >> lw, lx = q & (tw - 1);
-        const int x = X + lx, y = Y + ly;
-        if (q >= tw * th || x >= W || y >= H) continue;
-        const size_t pix = (size_t)y * W + x;
-        const uint4 cn = __ldg(&A.pcur[pix]);             // blended records of each of the four lists
+        if (q >= tw * th || X + lx >= W || Y + ly >= H) continue;
+        const uint4 cn = s_cn[q];                         // blended records of each of the four lists
         const uint32_t nb = cn.x + cn.y + cn.z + cn.w;
         if (nb == 0u) continue;
         // smem record of global slot g in cell row r: g + (s_sbase[r] - s_a4row[r]); corners 2, 3 lie in the top cell row
         const uint32_t bt = s_sbase[ly] - s_a4row[ly], bb = s_sbase[ly + 1] - s_a4row[ly + 1];
         float* gDtop = A.gD + 4 * ((ptrdiff_t)(int32_t)(0u - bt));
         float* gDbot = A.gD + 4 * ((ptrdiff_t)(int32_t)(0u - bb));
-        float g[D], gA;
-        load_pixel_grad<D>(A.io, A.g_feat, A.g_alpha, pix, g, gA);
+        float g[D];
+#pragma unroll
+        for (int d = 0; d < D; ++d) g[d] = s_g[q][d];
+        const float gA = s_g[q][D];
         const uint32_t sa = smem_u32(s_a4), sf = smem_u32(s_f), st = smem_u32(s_t4);
         const uint32_t so = smem_u32(s_ord) + 2u * s_pixbase[q];
 

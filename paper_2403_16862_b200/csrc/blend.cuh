@@ -14,10 +14,12 @@
 //      head key selects the list with predicates, and only "two heads with equal depth bits" (ascending
 //      point index decides, read from global memory) and the two loop exits are branches.
 // With INPC_SAVE_FOR_BACKWARD the transmittance in front of every blended fragment goes to
-// gT[(slot, corner)], the four list positions at the stop to pcur[pixel], and the ORDER itself to
-// ord[pixoff[pixel] + k] = which staged (record, corner) was blended k-th (16 bits: the fragment's byte offset
-// record * 16 + 4 * corner inside the tile's staged records) -- the backward pass stages the same tile the same
-// way and walks that list backwards without merging anything again (back.cuh).
+// gT[(slot, corner)], the four list positions at the stop to pcur[pixel], and the ORDER itself is kept: which
+// staged (record, corner) was blended k-th (16 bits: the fragment's byte offset record * 16 + 4 * corner inside the
+// tile's staged records), one list per pixel, the tile's lists back to back in shared memory and written out as
+// ONE block of ord[] by a bulk (TMA) store while the next tile is already being staged; ordinfo[item] = { start of
+// the block, entries }.  The backward pass stages the same tile the same way and walks those lists backwards
+// without merging anything again (back.cuh).
 #pragma once
 #include "common.cuh"
 
@@ -38,9 +40,11 @@ struct BlendArgs {
     ImageIO io;
     float* gT;               // NULL unless INPC_SAVE_FOR_BACKWARD
     uint4* pcur;
-    uint16_t* ord;           // blend order of every pixel (INPC_SAVE_FOR_BACKWARD), indexed through pixoff
-    const uint32_t* pixoff;  // exclusive scan of the per-pixel fragment counts (save or dump)
+    uint16_t* ord;           // blend order, one block per tile item (INPC_SAVE_FOR_BACKWARD)
+    uint2* ordinfo;          // per item of this band: { first entry of its block, entries }
+    uint32_t* ord_cursor;    // bump allocator of the blocks
     // dump (INPC_SAVE_SORTED)
+    const uint32_t* pixoff;  // exclusive scan of the per-pixel fragment counts
     uint32_t* sorted_idx;
     uint32_t* sorted_depth;
     float* sorted_T;         // transmittance in front of every blended fragment, -1 behind the cut-off
@@ -71,11 +75,6 @@ __device__ __forceinline__ uint32_t pack_list(uint32_t start_rec, uint32_t end_r
         p0 = jb == 0; p1 = jb == 1; p2 = jb == 2; p3 = jb == 3;                                                           \
     } while (0)
 
-#ifdef INPC_EXP_NO_STS
-#define INPC_EXP_STS(a, v)
-#else
-#define INPC_EXP_STS(a, v) sts_u16(a, v)
-#endif
 template <int D, bool SAVE, bool DUMP>
 __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
     constexpr int FV  = D / 4;                     // float4 of features per record
@@ -87,7 +86,6 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
     const unsigned char* s_ab = smem + (size_t)CAP * 4;
     uint16_t* s_ord = reinterpret_cast<uint16_t*>(smem + (size_t)CAP * (20 + 16 * FV));   // SAVE only
     __shared__ uint32_t s_pixbase[kTileThreads], s_wsum[kTileThreads / 32], s_ordtot;     // SAVE: starts of the tile's order lists
-    __shared__ uint32_t s_rowg[kTileH];                                                   // ... and of its pixel rows' runs in ord[]
 
     __shared__ uint32_t s_off[kTileH + 1][kTileW + 2];
     __shared__ uint32_t s_sbase[kTileH + 1], s_a4row[kTileH + 1];
@@ -107,22 +105,19 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
     }
     uint32_t parity = 0;
     bool have_prev = false;                               // SAVE: the previous item's order lists still sit in shared memory
-    int pX = 0, pY = 0, plw = 0, pth = 0;
+    uint32_t p_item = 0;
 
     while (true) {
         __syncthreads();                                  // everyone is done with the previous item's smem
         if constexpr (SAVE) {
-            // The previous tile's order lists go out to ord[], coalesced: pixel row r of the tile is one contiguous run
-            // both in shared memory (pixels in natural order) and in the global array (pixoff is row-major).
-#ifndef INPC_EXP_NO_COPYOUT
-            if (have_prev) {
-                for (int r = 0; r < pth && pY + r < H; ++r) {
-                    const uint32_t s0 = s_pixbase[r << plw], s1 = r + 1 < pth ? s_pixbase[(r + 1) << plw] : s_ordtot;
-                    uint16_t* dst = A.ord + s_rowg[r];
-                    for (uint32_t i = tid; i < s1 - s0; i += kTileThreads) dst[i] = s_ord[s0 + i];
-                }
+            // The previous tile's order lists (back to back in shared memory, pixels in natural order) go out to ord[] as
+            // one block: a bulk store issued by one thread; it has finished reading before this tile's walk overwrites them.
+            if (tid == 0 && have_prev) {
+                const uint32_t n8 = (s_ordtot + 7u) & ~7u;
+                const uint32_t base = n8 ? atomicAdd(A.ord_cursor, n8) : 0u;
+                A.ordinfo[p_item] = make_uint2(base, s_ordtot);
+                if (n8) { fence_proxy_async(); bulk_s2g(A.ord + base, s_ord, n8 * 2u); }
             }
-#endif
         }
         const uint32_t item_i = s_next;
         if (item_i >= n_items) break;
@@ -130,8 +125,6 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
         const int X = it & 0xfff, Y = (it >> 12) & 0xfff, lw = (it >> 24) & 7, lh = (it >> 27) & 3;
         const int tw = 1 << lw, th = 1 << lh;
 
-        uint32_t rowg = 0;                                // SAVE: where pixel row `tid - 64` of this tile starts in ord[]
-        if constexpr (SAVE) { if (tid >= 64 && tid - 64 < th && Y + tid - 64 < H) rowg = __ldg(&A.pixoff[(size_t)(Y + tid - 64) * W + X]); }
         // cell offsets of the tile's (th+1) x (tw+2) window
         for (int e = tid; e < (th + 1) * (tw + 2); e += kTileThreads) {
             const int r = e / (tw + 2), c = e - r * (tw + 2);
@@ -142,7 +135,6 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
         }
         if (tid < 64) s_hist[tid] = 0;
         __syncthreads();
-        if constexpr (SAVE) { if (tid >= 64 && tid - 64 < th) s_rowg[tid - 64] = rowg; }
         if (tid == 32) {                                  // fetch the next work item while this one is processed
             const uint32_t nx = atomicAdd(A.item_cursor, 1u);
             s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
@@ -194,7 +186,7 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
             for (int w = 0; w < kTileThreads / 32; ++w) before += w < (tid >> 5) ? s_wsum[w] : 0u;
             s_pixbase[tid] = before + inc_mine - n_mine;
             if (tid == kTileThreads - 1) s_ordtot = before + inc_mine;
-            have_prev = true; pX = X; pY = Y; plw = lw; pth = th;
+            have_prev = true; p_item = item_i;
         }
         if (tid < 32) {                                                // exclusive scan of the 64 buckets
             const uint32_t h0 = s_hist[2 * tid], h1 = s_hist[2 * tid + 1];
@@ -214,6 +206,7 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
             const float wx0 = 1.f - q.x, wy0 = 1.f - q.y;
             s_a4[r] = make_float4(q.z * (wx0 * wy0), q.z * (q.x * wy0), q.z * (wx0 * q.y), q.z * (q.x * q.y));
         }
+        if constexpr (SAVE) { if (tid == 0) bulk_wait_read(); }       // the previous tile's order lists have left shared memory
         __syncthreads();
 
         // ---------------------------------------------------------------- 3. one thread per pixel
@@ -305,7 +298,7 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
                 acc[4 * v] += c * f##X[v].x; acc[4 * v + 1] += c * f##X[v].y;                                             \
                 acc[4 * v + 2] += c * f##X[v].z; acc[4 * v + 3] += c * f##X[v].w;                                         \
             }                                                                                                             \
-            if constexpr (SAVE) { ((cur##X & 8u) ? gTtop : gTbot)[cur##X >> 2] = T; INPC_EXP_STS(so, cur##X); so += 2u; }        \
+            if constexpr (SAVE) { ((cur##X & 8u) ? gTtop : gTbot)[cur##X >> 2] = T; sts_u16(so, cur##X); so += 2u; }        \
             if constexpr (DUMP) A.sorted_T[obase + kd##X] = T;                                                            \
             T *= (1.f - a##X);                                                                                            \
         }
@@ -368,6 +361,7 @@ __global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
         store_pixel<D>(A.io, A.out_feat, A.out_alpha, pix, acc, accA);
         if constexpr (SAVE) A.pcur[pix] = consumed;
     }
+    if constexpr (SAVE) { if (tid == 0) bulk_wait_read(); }           // the last block has left shared memory
 }
 
 #undef INPC_BLEND_RESOLVE_TIE

@@ -72,7 +72,8 @@ struct Header {
     uint32_t cellsort_cursor;
     uint32_t bwd_ok;               // written by the backward pass's header check: 1 = the workspace matches its arguments
     int32_t  status;               // sticky inpc_status of device-side checks (read by inpc_raster_get_status)
-    uint32_t pad[9];
+    uint32_t ord_cursor;           // bump allocator of the per-tile blocks of the saved blend order (entries)
+    uint32_t pad[8];
     // Tile work items, one list per BAND of tile rows (kMaxBands bands): a band's tiles can be blended as soon as
     // its cell rows are sorted, while the next band's cells are still being sorted on another stream.
     uint32_t band_items[8];        // items of band b
@@ -142,6 +143,16 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
                      smem_u32(dst_smem)),
                  "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
+}
+
+// TMA bulk copy shared -> global (1-D): same alignment rules; completion is tracked per thread by bulk groups.
+__device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read() {        // the issuing thread's bulk stores have finished READING shared memory
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 // ---- step a1: canonical fp32 projection (Eq. 6; reading R1) ------------

@@ -87,8 +87,8 @@ struct StageTimer {                       // RAII: start event now, stop event a
 struct Layout {
     size_t header, status0, status1, cellcnt, zero_end;   // [header, zero_end) is cleared every forward
     size_t kept, cursor, A, gT, gD, dk, Ra, Rf, items, bigpix, bigcells, bigkeys;
-    size_t pixoff;                                        // per-pixel list offsets (order lists, sorted dump)
-    size_t pcur, gpt, ord;                                // only with INPC_SAVE_FOR_BACKWARD
+    size_t pcur, gpt, ord, ordinfo;                       // only with INPC_SAVE_FOR_BACKWARD
+    size_t pixoff;                                        // only with INPC_SAVE_SORTED
     size_t shfeat;                                        // only with INPC_FUSED_SH: per-point features out of the SH pass
     size_t sorted_idx, sorted_depth, sorted_T;            // only with INPC_SAVE_SORTED
     size_t total;
@@ -118,18 +118,20 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     L.Ra = o;      o = align_up(o + (n + 8) * 16);
     L.Rf = o;      o = align_up(o + (n + 8) * (size_t)(4 * D));
     const size_t nbase = (size_t)((W + kTileW - 1) / kTileW) * ((H + kTileH - 1) / kTileH);
-    L.items = o;   o = align_up(o + ((size_t)L.P + nbase + 16 * (kMaxBands + 1)) * 4);
+    L.items = o;   o = align_up(o + ((size_t)L.P + nbase + 16 * (kMaxBands + 1)) * 4);   // (max_items below)
     L.bigpix = o;  o = align_up(o + ((size_t)L.P + 16) * 4);
     L.bigcells = o; o = align_up(o + ((size_t)L.max_big_cells + 1) * sizeof(BigCell));
     L.bigkeys = o; o = align_up(o + (n + 8) * 8);
-    L.pixoff = o;  o = align_up(o + ((size_t)L.P + 1) * 4);
+    const size_t max_items = (size_t)L.P + nbase + 16 * (kMaxBands + 1);
     if (flags & INPC_SAVE_FOR_BACKWARD) {
         L.pcur = o; o = align_up(o + (size_t)L.P * 16);
         L.gpt = o;  o = align_up(o + n * (size_t)(D == 4 ? 32 : 64) + 64);
-        L.ord = o;  o = align_up(o + (4 * n + 64) * 2);
+        L.ord = o;  o = align_up(o + (4 * n + 8 * 16 * nbase + 64) * 2);   // blocks in 8-entry units, <= 16 items per base tile
+        L.ordinfo = o; o = align_up(o + max_items * 8);
     }
     if (flags & INPC_FUSED_SH) { L.shfeat = o; o = align_up(o + (n + 8) * 16); }
     if (flags & INPC_SAVE_SORTED) {
+        L.pixoff = o;       o = align_up(o + ((size_t)L.P + 1) * 4);
         L.sorted_idx = o;   o = align_up(o + (4 * n + 8) * 4);
         L.sorted_depth = o; o = align_up(o + (4 * n + 8) * 4);
         L.sorted_T = o;     o = align_up(o + (4 * n + 8) * 4);
@@ -364,7 +366,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     BigCell* bigcells = reinterpret_cast<BigCell*>(ws + L.bigcells);
     const bool dump = (flags & INPC_SAVE_SORTED) != 0;
     const bool save = (flags & INPC_SAVE_FOR_BACKWARD) != 0;
-    uint32_t* pixoff = (dump || save) ? reinterpret_cast<uint32_t*>(ws + L.pixoff) : nullptr;
+    uint32_t* pixoff = dump ? reinterpret_cast<uint32_t*>(ws + L.pixoff) : nullptr;
 
     // two streams unless per-stage timing wants every kernel alone
     std::unique_lock<std::mutex> side_lock(g_side_mu, std::defer_lock);
@@ -404,7 +406,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     { StageTimer tm(kStClassify, s2);
       k_classify<<<(L.C + 255) / 256, 256, 0, s2>>>(cellcnt, W, H, hdr, bigcells, pixoff); }
     INPC_LAUNCHED("k_classify");
-    if (pixoff) {                                         // starts of the per-pixel lists (saved blend order, sorted dump)
+    if (dump) {
         { StageTimer tm(kStOther, s2);
           k_scan_u32<<<(L.P + kScanTile - 1) / kScanTile, kScanThreads, 0, s2>>>(
               pixoff, L.P, reinterpret_cast<unsigned long long*>(ws + L.status1), &hdr->pad0, nullptr, nullptr); }
@@ -444,7 +446,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
     if (save) {
         A.gT = Bg.gT = reinterpret_cast<float*>(ws + L.gT);
         A.pcur = Bg.pcur = reinterpret_cast<uint4*>(ws + L.pcur);
-        A.ord = reinterpret_cast<uint16_t*>(ws + L.ord);
+        A.ord = reinterpret_cast<uint16_t*>(ws + L.ord); A.ord_cursor = &hdr->ord_cursor;
     }
     Bg.pixoff = A.pixoff = pixoff;
     if (dump) {
@@ -464,6 +466,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
         }
         INPC_CUDA(fork(st, s2));                                              // band b is sorted: blend it
         A.items = items + B.plan.item_base[b]; A.n_items = &hdr->band_items[b]; A.item_cursor = &hdr->band_cursor[b];
+        if (save) A.ordinfo = reinterpret_cast<uint2*>(ws + L.ordinfo) + B.plan.item_base[b];
         int rc = dump ? (save ? launch_blend<D, true, true>(A, di, s2) : launch_blend<D, false, true>(A, di, s2))
                       : (save ? launch_blend<D, true, false>(A, di, s2) : launch_blend<D, false, false>(A, di, s2));
         if (rc != INPC_OK) return rc;
@@ -516,12 +519,13 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     if (rc != INPC_OK) return rc;
     BackArgs A{};
     A.hdr = hdr; A.celloff = celloff; A.Ra = Ra; A.Rf = Rf;
-    A.pixoff = reinterpret_cast<const uint32_t*>(ws + L.pixoff); A.ord = reinterpret_cast<const uint16_t*>(ws + L.ord);
+    A.ord = reinterpret_cast<const uint16_t*>(ws + L.ord);
     A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD; A.io = io;
     const Bands Bf = make_bands(W, H, L.C, kDefaultBands);     // the plan the forward built the item lists with
     uint32_t u0 = 0;
     for (int b = 0; b < Bf.plan.n_bands; ++b) {
         A.items = items + Bf.plan.item_base[b]; A.n_items = &hdr->band_items[b]; A.item_cursor = &hdr->band_cursor[b];
+        A.ordinfo = reinterpret_cast<const uint2*>(ws + L.ordinfo) + Bf.plan.item_base[b];
         rc = launch_back<D>(A, di, st);
         if (rc != INPC_OK) return rc;
         const uint32_t u1 = Bf.comb_end[b];
