@@ -87,7 +87,7 @@ __device__ __forceinline__ void back_prefetch(const BackArgs& A, uint32_t item_i
 }
 
 template <int D>
-__global__ void __launch_bounds__(kTileThreads, 3) k_back(BackArgs A) {
+__global__ void __launch_bounds__(kTileThreads, 384 / kTileThreads) k_back(BackArgs A) {
     constexpr int FV  = D / 4;
     constexpr int CAP = TileCfg<D>::kCap;
     static_assert((kTileH + 1) * (kTileW + 2) <= 2 * kTileThreads, "two window entries per thread");

@@ -76,7 +76,7 @@ __device__ __forceinline__ uint32_t pack_list(uint32_t start_rec, uint32_t end_r
     } while (0)
 
 template <int D, bool SAVE, bool DUMP>
-__global__ void __launch_bounds__(kTileThreads, 4) k_blend(BlendArgs A) {
+__global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(BlendArgs A) {
     constexpr int FV  = D / 4;                     // float4 of features per record
     constexpr int CAP = TileCfg<D>::kCap;
     extern __shared__ __align__(128) unsigned char smem[];

@@ -27,9 +27,18 @@
 namespace inpc {
 
 // ---- tunables -------------------------------------------------------------------------------------
-constexpr int kTileW       = 16;    // base screen tile (pixels); halved (larger side first) down to kMinTilePix
+#ifndef INPC_TILE_LW
+#define INPC_TILE_LW 4
+#endif
+#ifndef INPC_CAP4
+#define INPC_CAP4 1216
+#endif
+#ifndef INPC_CAP8
+#define INPC_CAP8 1024
+#endif
+constexpr int kTileLW      = INPC_TILE_LW;     // log2(kTileW)
+constexpr int kTileW       = 1 << kTileLW;    // base screen tile (pixels); halved (larger side first) down to kMinTilePix
 constexpr int kTileH       = 8;
-constexpr int kTileLW      = 4;     // log2(kTileW)
 constexpr int kTileLH      = 3;     // log2(kTileH)
 constexpr int kTileThreads = kTileW * kTileH;   // one thread per pixel
 constexpr int kMinTilePix  = 8;     // a sub-tile this small that still does not fit goes to the long-run path
@@ -41,8 +50,8 @@ constexpr float kTMin      = 1e-4f; // transmittance cut-off (BASELINE.json nort
 constexpr uint32_t kSentHi = 0xFFFFFFFFu;   // "list exhausted" for the ascending merge (depth bits < 0x7F800000)
 
 template <int D> struct TileCfg;
-template <> struct TileCfg<4> { static constexpr int kCap = 1216; };   // records per tile item
-template <> struct TileCfg<8> { static constexpr int kCap = 1024; };
+template <> struct TileCfg<4> { static constexpr int kCap = INPC_CAP4; };   // records per tile item
+template <> struct TileCfg<8> { static constexpr int kCap = INPC_CAP8; };
 
 struct Camera {
     float fx, fy, cx, cy;
@@ -73,7 +82,8 @@ struct Header {
     uint32_t bwd_ok;               // written by the backward pass's header check: 1 = the workspace matches its arguments
     int32_t  status;               // sticky inpc_status of device-side checks (read by inpc_raster_get_status)
     uint32_t ord_cursor;           // bump allocator of the per-tile blocks of the saved blend order (entries)
-    uint32_t pad[8];
+    uint32_t combine_cursor;       // work cursor of k_combine (reset by the backward pass's header check)
+    uint32_t pad[7];
     // Tile work items, one list per BAND of tile rows (kMaxBands bands): a band's tiles can be blended as soon as
     // its cell rows are sorted, while the next band's cells are still being sorted on another stream.
     uint32_t band_items[8];        // items of band b

@@ -26,7 +26,7 @@ constexpr int kGradCells   = 128;      // cells per work unit: small, so that a 
 template <int D> __host__ __device__ constexpr int gpt_floats() { return D == 4 ? 8 : 16; }
 
 template <int D>
-__global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restrict__ hdr,
+__global__ void __launch_bounds__(kGradThreads) k_combine(Header* __restrict__ hdr,
                                                            const uint32_t* __restrict__ celloff, uint32_t C,
                                                            uint32_t unit_begin, uint32_t unit_end, int W,
                                                            int H, const float4* __restrict__ Ra,
@@ -35,13 +35,47 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                                                            const float* __restrict__ g_feat, ImageIO io,
                                                            float* __restrict__ gpt) {
     constexpr int GP = gpt_floats<D>();
+    constexpr int FV = D / 4;
     __shared__ uint32_t s_off[kGradCells + 1];
+    // per (cell of the unit, corner): how many records of the cell the corner's pixel blended (0: pixel outside the
+    // image) and that pixel's image gradient, loaded ONCE per cell -- every record of a cell needs the same four pixels
+    __shared__ uint32_t s_lim[kGradCells][4];
+    __shared__ float4   s_g[kGradCells][4][FV];
+    __shared__ uint32_t s_unit;
     const int tid = threadIdx.x;
     if (!hdr->bwd_ok) return;
-    for (uint32_t unit = unit_begin + blockIdx.x; unit < unit_end; unit += gridDim.x) {   // this launch's band of units
-        const uint32_t c0 = unit * kGradCells, nc = min((uint32_t)kGradCells, C - c0);
+    while (true) {                                        // units are handed out dynamically: their record counts differ widely
         __syncthreads();
+        if (tid == 0) s_unit = atomicAdd(&hdr->combine_cursor, 1u);
+        __syncthreads();
+        const uint32_t unit = unit_begin + s_unit;
+        if (unit >= unit_end) break;
+        const uint32_t c0 = unit * kGradCells, nc = min((uint32_t)kGradCells, C - c0);
         for (uint32_t c = tid; c <= nc; c += kGradThreads) s_off[c] = __ldg(&celloff[c0 + c]);
+        for (uint32_t e = tid; e < nc * 4u; e += kGradThreads) {
+            const uint32_t cl = e >> 2, c = e & 3u;
+            const uint32_t cell = c0 + cl;
+            const int j = cell / (W + 1), i = cell - j * (W + 1);
+            const int px = i - 1 + (int)(c & 1u), py = j - 1 + (int)(c >> 1);
+            uint32_t lim = 0;
+            float4 g[FV];
+#pragma unroll
+            for (int v = 0; v < FV; ++v) g[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (px >= 0 && px < W && py >= 0 && py < H) {                    // else: the fragment does not exist
+                const size_t pp = (size_t)py * W + px;
+                const uint4 cur = __ldg(&pcur[pp]);
+                lim = c == 3 ? cur.x : (c == 2 ? cur.y : (c == 1 ? cur.z : cur.w));   // the cell is the pixel's list 3 - c
+#pragma unroll
+                for (int v = 0; v < FV; ++v) {
+                    if (!io.planar) g[v] = __ldg(reinterpret_cast<const float4*>(g_feat + pp * D) + v);
+                    else g[v] = make_float4(__ldg(g_feat + (size_t)(4 * v) * io.P + pp), __ldg(g_feat + (size_t)(4 * v + 1) * io.P + pp),
+                                            __ldg(g_feat + (size_t)(4 * v + 2) * io.P + pp), __ldg(g_feat + (size_t)(4 * v + 3) * io.P + pp));
+                }
+            }
+            s_lim[cl][c] = lim;
+#pragma unroll
+            for (int v = 0; v < FV; ++v) s_g[cl][c][v] = g[v];
+        }
         __syncthreads();
         const uint32_t S = s_off[0], E = s_off[nc];
         uint32_t lo = 0;                                         // a thread's slots ascend: the search resumes at its last cell
@@ -55,27 +89,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                 const uint32_t mid = (lo + hi + 1) >> 1;
                 if (s_off[mid] <= slot) lo = mid; else hi = mid - 1;
             }
-            const uint32_t cell = c0 + lo, r = slot - s_off[lo];
-            const int j = cell / (W + 1), i = cell - j * (W + 1);
-            const int x0 = i - 1, y0 = j - 1;
-            // every gather of the four corner pixels is issued before any of them is used
-            uint4 cur[4];
-            float4 gp[4][D / 4];
-            bool in[4];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int px = x0 + (c & 1), py = y0 + (c >> 1);
-                in[c] = px >= 0 && px < W && py >= 0 && py < H;               // else: fragment does not exist
-                const size_t pp = in[c] ? (size_t)py * W + px : 0;
-                cur[c] = in[c] ? __ldg(&pcur[pp]) : make_uint4(0, 0, 0, 0);
-#pragma unroll
-                for (int v = 0; v < D / 4; ++v) {
-                    if (!in[c]) gp[c][v] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    else if (!io.planar) gp[c][v] = __ldg(reinterpret_cast<const float4*>(g_feat + pp * D) + v);
-                    else gp[c][v] = make_float4(__ldg(g_feat + (size_t)(4 * v) * io.P + pp), __ldg(g_feat + (size_t)(4 * v + 1) * io.P + pp),
-                                                __ldg(g_feat + (size_t)(4 * v + 2) * io.P + pp), __ldg(g_feat + (size_t)(4 * v + 3) * io.P + pp));
-                }
-            }
+            const uint32_t r = slot - s_off[lo];
             const float tc[4] = {t4.x, t4.y, t4.z, t4.w}, dc[4] = {d4.x, d4.y, d4.z, d4.w};
             float df[D];
 #pragma unroll
@@ -84,8 +98,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const int dx = c & 1, dy = c >> 1;
-                const uint32_t lim = c == 3 ? cur[c].x : (c == 2 ? cur[c].y : (c == 1 ? cur[c].z : cur[c].w));   // list 3 - c
-                if (!in[c] || r >= lim) continue;                          // behind the cut-off: exactly 0
+                if (r >= s_lim[lo][c]) continue;                           // behind the cut-off or outside the image: exactly 0
                 const float wx = dx ? r0.x : 1.f - r0.x, wy = dy ? r0.y : 1.f - r0.y;
                 const float Ta = tc[c] * (r0.z * (wx * wy));
                 const float dl = dc[c];
@@ -95,8 +108,8 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(const Header* __restri
                 dv += (dy ? wx : -wx) * dl;
                 const float Tg = io.scale * Ta;                            // the gradient image's scale, applied once (1: exact)
 #pragma unroll
-                for (int v = 0; v < D / 4; ++v) {
-                    const float4 t = gp[c][v];
+                for (int v = 0; v < FV; ++v) {
+                    const float4 t = s_g[lo][c][v];
                     df[4 * v] += Tg * t.x; df[4 * v + 1] += Tg * t.y; df[4 * v + 2] += Tg * t.z; df[4 * v + 3] += Tg * t.w;
                 }
             }

@@ -288,6 +288,7 @@ __global__ void k_check_backward(Header* h, int W, int H, int D, uint32_t N) {
     h->bwd_ok = st == INPC_OK ? 1u : 0u;
     if (st != INPC_OK) h->status = st;
     for (int b = 0; b < kMaxBands; ++b) h->band_cursor[b] = 0;
+    h->combine_cursor = 0;
 }
 
 // ---- band plan + the library's own side stream --------------------------------------------------------------------
