@@ -83,7 +83,8 @@ struct Header {
     int32_t  status;               // sticky inpc_status of device-side checks (read by inpc_raster_get_status)
     uint32_t ord_cursor;           // bump allocator of the per-tile blocks of the saved blend order (entries)
     uint32_t combine_cursor;       // work cursor of k_combine (reset by the backward pass's header check)
-    uint32_t pad[7];
+    uint32_t combine_q_head, combine_q_tail, combine_done;   // queue of the parts of large units (k_combine)
+    uint32_t pad[4];
     // Tile work items, one list per BAND of tile rows (kMaxBands bands): a band's tiles can be blended as soon as
     // its cell rows are sorted, while the next band's cells are still being sorted on another stream.
     uint32_t band_items[8];        // items of band b

@@ -21,7 +21,8 @@
 namespace inpc {
 
 constexpr int kGradThreads = 256;
-constexpr int kGradCells   = 128;      // cells per work unit: small, so that a unit full of deep cells does not become one CTA's tail
+constexpr int kGradCells   = 128;      // cells per work unit
+constexpr int kGradPart    = 4096;     // a unit with more records than this is cut into parts of this many (see k_combine)
 
 template <int D> __host__ __device__ constexpr int gpt_floats() { return D == 4 ? 8 : 16; }
 
@@ -33,7 +34,7 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(Header* __restrict__ h
                                                            const float4* __restrict__ gT, const float4* __restrict__ gD,
                                                            const uint4* __restrict__ pcur,
                                                            const float* __restrict__ g_feat, ImageIO io,
-                                                           float* __restrict__ gpt) {
+                                                           float* __restrict__ gpt, unsigned long long* __restrict__ queue) {
     constexpr int GP = gpt_floats<D>();
     constexpr int FV = D / 4;
     __shared__ uint32_t s_off[kGradCells + 1];
@@ -41,15 +42,41 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(Header* __restrict__ h
     // image) and that pixel's image gradient, loaded ONCE per cell -- every record of a cell needs the same four pixels
     __shared__ uint32_t s_lim[kGradCells][4];
     __shared__ float4   s_g[kGradCells][4][FV];
-    __shared__ uint32_t s_unit;
+    __shared__ uint32_t s_unit, s_part;
     const int tid = threadIdx.x;
     if (!hdr->bwd_ok) return;
-    while (true) {                                        // units are handed out dynamically: their record counts differ widely
+    const uint32_t n_units = unit_end - unit_begin;
+    // Units (kGradCells cells) are handed out dynamically.  Their record counts differ by orders of magnitude (a cell
+    // holds anything from 0 to tens of thousands of records), so a unit with more than kGradPart records is cut into
+    // parts: the CTA that draws the unit takes part 0 and queues the others (queue[]: unit | part << 32); a CTA that
+    // finds no unit left takes parts from the queue.  A CTA that queues parts keeps drawing work itself afterwards, so
+    // every queued part is taken by someone.
+    while (true) {
         __syncthreads();
-        if (tid == 0) s_unit = atomicAdd(&hdr->combine_cursor, 1u);
+        if (tid == 0) {
+            uint32_t u = atomicAdd(&hdr->combine_cursor, 1u), part = 0u;
+            if (u >= n_units) {
+                // take a ticket; it is good once the queue has grown past it, and void once every unit has been drawn and
+                // has queued what it was going to queue (combine_done == n_units: the tail is final)
+                u = 0xFFFFFFFFu;
+                const uint32_t t = atomicAdd(&hdr->combine_q_head, 1u);
+                while (true) {
+                    const bool final = *reinterpret_cast<volatile uint32_t*>(&hdr->combine_done) >= n_units;
+                    __threadfence();
+                    if (t < *reinterpret_cast<volatile uint32_t*>(&hdr->combine_q_tail)) {
+                        unsigned long long e;                                                      // (queue[] starts out as all ones)
+                        while ((e = *reinterpret_cast<volatile unsigned long long*>(&queue[t])) == ~0ull) { }   // its writer is about to store it
+                        u = (uint32_t)e; part = (uint32_t)(e >> 32);
+                        break;
+                    }
+                    if (final) break;
+                }
+            }
+            s_unit = u; s_part = part;
+        }
         __syncthreads();
-        const uint32_t unit = unit_begin + s_unit;
-        if (unit >= unit_end) break;
+        if (s_unit == 0xFFFFFFFFu) break;
+        const uint32_t unit = unit_begin + s_unit, part = s_part;
         const uint32_t c0 = unit * kGradCells, nc = min((uint32_t)kGradCells, C - c0);
         for (uint32_t c = tid; c <= nc; c += kGradThreads) s_off[c] = __ldg(&celloff[c0 + c]);
         for (uint32_t e = tid; e < nc * 4u; e += kGradThreads) {
@@ -77,7 +104,18 @@ __global__ void __launch_bounds__(kGradThreads) k_combine(Header* __restrict__ h
             for (int v = 0; v < FV; ++v) s_g[cl][c][v] = g[v];
         }
         __syncthreads();
-        const uint32_t S = s_off[0], E = s_off[nc];
+        const uint32_t S0 = s_off[0], E0 = s_off[nc];
+        const uint32_t n_parts = (E0 - S0 + kGradPart - 1) / kGradPart;
+        if (part == 0u && tid == 0) {                            // queue the other parts of a large unit
+            if (n_parts > 1u) {
+                const uint32_t at = atomicAdd(&hdr->combine_q_tail, n_parts - 1u);
+                for (uint32_t q = 1; q < n_parts; ++q)
+                    *reinterpret_cast<volatile unsigned long long*>(&queue[at + q - 1u]) = (unsigned long long)s_unit | ((unsigned long long)q << 32);
+            }
+            __threadfence();
+            atomicAdd(&hdr->combine_done, 1u);
+        }
+        const uint32_t S = S0 + part * kGradPart, E = min(E0, S + (uint32_t)kGradPart);
         uint32_t lo = 0;                                         // a thread's slots ascend: the search resumes at its last cell
         for (uint32_t slot = S + tid; slot < E; slot += kGradThreads) {
             // the record's own (coalesced) loads first: they do not depend on the cell search

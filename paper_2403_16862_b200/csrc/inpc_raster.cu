@@ -288,7 +288,7 @@ __global__ void k_check_backward(Header* h, int W, int H, int D, uint32_t N) {
     h->bwd_ok = st == INPC_OK ? 1u : 0u;
     if (st != INPC_OK) h->status = st;
     for (int b = 0; b < kMaxBands; ++b) h->band_cursor[b] = 0;
-    h->combine_cursor = 0;
+    h->combine_cursor = 0; h->combine_q_head = 0; h->combine_q_tail = 0; h->combine_done = 0;
 }
 
 // ---- band plan + the library's own side stream --------------------------------------------------------------------
@@ -523,25 +523,20 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     A.ord = reinterpret_cast<const uint16_t*>(ws + L.ord);
     A.W = W; A.H = H; A.gT = gT; A.pcur = pcur; A.g_feat = g_feat; A.g_alpha = g_alpha; A.gD = gD; A.io = io;
     const Bands Bf = make_bands(W, H, L.C, kDefaultBands);     // the plan the forward built the item lists with
-    uint32_t u0 = 0;
     for (int b = 0; b < Bf.plan.n_bands; ++b) {
         A.items = items + Bf.plan.item_base[b]; A.n_items = &hdr->band_items[b]; A.item_cursor = &hdr->band_cursor[b];
         A.ordinfo = reinterpret_cast<const uint2*>(ws + L.ordinfo) + Bf.plan.item_base[b];
         rc = launch_back<D>(A, di, st);
         if (rc != INPC_OK) return rc;
-        const uint32_t u1 = Bf.comb_end[b];
-        if (u1 > u0) {
-            INPC_CUDA(fork(st, s2));                                          // band b is walked: combine its cells
-            { StageTimer tm(kStCombine, s2);
-              constexpr uint32_t kSub = kCsCells / kGradCells;               // the band plan counts kCsCells-cell units
-              const uint32_t g0 = u0 * kSub, g1 = std::min<uint32_t>(u1 * kSub, (L.C + kGradCells - 1) / kGradCells);
-              k_combine<D><<<(int)std::min<uint32_t>(g1 - g0, (uint32_t)di.sms * 8), kGradThreads, 0, s2>>>(
-                  hdr, celloff, L.C, g0, g1, W, H, Ra, reinterpret_cast<const float4*>(gT),
-                  reinterpret_cast<const float4*>(gD), pcur, g_feat, io, gpt); }
-            INPC_LAUNCHED(kname<D>("k_combine"));
-            u0 = u1;
-        }
     }
+    { StageTimer tm(kStCombine, st);                                          // every fragment is walked: combine the records
+      const uint32_t n_units = (L.C + kGradCells - 1) / kGradCells;
+      // the queue of parts lives in the large-cell sort's key scratch (dead since the forward pass): <= N / kGradPart entries
+      INPC_CUDA(cudaMemsetAsync(ws + L.bigkeys, 0xFF, ((size_t)N / kGradPart + 2) * 8, st));
+      k_combine<D><<<(int)std::min<uint32_t>(n_units, (uint32_t)di.sms * 8), kGradThreads, 0, st>>>(
+          hdr, celloff, L.C, 0u, n_units, W, H, Ra, reinterpret_cast<const float4*>(gT),
+          reinterpret_cast<const float4*>(gD), pcur, g_feat, io, gpt, reinterpret_cast<unsigned long long*>(ws + L.bigkeys)); }
+    INPC_LAUNCHED(kname<D>("k_combine"));
     INPC_CUDA(fork(s2, st));                                                  // join
     { StageTimer tm(kStSplit, st);
       const int grid = (int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16);
