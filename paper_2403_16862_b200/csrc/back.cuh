@@ -81,7 +81,18 @@ __device__ __forceinline__ void back_prefetch(const BackArgs& A, uint32_t item_i
     if (tid < tw * th && X + lx0 < W && Y + ly0 < H) {
         const size_t p0 = (size_t)(Y + ly0) * W + X + lx0;
         P.cn = __ldg(&A.pcur[p0]);
-        load_pixel_grad<D>(A.io, A.g_feat, A.g_alpha, p0, P.g, P.gA);
+        // raw loads only: nothing here may wait for a load (the values are scaled when they go to shared memory)
+        if (!A.io.planar) {
+#pragma unroll
+            for (int v = 0; v < D / 4; ++v) {
+                const float4 t = __ldg(reinterpret_cast<const float4*>(A.g_feat + p0 * D) + v);
+                P.g[4 * v] = t.x; P.g[4 * v + 1] = t.y; P.g[4 * v + 2] = t.z; P.g[4 * v + 3] = t.w;
+            }
+        } else {
+#pragma unroll
+            for (int d = 0; d < D; ++d) P.g[d] = __ldg(A.g_feat + (size_t)d * A.io.P + p0);
+        }
+        P.gA = A.g_alpha ? __ldg(A.g_alpha + p0) : 0.f;
     }
     if (tid == 0) P.info = __ldg(&A.ordinfo[item_i]);
 }
@@ -134,8 +145,8 @@ __global__ void __launch_bounds__(kTileThreads, 384 / kTileThreads) k_back(BackA
         if (tid + kTileThreads < (th + 1) * ws) s_off[tid + kTileThreads] = P.off1;
         s_cn[tid] = P.cn;
 #pragma unroll
-        for (int d = 0; d < D; ++d) s_g[tid][d] = P.g[d];
-        s_g[tid][D] = P.gA;
+        for (int d = 0; d < D; ++d) s_g[tid][d] = A.io.scale * P.g[d];     // as load_pixel_grad: the gradient image's scale
+        s_g[tid][D] = A.io.scale * P.gA;
         if (tid == 0) s_ordn = P.info.y;
         const uint32_t ord_base = P.info.x;               // (thread 0)
         const uint32_t n_bl = P.cn.x + P.cn.y + P.cn.z + P.cn.w;
