@@ -8,9 +8,9 @@ inputs and compare them element by element (BASELINE.json north_star tolerances)
   fused per-point blending weights (f1, Eq. 3 input)   : max abs error <= 1e-5, EVERY point
 
 Every workload is run in the three launch configurations that exist:
-  A  flags SAVE_FOR_BACKWARD | SAVE_SORTED  (k_blend<D,1>, k_big<D,1>): counts, order, per-fragment transmittance
-  B  flags bench.FLAGS_STEP  (= SAVE_FOR_BACKWARD; k_blend<D,0>, k_big<D,0>): what bench.py's fwd+bwd step times
-  C  flags bench.FLAGS_FWD   (= 0): what bench.py's forward-only figure times
+  A  flags SAVE_FOR_BACKWARD | SAVE_SORTED  (k_blend<D,SAVE=1,DUMP=1>, k_big<D,1>): counts, order, per-fragment transmittance
+  B  flags bench.FLAGS_STEP  (= SAVE_FOR_BACKWARD; k_blend<D,1,0>, k_big<D,0>): what bench.py's fwd+bwd step times
+  C  flags bench.FLAGS_FWD   (= 0; k_blend<D,0,0>): what bench.py's forward-only figure times
 and image / alpha of A, B and C and the gradients of A and B are each compared with the oracle (and with one
 another, bit for bit: there are no atomics in the value path).
 
