@@ -20,8 +20,10 @@
  *
  * Memory, ownership, streams
  *   - Every pointer is DEVICE memory owned by the caller unless marked "host".  The library allocates
- *     no device memory and keeps no state between calls, on the host or on the device: scratch and the
- *     state saved for the backward pass live in the caller's `workspace`, which starts with a small
+ *     no device memory and keeps no state between calls, on the host or on the device (apart from one
+ *     side stream, a few events and an occupancy figure per device, created on first use): scratch and the
+ *     state saved for the backward pass (per-fragment transmittances, per-pixel blended counts and the
+ *     blend order itself, 2 bytes per fragment) live in the caller's `workspace`, which starts with a small
  *     header (magic, shape, D, N, flags) the forward pass writes.  Later calls on a workspace
  *     (backward, get_*) are validated against THAT header, so a workspace may be copied, moved or
  *     freed by the caller at will; a workspace that holds no matching forward is never interpreted.

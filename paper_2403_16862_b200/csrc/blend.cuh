@@ -254,7 +254,8 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
         const uint32_t obase = DUMP ? A.pixoff[pix] : 0u;
         uint32_t so = SAVE ? smem_u32(s_ord) + 2u * s_pixbase[q] : 0u;   // next entry of this pixel's order list
         (void)so;
-        uint32_t m = min(min(h0, h1), min(h2, h3));
+        uint32_t m01 = min(h0, h1), m23 = min(h2, h3);
+        uint32_t m = min(m01, m23);
         bool p0, p1, p2, p3;
         float aA = 0.f, aB = 0.f;
         float4 fA[FV], fB[FV];
@@ -265,7 +266,8 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
 #define INPC_PICK()                                                                                                       \
         {                                                                                                                 \
             p0 = h0 == m; p1 = h1 == m; p2 = h2 == m; p3 = h3 == m;                                                       \
-            if ((p0 & (p1 | p2 | p3)) | (p1 & (p2 | p3)) | (p2 & p3)) INPC_BLEND_RESOLVE_TIE();                           \
+            /* two heads share the minimum iff the two pair minima are equal or a pair's heads are equal to it */       \
+            if ((m01 == m23) | ((h0 == h1) & p0) | ((h2 == h3) & p2)) INPC_BLEND_RESOLVE_TIE();                           \
         }
 // issue the loads of the picked fragment into set X, advance its list, recompute the minimum head
 #define INPC_SELECT(X)                                                                                                    \
@@ -287,7 +289,7 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
             h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;                                                                       \
             h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;                                                                       \
             h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;                                                                       \
-            m = min(min(h0, h1), min(h2, h3));                                                                            \
+            m01 = min(h0, h1); m23 = min(h2, h3); m = min(m01, m23);                                                      \
         }
 // composite the pending fragment of set X (Eq. 1); lists 0, 1 (corners 3, 2: bit 3 of the cursor) lie in the top cell row
 #define INPC_BLEND(X)                                                                                                     \
@@ -310,7 +312,7 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
             if constexpr (DUMP) {                                                                                         \
                 const uint32_t hk = s_dk[cur##X >> 4];                                                                    \
                 h0 = cj == 3u ? hk : h0; h1 = cj == 2u ? hk : h1; h2 = cj == 1u ? hk : h2; h3 = cj == 0u ? hk : h3;       \
-                m = min(min(h0, h1), min(h2, h3));                                                                        \
+                m01 = min(h0, h1); m23 = min(h2, h3); m = min(m01, m23);                                                  \
                 --kd;                                                                                                     \
             }                                                                                                             \
         }
@@ -354,7 +356,7 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
                 h1 = p1 ? nh : h1; ce1 = p1 ? nx : ce1;
                 h2 = p2 ? nh : h2; ce2 = p2 ? nx : ce2;
                 h3 = p3 ? nh : h3; ce3 = p3 ? nx : ce3;
-                m = min(min(h0, h1), min(h2, h3));
+                m01 = min(h0, h1); m23 = min(h2, h3); m = min(m01, m23);
             }
         }
 #undef INPC_PICK

@@ -417,6 +417,24 @@ def test_forward_is_repeatable_and_workspace_reusable():
         assert torch.equal(a, b)
 
 
+def test_backward_twice_on_split_tiles_and_large_cells():
+    """The backward pass walks the blend order the forward pass saved (ord[], one block per tile item) and hands
+    k_combine's large units through a device-side queue: both must leave the saved state intact and be re-entrant.
+    The reduced stress draw has split tiles, long-run pixels and cells of thousands of points."""
+    wl = make_workload("stress", n_points=1 << 18)
+    st = gpu_forward(wl, flags=raster.SAVE_FOR_BACKWARD)
+    g1 = [g.clone() for g in gpu_backward(wl, st, weights=True)]
+    g2 = gpu_backward(wl, st, weights=True)
+    for a, b in zip(g1, g2):
+        assert torch.equal(a, b)
+    # and a second forward into the same workspace reproduces the saved state the backward reads
+    raster.inpc_raster_forward(st["pos"], st["op"], st["feat"], wl.cam, out_feat=st["img"], out_alpha=st["alpha"],
+                               workspace=st["ws"], flags=raster.SAVE_FOR_BACKWARD)
+    g3 = gpu_backward(wl, st, weights=True)
+    for a, b in zip(g1, g3):
+        assert torch.equal(a, b)
+
+
 def _carve(nbytes, canary=0xA5, pad=1 << 16):
     """A buffer of nbytes in the middle of a larger canary-filled allocation (256-byte aligned start)."""
     whole = torch.full((nbytes + 2 * pad,), canary, dtype=torch.uint8, device="cuda")
