@@ -322,7 +322,12 @@ __global__ void __launch_bounds__(128) k_build_items(const uint32_t* __restrict_
                 if (pass == 0) ++n_it; else items[at_it++] = it;
                 continue;
             }
-            if (tw * th <= kMinTilePix) {
+            // a small sub-tile that still does not fit: its pixels go to the long-run path -- unless it misses the capacity by
+            // less than half, in which case halving it further (down to one pixel) keeps its pixels in shared memory
+            // (infer: 1784 such pixels cost 226 us as long runs, one thread each and every step a round trip to L2, and 7 us
+            // as small tiles: forward 4.36 -> 4.12 ms; stress: a cluster pixel has 10^3..10^4 fragments of which the cut-off
+            // keeps ~10^2, staging them all would be the waste, and the long-run path has 2 x 10^4 pixels to overlap)
+            if (tw * th <= kMinTilePix && (n > (uint32_t)cap + (uint32_t)cap / 2u || tw * th == 1)) {
                 for (int y = Y; y < min(Y + th, H); ++y)
                     for (int x = X; x < min(X + tw, W); ++x) {
                         if (pass == 0) { ++n_bp; n_bf += pixel_count(celloff, W, x, y); }

@@ -41,7 +41,7 @@ constexpr int kTileW       = 1 << kTileLW;    // base screen tile (pixels); halv
 constexpr int kTileH       = 8;
 constexpr int kTileLH      = 3;     // log2(kTileH)
 constexpr int kTileThreads = kTileW * kTileH;   // one thread per pixel
-constexpr int kMinTilePix  = 8;     // a sub-tile this small that still does not fit goes to the long-run path
+constexpr int kMinTilePix  = 8;     // a sub-tile this small that misses the capacity by more than 2x goes to the long-run path
 constexpr int kCellSmall   = 256;   // cells up to this many points are ranked by counting; larger: bitonic
 constexpr int kBigThreads  = 512;
 constexpr int kBigChunk    = 8192;  // keys sorted in shared memory at a time by the large-cell sort

@@ -126,7 +126,7 @@ static Layout make_layout(int64_t N, int D, int W, int H, uint32_t flags) {
     if (flags & INPC_SAVE_FOR_BACKWARD) {
         L.pcur = o; o = align_up(o + (size_t)L.P * 16);
         L.gpt = o;  o = align_up(o + n * (size_t)(D == 4 ? 32 : 64) + 64);
-        L.ord = o;  o = align_up(o + (4 * n + 8 * 16 * nbase + 64) * 2);   // blocks in 8-entry units, <= 16 items per base tile
+        L.ord = o;  o = align_up(o + (4 * n + 8 * (size_t)kTileThreads * nbase + 64) * 2);   // blocks in 8-entry units, <= one item per pixel
         L.ordinfo = o; o = align_up(o + max_items * 8);
     }
     if (flags & INPC_FUSED_SH) { L.shfeat = o; o = align_up(o + (n + 8) * 16); }
