@@ -17,6 +17,8 @@
 //   gT[4*nrec]  : transmittance in front of fragment (slot, corner), written by the forward pass
 //   gD[4*nrec]  : dL/da of fragment (slot, corner), written by the backward pass   (gT|gD reuse A's bytes)
 //   pcur[P]     : per pixel, how many records of each of its four lists were blended before the cut-off
+//   ord[], ordinfo[items] : the blend order the forward pass took, 16 bits per fragment (record * 16 + 4 * corner,
+//                 tile-local), one block per tile item; ordinfo[item] = { first entry, entries }   (blend.cuh, back.cuh)
 //   gpt[N]      : per-point gradient records (8 or 16 floats), one or two full 32-byte sectors each
 // Corner c = 2*dy + dx is the pixel's offset from the record's top-left pixel; list j of a pixel
 // (0: cell (x,y), 1: (x+1,y), 2: (x,y+1), 3: (x+1,y+1)) holds its fragments of corner 3 - j.

@@ -3,7 +3,8 @@
 //
 //   k_combine  one thread per RECORD (slot order, coalesced): reads the record's four (T, dL/da) pairs
 //              from gT / gD, decides per corner whether that fragment was blended (its position in the
-//              cell list < the pixel's stop position pcur), and forms
+//              cell list < the pixel's stop position pcur; the four corner pixels' limits and image gradients
+//              are staged once per CELL in shared memory), and forms
 //                 dL/dfeat    = sum_c T_c a_c g_img[pixel_c]            (S5)
 //                 dL/dopacity = sum_c w_c dL/da_c                        (S6)
 //                 dL/d(u, v)  = opacity * sum_c (dw_c/du, dw_c/dv) dL/da_c

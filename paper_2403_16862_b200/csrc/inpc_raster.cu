@@ -3,8 +3,9 @@
 //
 // Forward  = memset | k_write_header | k_project_count | k_scan_u32 | k_scatter | k_classify | k_cellsort |
 //            k_cellsort_big x2 | [k_scan_u32 (dump)] | k_build_items | k_blend | k_big<fwd>
-// Backward = k_check_backward | k_back | k_big<bwd> | k_combine | k_split
-// All on the caller's stream, no host synchronisation.  No device memory is allocated here, no state is kept
+// Backward = k_check_backward | k_big<bwd> | k_back | memset(queue) | k_combine | k_split
+// All ordered on the caller's stream (k_classify / k_build_items run on a library-owned side stream that is forked from
+// and joined back into it with events), no host synchronisation.  No device memory is allocated here, no state is kept
 // on the host between calls (what a later call needs to know about a workspace is read from the Header the
 // forward pass wrote into it), and there is no CPU fallback.
 #include "../../include/inpc_raster.h"
