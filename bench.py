@@ -335,7 +335,8 @@ def ncu_traffic(workload: str) -> dict:
 def traffic_of_stage(traffic: dict, stage: str, D: int = 4, save: bool = True):
     """Stage names carry no template arguments; the capture's kernel names do: k_blend<D, SAVE, DUMP>,
     k_big<D, MODE> (0 forward, 2 backward), k_cellsort_big<D, THREADS, CHUNK> (two launches per stage: summed)."""
-    want = {"k_blend": f"k_blend<{D}, {1 if save else 0}, 0>", "k_big_fwd": f"k_big<{D}, 0>", "k_big_bwd": f"k_big<{D}, 2>"}
+    want = {"k_blend": f"k_blend<{D}, {1 if save else 0}, 0>", "k_big_fwd": f"k_big<{D}, 0>", "k_big_bwd": f"k_big<{D}, 2>",
+            "k_scatter": "k_scatter<0>", "k_split": f"k_split<{D}, 0>"}          # <1> / <D, 1>: the fused-SH variants (next_rows)
     if stage in want:
         return traffic.get(want[stage])
     vals = [v for k, v in traffic.items() if not k.startswith("_") and k.split("<")[0] == stage
