@@ -247,6 +247,8 @@ def workload_config(wl, args, n_sets: int = 1) -> dict:
                         f"{wl.cam.width}x{wl.cam.height}, D={wl.D}, seed {wl.seed}",
             "n_points": wl.N, "width": wl.cam.width, "height": wl.cam.height, "D": wl.D,
             "pass": "forward + backward (grad_feat, grad_opacity, grad_uv)" if wl.backward else "forward only (feature image + alpha)",
+            "point_order": "leaf-coherent (Morton order of the octree grid: secondary measurement)" if getattr(args, "order", "sampler") == "leaf"
+                           else "unordered sampler output (random permutation)",
             "parallelism": "replicas only (one cloud per GPU, no data-path collective)",
             "l2_hygiene": "inputs + records larger than L2 (see l2 key)" if n_sets == 1 else
                           f"working set fits L2: {n_sets} independent buffer sets rotated (see l2 key)"}
@@ -477,6 +479,9 @@ def run_ours(args) -> int:
     assert FLAGS_STEP == raster.SAVE_FOR_BACKWARD
 
     wl = make_workload(args.workload, seed=CONFIGS[args.workload]["seed"] + rank)
+    if args.order == "leaf":                              # SURVEY 8d's secondary measurement; the headline order is the sampler's
+        from paper_2403_16862_b200.workloads import leaf_coherent_order
+        wl = leaf_coherent_order(wl)
     W, H, D, N = wl.cam.width, wl.cam.height, wl.D, wl.N
     stream = torch.cuda.current_stream()
     # L2 hygiene: a working set that fits the 126 MB L2 would be timed L2-warm, so small workloads rotate through
@@ -748,6 +753,8 @@ def main(argv=None) -> int:
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default="train", choices=["tiny", "1m", "train", "infer", "stress"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--order", default="sampler", choices=["sampler", "leaf"],
+                    help="point storage order: the unordered sampler output (headline) or leaf-coherent (secondary, SURVEY 8d)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle leg (profiling runs)")
     ap.add_argument("--no-stats", action="store_true", help="skip the workload statistics (profiling runs)")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the timings of the NEXT rows f1-f4 (profiling runs)")

@@ -212,6 +212,22 @@ def make_workload(name: str, n_points: int | None = None, seed: int | None = Non
                     backward=bool(cfg["backward"]), seed=seed)
 
 
+def leaf_coherent_order(wl: Workload, bits: int = 10) -> Workload:
+    """The same cloud with its points stored in a leaf-coherent order (the secondary measurement; the
+    headline is the unordered multinomial sampler output): a stable sort by the 3-D Morton code of the
+    position on the 2^bits grid of the octree's root cube [-32,32]^2 x [0,64] -- points of one leaf become contiguous,
+    leaves follow a z-order curve.  Only the storage order changes; no value does."""
+    q = np.clip(((wl.pos.astype(np.float64) - np.array([-32.0, -32.0, 0.0])) / 64.0 * (1 << bits)).astype(np.int64), 0, (1 << bits) - 1)
+    code = np.zeros(wl.N, dtype=np.int64)
+    for b in range(bits):
+        for a in range(3):
+            code |= ((q[:, a] >> b) & 1) << (3 * b + a)
+    order = np.argsort(code, kind="stable")
+    return Workload(name=wl.name + "+leaf-coherent", pos=np.ascontiguousarray(wl.pos[order]),
+                    opacity=np.ascontiguousarray(wl.opacity[order]), feat=np.ascontiguousarray(wl.feat[order]),
+                    cam=wl.cam, g_img=wl.g_img, g_alpha=wl.g_alpha, backward=wl.backward, seed=wl.seed)
+
+
 def make_octree(n_leaves: int = 1 << 16, seed: int = 7, cam: dict = CAM_1297, root_side: float = 64.0):
     """Synthetic probability octree for the view-specific sampler (NEXT row f4; PAPER.md:62-84 describes the real
     one, which needs the optimisation loop): leaves of levels 4..12 of the root cube [-32,32]^2 x [0,64] placed on
