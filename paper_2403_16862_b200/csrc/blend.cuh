@@ -135,10 +135,6 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
         }
         if (tid < 64) s_hist[tid] = 0;
         __syncthreads();
-        if (tid == 32) {                                  // fetch the next work item while this one is processed
-            const uint32_t nx = atomicAdd(A.item_cursor, 1u);
-            s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
-        }
         if (tid < 32) {                                   // warp 0: one lane per cell row issues that row's copies
             const bool row = tid <= th;
             uint32_t a4 = 0, len = 0;
@@ -209,6 +205,12 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
         if constexpr (SAVE) { if (tid == 0) bulk_wait_read(); }       // the previous tile's order lists have left shared memory
         __syncthreads();
 
+        // The next work item is drawn HERE, behind the tile's last set-up barrier: its two dependent round trips (ticket,
+        // item code) used to sit between two of those barriers, where the whole CTA waited for them.
+        if (tid == kTileThreads - 1) {
+            const uint32_t nx = atomicAdd(A.item_cursor, 1u);
+            s_next = nx; s_next_code = nx < n_items ? A.items[nx] : 0u;
+        }
         // ---------------------------------------------------------------- 3. one thread per pixel
         const int q = s_perm[tid];
         const int ly = q >> lw, lx = q & (tw - 1);
