@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
     float4*   s_f  = reinterpret_cast<float4*>(smem + (size_t)CAP * 20);
     const unsigned char* s_ab = smem + (size_t)CAP * 4;
     uint16_t* s_ord = reinterpret_cast<uint16_t*>(smem + (size_t)CAP * (20 + 16 * FV));   // SAVE only
-    __shared__ uint32_t s_pixbase[kTileThreads], s_wsum[kTileThreads / 32], s_ordtot;     // SAVE: starts of the tile's order lists
+    __shared__ uint32_t s_pixbase[kTileThreads], s_wsum[kTileThreads / 32], s_ordtot, s_ordbase;   // SAVE: starts of the tile's order lists, its block of ord[]
 
     __shared__ uint32_t s_off[kTileH + 1][kTileW + 2];
     __shared__ uint32_t s_sbase[kTileH + 1], s_a4row[kTileH + 1];
@@ -105,7 +105,6 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
     }
     uint32_t parity = 0;
     bool have_prev = false;                               // SAVE: the previous item's order lists still sit in shared memory
-    uint32_t p_item = 0;
 
     while (true) {
         __syncthreads();                                  // everyone is done with the previous item's smem
@@ -114,9 +113,7 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
             // one block: a bulk store issued by one thread; it has finished reading before this tile's walk overwrites them.
             if (tid == 0 && have_prev) {
                 const uint32_t n8 = (s_ordtot + 7u) & ~7u;
-                const uint32_t base = n8 ? atomicAdd(A.ord_cursor, n8) : 0u;
-                A.ordinfo[p_item] = make_uint2(base, s_ordtot);
-                if (n8) { fence_proxy_async(); bulk_s2g(A.ord + base, s_ord, n8 * 2u); }
+                if (n8) { fence_proxy_async(); bulk_s2g(A.ord + s_ordbase, s_ord, n8 * 2u); }
             }
         }
         const uint32_t item_i = s_next;
@@ -181,8 +178,13 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
 #pragma unroll
             for (int w = 0; w < kTileThreads / 32; ++w) before += w < (tid >> 5) ? s_wsum[w] : 0u;
             s_pixbase[tid] = before + inc_mine - n_mine;
-            if (tid == kTileThreads - 1) s_ordtot = before + inc_mine;
-            have_prev = true; p_item = item_i;
+            if (tid == kTileThreads - 1) {                 // this tile's block of ord[]: reserved here, off warp 0's path
+                const uint32_t total = before + inc_mine, n8 = (total + 7u) & ~7u;
+                const uint32_t base = n8 ? atomicAdd(A.ord_cursor, n8) : 0u;
+                s_ordtot = total; s_ordbase = base;
+                A.ordinfo[item_i] = make_uint2(base, total);
+            }
+            have_prev = true;
         }
         if (tid < 32) {                                                // exclusive scan of the 64 buckets
             const uint32_t h0 = s_hist[2 * tid], h1 = s_hist[2 * tid + 1];
