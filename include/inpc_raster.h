@@ -64,7 +64,8 @@ typedef enum inpc_status {
     INPC_ERR_CUDA                = -3,  /* launch failure or sticky error; see inpc_raster_last_cuda_error   */
     INPC_ERR_NO_SAVED_STATE      = -4,  /* backward / get_* on a workspace no matching forward has filled (get_* return
                                            it at once; for backward it is reported by inpc_raster_get_status)  */
-    INPC_ERR_UNSUPPORTED         = -5   /* D not in {4, 8}, W or H > 4095                                     */
+    INPC_ERR_UNSUPPORTED         = -5,  /* D not in {4, 8}, W or H > 4095                                     */
+    INPC_ERR_STATIC_LIMIT        = -6   /* inpc_sample_view_static: n_leaves > inpc_sample_static_max_leaves()  */
 } inpc_status;
 
 /* flags of inpc_raster_forward / inpc_raster_workspace_bytes */
@@ -225,6 +226,30 @@ int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const 
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
 int inpc_sample_get_stats(const void* workspace, uint64_t* n_valid, uint64_t* cdf_total, double* max_weight,
                           void* cuda_stream);
+
+/* ---- The sampler for callers that cannot allocate device memory. ---------------------------------------------
+ * inpc_sample_view needs a workspace, and somebody has to cudaMalloc it.  Not every caller can: a plugin inside a
+ * host application whose allocator owns the whole GPU, a frame loop that must never hit cudaMalloc's device-wide
+ * synchronisation, a process that is already at its memory budget.  inpc_sample_view_static is the same sampler
+ * (same kernels, same checks, bit-identical pos / leaf) with its scratch in a fixed array that is part of the
+ * library image, so the call itself and everything under it allocates and frees nothing.
+ *   Limit:  n_leaves <= inpc_sample_static_max_leaves() = 262,144 (2^18).  More returns INPC_ERR_STATIC_LIMIT
+ *           and enqueues nothing; use inpc_sample_view with a workspace of your own then.
+ *   Cost:   the array is 4,195,840 bytes (16 per leaf + 1.5 KB) of every GPU that loads this library, from module
+ *           load to process exit, used or not.
+ *   Set-up: the first call on each device looks up that device's address of the array (cudaGetSymbolAddress, with
+ *           that device current; no allocation, but it may make the runtime load the module).  Make that first
+ *           call outside any stream capture.  Later calls on the device do no set-up.
+ *   Sharing: there is ONE array per device and every call on that device uses it.  The call clears the words
+ *           that must start at zero and overwrites the rest before reading it, so leftovers of the previous call are
+ *           harmless -- but two calls that are in flight on the GPU at the same time (different streams, or
+ *           different host threads on different streams) write over each other and both results are garbage.
+ *           Calls on one stream are ordered and safe.  The statistics of inpc_sample_get_stats are not available.
+ * pos[N][3], leaf[N] and the leaf arrays are the caller's device buffers exactly as for inpc_sample_view. */
+int64_t inpc_sample_static_max_leaves(void);
+int inpc_sample_view_static(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
+                            float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
+                            void* cuda_stream);
 
 const char* inpc_raster_strerror(int status);
 /* CUDA error string of the last INPC_ERR_CUDA on this thread ("" if none). */

@@ -871,6 +871,53 @@ int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const 
     return INPC_OK;
 }
 
+// ---- inpc_sample_view for callers that cannot allocate device memory ------------------------------------------------
+// Some users of the sampler have no way to obtain a workspace: a renderer plugin running inside a host application
+// that has handed the whole GPU to its own memory pool, a real-time loop in which cudaMalloc's implicit device-wide
+// synchronisation is forbidden, code that runs after the process has hit its memory budget.  For them the sampler's
+// scratch (p^, the integer CDF, the tile sums and the three statistics words: 16 bytes per leaf plus 1.5 KB) is carved
+// out of the library image itself: the array below is part of the module, so every device that loads the library pays
+// its 4 MiB from the moment the module is loaded until the process exits, whether or not this entry point is ever used.
+//
+// g_sample_scratch is a DEVICE symbol.  The name, used in host code, is only the host-side shadow the runtime keeps
+// for it -- not an address a kernel may dereference -- so the device address is looked up per device with
+// cudaGetSymbolAddress (each device has its own copy of the array) and it is that address the kernels are given.
+constexpr int64_t kStaticSampleMaxLeaves = 1ll << 18;
+constexpr size_t kStaticSampleBytes =       // sample_layout(kStaticSampleMaxLeaves).total, spelled out so that it is a constant
+    256 + 2 * (size_t)kStaticSampleMaxLeaves * 8 + ((kStaticSampleMaxLeaves / kScan64Tile + 1) * 8 + 255) / 256 * 256;
+static __device__ __align__(256) unsigned char g_sample_scratch[kStaticSampleBytes];
+
+static void* static_sample_scratch(const DeviceInfo& di, cudaError_t* err) {
+    static void* ptr_by_dev[kMaxDevices] = {};
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    if (!ptr_by_dev[di.dev]) {                    // first call on this device (it is the current one: device_info() read it)
+        void* p = nullptr;
+        *err = cudaGetSymbolAddress(&p, g_sample_scratch);
+        if (*err != cudaSuccess) return nullptr;
+        ptr_by_dev[di.dev] = p;
+    }
+    return ptr_by_dev[di.dev];
+}
+
+int64_t inpc_sample_static_max_leaves(void) { return kStaticSampleMaxLeaves; }
+
+int inpc_sample_view_static(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
+                            float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
+                            void* cuda_stream) {
+    if (n_leaves > kStaticSampleMaxLeaves) return INPC_ERR_STATIC_LIMIT;
+    if (n_leaves >= 1 && sample_layout(n_leaves).total > sizeof(g_sample_scratch)) return INPC_ERR_STATIC_LIMIT;
+    const DeviceInfo di = device_info();
+    if (!di.ok) return cuda_fail(cudaErrorNoDevice);
+    cudaError_t e = cudaSuccess;
+    void* scratch = static_sample_scratch(di, &e);
+    if (!scratch) return cuda_fail(e);
+    // From here on this IS inpc_sample_view, with the library's array as its workspace: same kernels, same argument
+    // checks, same results.  It clears the statistics words itself and overwrites every other byte it later reads, so
+    // what an earlier call left in the array does not matter.
+    return inpc_sample_view(leaf_centre, leaf_level, leaf_prob, n_leaves, root_side, cam, seed, N, pos, leaf, scratch,
+                            sizeof(g_sample_scratch), cuda_stream);
+}
+
 int inpc_sample_get_stats(const void* workspace, uint64_t* n_valid, uint64_t* cdf_total, double* max_weight, void* cuda_stream) {
     if (!workspace) return INPC_ERR_INVALID_ARG;
     unsigned long long h[3];
@@ -891,6 +938,7 @@ const char* inpc_raster_strerror(int status) {
         case INPC_ERR_CUDA: return "CUDA error (see inpc_raster_last_cuda_error)";
         case INPC_ERR_NO_SAVED_STATE: return "workspace holds no matching forward state";
         case INPC_ERR_UNSUPPORTED: return "unsupported D or image size";
+        case INPC_ERR_STATIC_LIMIT: return "more leaves than inpc_sample_view_static's built-in scratch holds (see inpc_sample_static_max_leaves)";
         default: return "unknown status";
     }
 }

@@ -26,6 +26,7 @@ EXPORTS = (
     "inpc_raster_forward_ex", "inpc_raster_backward_ex", "inpc_raster_level_camera", "inpc_raster_forward_levels",
     "inpc_raster_forward_multisample", "inpc_raster_forward_sh", "inpc_raster_backward_sh",
     "inpc_sample_workspace_bytes", "inpc_sample_view", "inpc_sample_get_stats",
+    "inpc_sample_static_max_leaves", "inpc_sample_view_static",
     "inpc_raster_get_counts", "inpc_raster_get_blended_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
     "inpc_raster_get_status",
     "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count", "inpc_raster_launched_kernels",
@@ -86,6 +87,10 @@ def load() -> C.CDLL:
         lib.inpc_sample_workspace_bytes.argtypes = [i64]
         lib.inpc_sample_view.restype = C.c_int
         lib.inpc_sample_view.argtypes = [vp, vp, vp, i64, C.c_float, C.POINTER(InpcCamera), C.c_uint64, i64, vp, vp, vp, C.c_size_t, vp]
+        lib.inpc_sample_static_max_leaves.restype = C.c_int64
+        lib.inpc_sample_static_max_leaves.argtypes = []
+        lib.inpc_sample_view_static.restype = C.c_int
+        lib.inpc_sample_view_static.argtypes = [vp, vp, vp, i64, C.c_float, C.POINTER(InpcCamera), C.c_uint64, i64, vp, vp, vp]
         lib.inpc_sample_get_stats.restype = C.c_int
         lib.inpc_sample_get_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_double), vp]
         lib.inpc_raster_level_camera.restype = C.c_int
@@ -238,6 +243,38 @@ def inpc_sample_view(leaf_centre, leaf_level, leaf_prob, root_side: float, cam, 
     if rc != 0:
         raise InpcError(rc, "inpc_sample_view")
     return pos, leaf, workspace
+
+
+def inpc_sample_static_max_leaves() -> int:
+    return int(load().inpc_sample_static_max_leaves())
+
+
+def inpc_sample_view_static(leaf_centre, leaf_level, leaf_prob, root_side: float, cam, seed: int, N: int, pos=None, leaf=None,
+                            stream=None):
+    """inpc_sample_view without a workspace, for callers that cannot allocate device memory (a plugin under a host
+    application's memory pool, a frame loop that may not touch cudaMalloc): the scratch is a fixed 4 MiB array inside
+    the library, good for up to inpc_sample_static_max_leaves() = 2^18 leaves (InpcError -6 beyond that).  Pass
+    pre-allocated pos[N,3] float32 / leaf[N] int32 and the call allocates nothing at all; without them this wrapper
+    makes the two output tensors (the C entry point never does).  All calls on a device share the one array: keep them
+    on one stream, or otherwise ordered -- two that overlap on the GPU corrupt each other.  The first call on a device
+    looks up the array's address; make it before any stream capture.  -> (pos, leaf).  No sync."""
+    lib = load()
+    _check(leaf_centre, torch.float32, "leaf_centre"); _check(leaf_level, torch.int32, "leaf_level")
+    _check(leaf_prob, torch.float32, "leaf_prob")
+    dev = leaf_centre.device
+    cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
+    if pos is None:
+        pos = torch.empty((N, 3), dtype=torch.float32, device=dev)
+    if leaf is None:
+        leaf = torch.empty((N,), dtype=torch.int32, device=dev)
+    _check(pos, torch.float32, "pos"); _check(leaf, torch.int32, "leaf")
+    if pos.numel() != 3 * N or leaf.numel() != N:
+        raise ValueError("pos must hold N x 3 and leaf N elements")
+    rc = lib.inpc_sample_view_static(_ptr(leaf_centre), _ptr(leaf_level), _ptr(leaf_prob), int(leaf_level.shape[0]),
+                                     float(root_side), C.byref(cs), C.c_uint64(seed), N, _ptr(pos), _ptr(leaf), _stream(stream))
+    if rc != 0:
+        raise InpcError(rc, "inpc_sample_view_static")
+    return pos, leaf
 
 
 def inpc_sample_get_stats(workspace, stream=None) -> dict:

@@ -114,3 +114,17 @@ def test_product_does_not_import_the_oracle():
                 src = open(os.path.join(dirpath, fn)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", src, flags=re.M), fn
                 assert "liboracle" not in src and "oracle.cpp" not in src, fn
+
+
+def test_static_scratch_sampler_limit_is_checked_on_the_host(lib):
+    """inpc_sample_view_static (the sampler for callers that cannot allocate device memory) refuses more leaves than its
+    built-in array holds before it touches the device, with a status and a message of its own."""
+    cam = raster.InpcCamera()
+    cam.fx = cam.fy = 64.0; cam.cx = cam.cy = 32.0
+    cam.near_z, cam.far_z, cam.width, cam.height = 0.01, 100.0, 64, 64
+    fake = C.c_void_p(0x1000)
+    mx = lib.inpc_sample_static_max_leaves()
+    assert mx == 1 << 18
+    assert lib.inpc_sample_workspace_bytes(mx) == 4195840          # the size the header states for the array
+    rc = lib.inpc_sample_view_static(fake, fake, fake, mx + 1, 8.0, C.byref(cam), 1, 16, fake, fake, None)
+    assert rc == -6 and b"inpc_sample_static_max_leaves" in lib.inpc_raster_strerror(rc)
