@@ -213,7 +213,8 @@ int inpc_raster_get_stats(const void* workspace, inpc_stats* stats, void* cuda_s
  * Leaves of the probability octree: leaf_centre[L][3] (world), leaf_level[L] (side = root_side / 2^level),
  * leaf_prob[L] in [0,1]; L <= 2^24 (the paper's 256^3 cap).  Each leaf gets the weight
  *   p^ = visible * p / (d * 2^(level * 0.5)),   d = max(|z_view - near| / (far - near), 1e-8)
- * (visible: its centre or one of its corners is inside the view frustum), N leaves are drawn with replacement
+ * (visible: the leaf's cube can intersect the view frustum -- its centre or a corner is inside, or no frustum plane
+ * has all eight corners outside; reading R19; a leaf_level outside [0, 30] gets p^ = 0), N leaves are drawn with replacement
  * from p^ / sum p^ (inverse CDF), each draw is offset uniformly inside its leaf, and a position outside the
  * frustum is drawn again (up to 8 times; then pos = NaN, leaf = -1: the rasterizer culls it).
  * pos[N][3] and leaf[N] are outputs; the result is a pure function of the inputs and `seed` (counter-based

@@ -3,7 +3,8 @@
 the paper's order.  It shares no code with paper_2403_16862_b200/csrc/sampler.cuh; both follow the arithmetic that
 DESIGN.md section 3 (reading R19) fixes so that the drawn leaves and positions are reproducible bit for bit:
 
-  1. per leaf: z_view by the canonical fp32 projection; visible <=> centre or one of the 8 corners inside the frustum;
+  1. per leaf: z_view by the canonical fp32 projection; visible <=> the leaf's cube can intersect the frustum: centre or
+     one of the 8 corners inside it, or no frustum plane with all 8 corners on its outer side (box_outside_a_plane);
      d = max(|z_view - near| / (far - near), 1e-8) (Eq. 9) and p^ = p / (d * 2^(level / 2)) (Eq. 4, lambda_l = 0.5)
      in fp64, one rounded operation per step;
   2. integer weights w = floor(p^ / max p^ * 2^32), inclusive prefix sums in u64 = the CDF;
@@ -60,15 +61,47 @@ def inside_frustum(cam, p):
                (v >= 0) & (v < np.float32(cam.height)), zc
 
 
+MAX_LEVEL = 30      # a leaf_level outside [0, 30] never gets a sample (2^-level must be a normal fp32; the paper stops at 8)
+
+
+def box_outside_a_plane(cam, corners):
+    """corners[8][L,3] float32 (world).  True where ONE of the six frustum planes has all eight corners on its outer
+    side -- then the cube cannot meet the frustum (PAPER.md:92 property (1): such a leaf must get no samples).  The
+    planes in camera space, fp32, one rounded operation at a time: near z_c > near, far z_c < far, and the four side
+    planes through the camera centre in the division-free form of 0 <= u < W, 0 <= v < H:
+        fx x_c + cx z_c >= 0,  fx x_c + (cx - W) z_c < 0,  fy y_c + cy z_c >= 0,  fy y_c + (cy - H) z_c < 0.
+    A corner is outside a plane when the inequality is NOT satisfied (so NaN is outside of everything)."""
+    f = np.float32
+    R = np.asarray(cam.R, dtype=np.float32).reshape(9); t = np.asarray(cam.t, dtype=np.float32).reshape(3)
+    all_out = None
+    for p in corners:
+        x, y, z = p[:, 0].astype(f), p[:, 1].astype(f), p[:, 2].astype(f)
+        with np.errstate(invalid="ignore", over="ignore"):
+            xc = ((R[0] * x + R[1] * y) + R[2] * z) + t[0]
+            yc = ((R[3] * x + R[4] * y) + R[5] * z) + t[1]
+            zc = ((R[6] * x + R[7] * y) + R[8] * z) + t[2]
+            fxx, fyy = f(cam.fx) * xc, f(cam.fy) * yc
+            inside = np.stack([zc > f(cam.near_z), zc < f(cam.far_z),
+                               fxx + f(cam.cx) * zc >= 0, fxx + (f(cam.cx) - f(cam.width)) * zc < 0,
+                               fyy + f(cam.cy) * zc >= 0, fyy + (f(cam.cy) - f(cam.height)) * zc < 0], 1)
+        all_out = ~inside if all_out is None else (all_out & ~inside)
+    return all_out.any(axis=1)
+
+
 def leaf_weights(centre, level, prob, root_side, cam):
     """Eq. 4 / Eq. 9 -> p^[L] in fp64 (0 for invisible leaves)."""
     centre = np.asarray(centre, dtype=np.float32).reshape(-1, 3)
     level = np.asarray(level, dtype=np.int64)
+    level_ok = (level >= 0) & (level <= MAX_LEVEL)
+    level = np.where(level_ok, level, 0)
     half = np.float32(0.5) * (np.float32(root_side) * np.exp2(-level).astype(np.float32))
     vis, zc = inside_frustum(cam, centre)
+    corners = []
     for k in range(8):
         off = np.stack([np.where(k & 1, half, -half), np.where(k & 2, half, -half), np.where(k & 4, half, -half)], 1)
-        vis = vis | inside_frustum(cam, centre + off.astype(np.float32))[0]
+        corners.append(centre + off.astype(np.float32))
+        vis = vis | inside_frustum(cam, corners[-1])[0]
+    vis = (vis | ~box_outside_a_plane(cam, corners)) & level_ok
     near, far = np.float64(np.float32(cam.near_z)), np.float64(np.float32(cam.far_z))
     d = np.maximum(np.abs(zc.astype(np.float64) - near) / (far - near), 1e-8)              # Eq. 9
     f = np.ldexp(np.where(level & 1, 1.4142135623730951, 1.0), level >> 1)                 # 2^(level * 0.5)

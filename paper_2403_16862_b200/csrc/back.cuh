@@ -43,6 +43,8 @@ struct BackArgs {
 template <int D> __host__ __device__ constexpr size_t back_smem_bytes() {
     return (size_t)TileCfg<D>::kCap * (16 + 4 * D + 16 + 8) + 16;     // alphas, features, gT, order lists
 }
+static_assert(back_smem_bytes<4>() + 12288 <= kMaxSmemPerCta && back_smem_bytes<8>() + 12288 <= kMaxSmemPerCta,
+              "k_back: tile capacity exceeds the shared memory of one CTA (dynamic + < 12 KB static)");
 
 // What a thread loads one tile ahead: up to two entries of the (th+1) x (tw+2) window of cell offsets, its pixel's
 // (natural order) blended counts and image gradient, and (thread 0) the tile's block of the saved order.
@@ -134,6 +136,7 @@ __global__ void __launch_bounds__(kTileThreads, 384 / kTileThreads) k_back(BackA
     uint32_t parity = 0;
 
     while (true) {
+        fence_proxy_async();                              // each thread's generic accesses to the tile's arrays, before the next bulk loads overwrite them
         __syncthreads();                                  // (A) everyone is done with the previous item's smem
         const uint32_t item_i = s_next;
         if (item_i >= n_items) break;

@@ -54,6 +54,8 @@ struct BlendArgs {
 template <int D, bool SAVE> __host__ __device__ constexpr size_t blend_smem_bytes() {
     return (size_t)TileCfg<D>::kCap * (4 + 16 + 4 * D + (SAVE ? 8 : 0));
 }
+static_assert(blend_smem_bytes<4, true>() + 4096 <= kMaxSmemPerCta && blend_smem_bytes<8, true>() + 4096 <= kMaxSmemPerCta,
+              "k_blend: tile capacity exceeds the shared memory of one CTA (dynamic + < 4 KB static)");
 
 // Packed list state: low 16 bits = byte offset of the head fragment's alpha inside s_a (record * 16 +
 // 4 * corner), high 16 bits = the same for the list's end.  One record further = + 16.
@@ -107,6 +109,10 @@ __global__ void __launch_bounds__(kTileThreads, 512 / kTileThreads) k_blend(Blen
     bool have_prev = false;                               // SAVE: the previous item's order lists still sit in shared memory
 
     while (true) {
+        // Every thread's generic-proxy accesses to the tile's shared memory (the order lists it wrote, the alphas it wrote
+        // in place, the records it read) are ordered before the async-proxy copies thread 0 / warp 0 issue behind the
+        // barrier (bulk store of the order lists, bulk loads over the record arrays): each writer fences, then the barrier.
+        fence_proxy_async();
         __syncthreads();                                  // everyone is done with the previous item's smem
         if constexpr (SAVE) {
             // The previous tile's order lists (back to back in shared memory, pixels in natural order) go out to ord[] as

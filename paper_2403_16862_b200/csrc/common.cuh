@@ -54,6 +54,12 @@ constexpr uint32_t kSentHi = 0xFFFFFFFFu;   // "list exhausted" for the ascendin
 template <int D> struct TileCfg;
 template <> struct TileCfg<4> { static constexpr int kCap = INPC_CAP4; };   // records per tile item
 template <> struct TileCfg<8> { static constexpr int kCap = INPC_CAP8; };
+// The merge kernels keep a list cursor as a 16-bit byte offset "record * 16 + 4 * corner" (pack_list, the entries of
+// ord[], the (nx >> 2) & 0x3ffc mask), and stage records four at a time: INPC_CAP4 / INPC_CAP8 are build-time overridable,
+// so the limits are checked here.
+constexpr size_t kMaxSmemPerCta = 227 * 1024;    // sm_100a opt-in dynamic shared memory per CTA
+static_assert(TileCfg<4>::kCap % 4 == 0 && TileCfg<4>::kCap * 16 <= 65536, "INPC_CAP4: a multiple of 4, at most 4096 records");
+static_assert(TileCfg<8>::kCap % 4 == 0 && TileCfg<8>::kCap * 16 <= 65536, "INPC_CAP8: a multiple of 4, at most 4096 records");
 
 struct Camera {
     float fx, fy, cx, cy;

@@ -839,6 +839,7 @@ int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const 
     if (!cam || !leaf_centre || !leaf_level || !leaf_prob || !workspace || N < 0 || N >= (1ll << 31)) return INPC_ERR_INVALID_ARG;
     if (n_leaves < 1 || n_leaves > (1ll << 24) || !(root_side > 0.f)) return INPC_ERR_INVALID_ARG;
     if (cam->width <= 0 || cam->height <= 0 || !(cam->near_z < cam->far_z)) return INPC_ERR_INVALID_ARG;
+    if (!(cam->near_z >= 0.f)) return INPC_ERR_INVALID_ARG;      // the camera rule of check_common: the rasterizer refuses it too
     if (N > 0 && (!pos || !leaf)) return INPC_ERR_INVALID_ARG;
     if (reinterpret_cast<uintptr_t>(workspace) & 255u) return INPC_ERR_INVALID_ARG;
     const SampleLayout S = sample_layout(n_leaves);

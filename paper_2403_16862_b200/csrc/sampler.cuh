@@ -5,7 +5,11 @@
 //   per leaf i (centre c_i, level l_i, probability p_i, side = root_side / 2^l_i):
 //     p^_i = 1_visible * p_i / (d_i * 2^(l_i * lambda_l)),  lambda_l = 0.5                                  (Eq. 4)
 //     d_i  = max(|z_view - near| / (far - near), 1e-8)                                                      (Eq. 9)
-//     visible <=> the leaf's centre or one of its eight corners lies inside the view frustum (reading R19)
+//     visible <=> the leaf's cube can intersect the view frustum (reading R19): its centre or one of its eight corners
+//                 lies inside the frustum, OR no frustum plane has all eight corners on its outer side (the conservative
+//                 box-against-planes test: it never misses a cube the frustum enters through a face or an edge, nor
+//                 the one that contains the camera; it may admit a few cubes next to a frustum edge, whose samples the
+//                 re-draw then rejects)
 //   multinomial sampling WITH replacement: N independent draws from the distribution p^ / sum p^, by inverse CDF;
 //   every draw is offset uniformly inside its leaf's cube; a position outside the frustum is drawn again (up to
 //   kSampleAttempts times; what still fails is returned as NaN / leaf -1 and culled by the rasterizer).
@@ -23,6 +27,7 @@
 namespace inpc {
 
 constexpr int kSampleAttempts = 8;
+constexpr int kMaxLeafLevel = 30;        // leaf_level outside [0, 30] is treated as "never sampled" (the paper's octree stops at 8: 256^3)
 constexpr int kScan64Threads = 256, kScan64Items = 8, kScan64Tile = kScan64Threads * kScan64Items;
 
 __host__ __device__ __forceinline__ unsigned long long splitmix64(unsigned long long seed, unsigned long long counter) {
@@ -44,6 +49,21 @@ __device__ __forceinline__ bool in_frustum(const Camera& c, float x, float y, fl
     return u >= 0.f && u < (float)c.W && v >= 0.f && v < (float)c.H;
 }
 
+// Which of the six frustum planes the point lies OUTSIDE of (bit set), in camera space, every operation rounded on its
+// own: near / far on z_c, the four side planes through the camera centre written without the division
+// (u >= 0 <=> fx x_c + cx z_c >= 0 for z_c > 0, and the plane form stays meaningful for z_c <= 0, where u does not).
+// Each test is the negation of "inside", so a NaN coordinate counts as outside of every plane.
+__device__ __forceinline__ unsigned outside_planes(const Camera& c, float x, float y, float z) {
+    const float xc = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c.R[0], x), __fmul_rn(c.R[1], y)), __fmul_rn(c.R[2], z)), c.t[0]);
+    const float yc = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c.R[3], x), __fmul_rn(c.R[4], y)), __fmul_rn(c.R[5], z)), c.t[1]);
+    const float zc = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c.R[6], x), __fmul_rn(c.R[7], y)), __fmul_rn(c.R[8], z)), c.t[2]);
+    const float fxx = __fmul_rn(c.fx, xc), fyy = __fmul_rn(c.fy, yc);
+    const float left = __fadd_rn(fxx, __fmul_rn(c.cx, zc)), right = __fadd_rn(fxx, __fmul_rn(__fsub_rn(c.cx, (float)c.W), zc));
+    const float top = __fadd_rn(fyy, __fmul_rn(c.cy, zc)), bottom = __fadd_rn(fyy, __fmul_rn(__fsub_rn(c.cy, (float)c.H), zc));
+    return (!(zc > c.near_z) ? 1u : 0u) | (!(zc < c.far_z) ? 2u : 0u) | (!(left >= 0.f) ? 4u : 0u) | (!(right < 0.f) ? 8u : 0u) |
+           (!(top >= 0.f) ? 16u : 0u) | (!(bottom < 0.f) ? 32u : 0u);
+}
+
 // Eq. 4 / Eq. 9 per leaf; the maximum of p^ (positive doubles order like their bit patterns) by one atomic per CTA.
 __global__ void __launch_bounds__(256) k_leaf_weight(const float* __restrict__ centre, const int32_t* __restrict__ level,
                                                       const float* __restrict__ prob, uint32_t L, float root_side, Camera cam,
@@ -52,14 +72,20 @@ __global__ void __launch_bounds__(256) k_leaf_weight(const float* __restrict__ c
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < L; i += gridDim.x * blockDim.x) {
         const float x = centre[3 * i], y = centre[3 * i + 1], z = centre[3 * i + 2];
         const int l = level[i];
-        const float h = __fmul_rn(0.5f, __fmul_rn(root_side, __int_as_float((127 - l) << 23)));   // half side, exact
+        const bool level_ok = l >= 0 && l <= kMaxLeafLevel;        // outside of it 2^-l is not a normal fp32: such a leaf gets p^ = 0
+        const float h = __fmul_rn(0.5f, __fmul_rn(root_side, __int_as_float((127 - (level_ok ? l : 0)) << 23)));   // half side, exact
         float zc;
         bool vis = in_frustum(cam, x, y, z, &zc);
+        unsigned all_out = 63u;                                    // planes that have every corner so far on their outer side
 #pragma unroll
-        for (int k = 0; k < 8; ++k)
-            vis = vis || in_frustum(cam, __fadd_rn(x, (k & 1) ? h : -h), __fadd_rn(y, (k & 2) ? h : -h), __fadd_rn(z, (k & 4) ? h : -h));
+        for (int k = 0; k < 8; ++k) {
+            const float qx = __fadd_rn(x, (k & 1) ? h : -h), qy = __fadd_rn(y, (k & 2) ? h : -h), qz = __fadd_rn(z, (k & 4) ? h : -h);
+            vis = vis || in_frustum(cam, qx, qy, qz);
+            all_out &= outside_planes(cam, qx, qy, qz);
+        }
+        vis = vis || all_out == 0u;
         double p = 0.0;
-        if (vis) {
+        if (vis && level_ok) {
             const double d = fmax(__ddiv_rn(fabs(__dsub_rn((double)zc, (double)cam.near_z)),
                                             __dsub_rn((double)cam.far_z, (double)cam.near_z)), 1e-8);
             const double f = ldexp((l & 1) ? 1.4142135623730951 : 1.0, l >> 1);                  // 2^(l / 2)

@@ -302,9 +302,18 @@ def inpc_raster_forward_sh(pos, opacity, sh_coeff, cam, flags: int = SAVE_FOR_BA
     return out_feat, out_alpha, ws
 
 
+def _raise_on_device_status(workspace, stream, where: str):
+    """The backward pass validates the workspace ON THE DEVICE (does it hold the forward these arguments describe?); on
+    a mismatch its kernels do nothing and leave the gradient buffers untouched.  check=True reads that verdict back
+    (inpc_raster_get_status; synchronises the stream) and raises instead of returning uninitialised gradients."""
+    st = inpc_raster_get_status(workspace, stream)
+    if st != 0:
+        raise InpcError(st, where + " (device-side workspace check)")
+
+
 def inpc_raster_backward_sh(pos, opacity, sh_coeff, cam, grad_out_feat, grad_out_alpha, workspace, flags: int = 0,
-                            grad_scale: float = 1.0, blend_weight: bool = False, stream=None):
-    """-> (grad_sh_coeff[N,36], grad_opacity[N], grad_uv[N,2][, blend_weight[N]])."""
+                            grad_scale: float = 1.0, blend_weight: bool = False, stream=None, check: bool = False):
+    """-> (grad_sh_coeff[N,36], grad_opacity[N], grad_uv[N,2][, blend_weight[N]]).  check=True: see inpc_raster_backward."""
     lib = load()
     N = int(pos.shape[0])
     cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
@@ -318,6 +327,8 @@ def inpc_raster_backward_sh(pos, opacity, sh_coeff, cam, grad_out_feat, grad_out
                                      workspace.numel(), flags, grad_scale, _stream(stream))
     if rc != 0:
         raise InpcError(rc, "inpc_raster_backward_sh")
+    if check:
+        _raise_on_device_status(workspace, stream, "inpc_raster_backward_sh")
     return (g_c, g_o, g_uv) + ((bw,) if blend_weight else ())
 
 
@@ -349,10 +360,13 @@ def inpc_raster_forward(pos, opacity, feat, cam, out_feat=None, out_alpha=None, 
 
 def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha, workspace,
                          grad_feat=None, grad_opacity=None, grad_uv=None, stream=None, blend_weight=None,
-                         flags: int = 0, grad_scale: float = 1.0):
+                         flags: int = 0, grad_scale: float = 1.0, check: bool = False):
     """-> (grad_feat[N,D], grad_opacity[N], grad_uv[N,2]).  Enqueues on the current stream; no sync.
     With blend_weight (True, or a float32 tensor [N]) the fused per-point blending weights (Eq. 3) come back
-    as a fourth result (inpc_raster_backward_weights)."""
+    as a fourth result (inpc_raster_backward_weights).
+    check=True synchronises and raises InpcError when the device-side check found that `workspace` does not hold the
+    forward pass these arguments describe (the host call returns INPC_OK in that case and the gradients are left as
+    they were); the default stays asynchronous -- query inpc_raster_get_status yourself."""
     lib = load()
     N, D = int(pos.shape[0]), int(feat.shape[1])
     cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
@@ -377,6 +391,8 @@ def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha,
                                          _stream(stream))
         if rc != 0:
             raise InpcError(rc, "inpc_raster_backward_ex")
+        if check:
+            _raise_on_device_status(workspace, stream, "inpc_raster_backward_ex")
         return (grad_feat, grad_opacity, grad_uv) + ((blend_weight,) if blend_weight is not None else ())
     if blend_weight is not None:
         rc = lib.inpc_raster_backward_weights(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(grad_out_feat),
@@ -384,12 +400,16 @@ def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha,
                                               _ptr(blend_weight), _ptr(workspace), workspace.numel(), _stream(stream))
         if rc != 0:
             raise InpcError(rc, "inpc_raster_backward_weights")
+        if check:
+            _raise_on_device_status(workspace, stream, "inpc_raster_backward_weights")
         return grad_feat, grad_opacity, grad_uv, blend_weight
     rc = lib.inpc_raster_backward(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), _ptr(grad_out_feat),
                                   _ptr(grad_out_alpha), _ptr(grad_feat), _ptr(grad_opacity), _ptr(grad_uv),
                                   _ptr(workspace), workspace.numel(), _stream(stream))
     if rc != 0:
         raise InpcError(rc, "inpc_raster_backward")
+    if check:
+        _raise_on_device_status(workspace, stream, "inpc_raster_backward")
     return grad_feat, grad_opacity, grad_uv
 
 

@@ -384,6 +384,30 @@ def test_view_specific_sampler_is_bit_exact(n_leaves, N, pose):
     assert raster.inpc_raster_get_stats(rws)["n_kept"] == int((rleaf[:n] >= 0).sum())
 
 
+def test_sampler_sees_leaves_the_frustum_only_crosses():
+    """Leaves with neither centre nor corner inside the frustum (one contains the camera, one is entered through a face,
+    large ones around the frustum) and leaf levels outside [0, 30]: same visible set, leaves and positions as the oracle."""
+    from oracle import sampler as osampler
+    cam = Camera(fx=1100.0, fy=1100.0, cx=648.5, cy=420.0, width=1297, height=840)
+    rng = np.random.default_rng(5)
+    centre = np.concatenate([[[0, 0, 0], [20, 0, 10], [0, 0, 5], [0, 0, 6]], rng.uniform(-60, 60, (2000, 3))]).astype(np.float32)
+    level = np.concatenate([[0, 1, -3, 31], rng.integers(0, 5, 2000)]).astype(np.int32)
+    prob = np.ones(len(level), np.float32)
+    for c in (cam, cam.with_pose(*second_pose())):
+        phat = osampler.leaf_weights(centre, level, prob, 64.0, c)
+        if c is cam:
+            assert phat[0] > 0 and phat[1] > 0 and phat[2] == 0 and phat[3] == 0
+        N = 200_000
+        pos, leaf, ws = raster.inpc_sample_view(_dev(centre), _dev(level), _dev(prob), 64.0, c, seed=99, N=N)
+        torch.cuda.synchronize()
+        rpos, rleaf = osampler.sample_view(centre, level, prob, 64.0, c, seed=99, N=N)
+        assert np.array_equal(leaf.cpu().numpy(), rleaf)
+        assert np.array_equal(pos.cpu().numpy().view(np.uint32)[rleaf >= 0], rpos.view(np.uint32)[rleaf >= 0])
+        st = raster.inpc_sample_get_stats(ws)
+        assert st["cdf_total"] == int(osampler.integer_cdf(phat)[-1]) and st["max_weight"] == float(phat.max())
+        assert not np.isin(rleaf, [2, 3]).any()
+
+
 def test_sampler_edge_cases():
     from paper_2403_16862_b200.workloads import make_octree
     cam = make_workload("tiny").cam
@@ -527,6 +551,11 @@ def test_error_codes():
     big.zero_()
     raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g, None, big, grad_feat=sentinel)
     assert raster.inpc_raster_get_status(big) == -4 and float(sentinel.min()) == 7.0
+    with pytest.raises(raster.InpcError) as e:     # the binding's checked mode reads the device's verdict back and raises
+        raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g, None, big, grad_feat=sentinel, check=True)
+    assert e.value.status == -4 and float(sentinel.min()) == 7.0
+    ok = gpu_forward(wl)                            # ... and stays silent on a matching workspace
+    raster.inpc_raster_backward(ok["pos"], ok["op"], ok["feat"], wl.cam, g, None, ok["ws"], check=True)
     with pytest.raises(raster.InpcError) as e:
         raster.inpc_raster_get_counts(big, 64, 64)
     assert e.value.status == -4

@@ -95,3 +95,71 @@ def test_determinism_and_seed():
     # no visible leaf: everything invalid
     e = sampler.sample_view(np.array([[0, 0, -5.0]], np.float32), [8], [1.0], 64.0, CAM, seed=1, N=10)
     assert (e[1] == -1).all() and np.isnan(e[0]).all()
+
+
+def test_inside_frustum_golden_borders():
+    """oracle.sampler.inside_frustum against hand-derived border points (tests/golden/frustum_points.txt): which of
+    u = 0, u = W, v = 0, v = H, z = near, z = far belong to the frustum, under two poses."""
+    poses = [(np.eye(3), np.zeros(3)), (np.array([[0, 0, -1.0], [0, 1, 0], [1, 0, 0]]), np.array([0, 0, 1.0]))]
+    cam = Camera(fx=1024.0, fy=1024.0, cx=648.5, cy=420.0, width=1297, height=840)
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "frustum_points.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 18
+    for r in rows:
+        p = np.array([[float(r[1]), float(r[2]), float(r[3])]])
+        assert np.array_equal(p.astype(np.float32).astype(np.float64), p), "fixture value is not an fp32 number"
+        got = sampler.inside_frustum(cam.with_pose(*poses[int(r[0])]), p)[0][0]
+        assert bool(got) == bool(int(r[4])), r
+
+
+def _cube_meets_frustum_brute_force(cam, centre, side, n=40):
+    """Does any point of a dense n^3 lattice of the cube (faces included) lie inside the frustum?  Plain fp64 pinhole
+    projection, nothing shared with the oracle's plane test."""
+    g = np.linspace(-0.5, 0.5, n)
+    q = centre[None, :] + side * np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    R = np.asarray(cam.R, np.float64).reshape(3, 3); t = np.asarray(cam.t, np.float64)
+    pc = q @ R.T + t
+    z = pc[:, 2]
+    ok = (z > cam.near_z) & (z < cam.far_z)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        u = cam.fx * pc[:, 0] / z + cam.cx; v = cam.fy * pc[:, 1] / z + cam.cy
+    return bool((ok & (u >= 0) & (u < cam.width) & (v >= 0) & (v < cam.height)).any())
+
+
+def test_visibility_never_misses_a_leaf_the_frustum_enters():
+    """Eq. 4's indicator must be 1 for every leaf whose volume intersects the frustum (PAPER.md:322 speaks of "leaves
+    whose volume intersects the faces of the viewing frustum" as sampled leaves), also when neither the centre nor a
+    corner is inside: a leaf that contains the camera, one the frustum crosses through a face.  Hand-built cases, then
+    brute force on large random leaves; and one leaf behind each of the six frustum planes must get p^ = 0."""
+    one = lambda c, l: sampler.leaf_weights(np.array([c], np.float64), [l], [1.0], 64.0, CAM)[0]
+    # contains the frustum apex: cube [-32, 32]^3 around the camera; all corners project outside or lie behind
+    assert not sampler.inside_frustum(CAM, np.array([[0, 0, 0.0]]))[0][0]
+    assert one([0, 0, 0], 0) > 0
+    # crossed through its face x = 4: cube [4,36] x [-16,16] x [-6,26]; the frustum point (4, 0, 26) is on that face,
+    # the corners at z = 26 project to v = 420 +- 677 (above and below the image), the centre to u = 2848
+    assert _cube_meets_frustum_brute_force(CAM, np.array([20.0, 0, 10]), 32.0)
+    assert one([20, 0, 10], 1) > 0
+    # side 8 cubes separated by exactly one plane each: left, right, top, bottom, near (behind the camera), far
+    for c in ([-30, 0, 10], [30, 0, 10], [0, -30, 10], [0, 30, 10], [0, 0, -10], [0, 0, 120]):
+        assert not _cube_meets_frustum_brute_force(CAM, np.array(c, np.float64), 8.0, n=12)
+        assert one(c, 3) == 0.0, c
+    # brute force: leaves of side 64 .. 8 scattered around both poses
+    rng = np.random.default_rng(11)
+    for cam in (CAM, CAM.with_pose(*second_pose())):
+        centre = rng.uniform(-60, 60, (300, 3)); level = rng.integers(0, 4, 300)
+        phat = sampler.leaf_weights(centre, level, np.ones(300), 64.0, cam)
+        c32 = centre.astype(np.float32).astype(np.float64)
+        meets = np.array([_cube_meets_frustum_brute_force(cam, c32[i], 64.0 / 2.0 ** level[i], n=24) for i in range(300)])
+        assert (phat[meets] > 0).all()
+        # the cases the centre-or-corner rule alone would lose exist in this draw, and the plane test is not "always visible"
+        corner_rule = sampler.inside_frustum(cam, c32)[0]
+        for k in range(8):
+            off = np.array([(k & 1) - 0.5, ((k >> 1) & 1) - 0.5, ((k >> 2) & 1) - 0.5]) * (64.0 / 2.0 ** level)[:, None]
+            corner_rule |= sampler.inside_frustum(cam, c32 + off)[0]
+        assert (meets & ~corner_rule).sum() >= 5
+        assert (phat == 0).sum() >= 30
+        assert ((phat > 0) & ~meets).mean() < 0.15          # conservative, not sloppy: few cubes admitted that the lattice does not reach
+
+
+def test_leaf_level_outside_0_30_is_never_sampled():
+    w = sampler.leaf_weights(np.tile([[0, 0, 5.0]], (4, 1)), np.array([-1, 31, 200, 6]), np.ones(4), 64.0, CAM)
+    assert list(w[:3]) == [0.0, 0.0, 0.0] and w[3] > 0
