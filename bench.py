@@ -400,7 +400,7 @@ def workload_statistics(raster, wl, T, dev) -> dict:
 
 
 # ------------------------------------------------------------------------------------------------
-def next_rows(raster, wl, T, dev, stream, reps: int = 10) -> dict:
+def next_rows(raster, wl, T, dev, stream, reps: int = 10, n_frag: int = 0, peak_gbs: float = 0.0) -> dict:
     """Timings of the NEXT rows of the scope table on the same workload, outside the headline:
     f1 blending weights fused into the backward pass, f2 SH fused into the emission pass, f3 three resolution levels
     and four-cloud multisampling, f4 the view-specific sampler.  CUDA events, 3 warm-ups, mean of `reps`."""
@@ -423,6 +423,12 @@ def next_rows(raster, wl, T, dev, stream, reps: int = 10) -> dict:
         return e0.elapsed_time(e1) / reps
 
     out = {}
+    alg = algorithmic_bytes(N, n_frag, W * H, D)
+
+    def roof(nbytes, t_ms):                       # algorithmic bytes of the row / its time, against the measured HBM peak
+        ach = nbytes / (t_ms * 1e-3) / 1e9
+        return {"algorithmic_bytes": int(nbytes), "achieved_gbs": ach, "frac": (ach / peak_gbs) if peak_gbs else None}
+
     pos, op, feat, g_img, g_alpha, ws = T["pos"], T["op"], T["feat"], T["g_img"], T["g_alpha"], T["ws"]
     raster.inpc_raster_forward(pos, op, feat, cam, out_feat=T["img"], out_alpha=T["alpha"], workspace=ws, flags=FLAGS_STEP)
     bw = torch.empty((N,), dtype=torch.float32, device=dev)
@@ -433,24 +439,29 @@ def next_rows(raster, wl, T, dev, stream, reps: int = 10) -> dict:
     out["f1_blend_weights"] = {"ms_backward": t_plain, "ms_backward_with_weights": t_w, "extra_bytes_per_point": 4}
     if D == 4:
         coeff = torch.randn((N, 36), dtype=torch.float32, device=dev) * 0.5
-        st = {}
-
-        def f_sh():
-            st["o"] = raster.inpc_raster_forward_sh(pos, op, coeff, cam, flags=FLAGS_STEP)
-
-        def b_sh():
-            raster.inpc_raster_backward_sh(pos, op, coeff, cam, g_img, g_alpha, st["o"][2])
-
-        t_f = ms(f_sh)
-        t_b = ms(b_sh)
+        o = raster.inpc_raster_forward_sh(pos, op, coeff, cam, flags=FLAGS_STEP)          # buffers allocated once, here
+        gsh = (torch.empty((N, 36), dtype=torch.float32, device=dev), T["d_op"], T["d_uv"])
+        t_f = ms(lambda: raster.inpc_raster_forward_sh(pos, op, coeff, cam, flags=FLAGS_STEP, out_feat=o[0], out_alpha=o[1],
+                                                       workspace=o[2]))
+        t_b = ms(lambda: raster.inpc_raster_backward_sh(pos, op, coeff, cam, g_img, g_alpha, o[2], grads=gsh))
+        # the row's bytes: the plain pass's, with 144 B of coefficients per point read (forward) / written (backward)
+        # in place of the 16 B of features
         out["f2_fused_sh"] = {"ms_forward": t_f, "ms_backward": t_b, "coefficient_bytes_per_point": 144,
-                              "note": "includes the allocation of outputs / workspace by the binding in every call"}
-        del coeff, st
-    t_l = ms(lambda: raster.inpc_raster_forward_levels(pos, op, feat, cam, 3, flags=FLAGS_FWD))
-    out["f3_three_levels_forward"] = {"ms": t_l, "note": "levels 0, 1, 2 of one cloud, forward only (binding allocates per call)"}
+                              "forward": roof(alg["fwd"] + (144 - 16) * N, t_f),
+                              "backward": roof(alg["bwd"] + (144 - 16) * N, t_b),
+                              "note": "outputs, gradients and workspace pre-allocated (no allocation in the timed loop)"}
+        del coeff, o, gsh
+    lv = raster.inpc_raster_forward_levels(pos, op, feat, cam, 3, flags=FLAGS_FWD)
+    t_l = ms(lambda: raster.inpc_raster_forward_levels(pos, op, feat, cam, 3, flags=FLAGS_FWD, outs=lv[:3]))
+    # three passes over the same cloud: the per-fragment / per-point bytes three times, the per-pixel bytes at 1 + 1/4 + 1/16
+    out["f3_three_levels_forward"] = {"ms": t_l, **roof(3 * alg["fwd"] - (3 - 21 / 16) * (12 + 4 * (D + 1)) * W * H, t_l),
+                                      "note": "levels 0, 1, 2 of one cloud, forward only; buffers pre-allocated"}
+    del lv
     clouds = [(pos, op, feat)] * 4
-    t_m = ms(lambda: raster.inpc_raster_forward_multisample(clouds, cam, n_levels=1, flags=raster.OUT_PLANAR))
-    out["f3_multisample_4_clouds"] = {"ms": t_m, "splats": 16 * N,
+    mo = raster.inpc_raster_forward_multisample(clouds, cam, n_levels=1, flags=raster.OUT_PLANAR)
+    mws = raster.alloc_workspace(N, D, W, H, 0, dev)
+    t_m = ms(lambda: raster.inpc_raster_forward_multisample(clouds, cam, n_levels=1, flags=raster.OUT_PLANAR, outs=mo, workspace=mws))
+    out["f3_multisample_4_clouds"] = {"ms": t_m, "splats": 16 * N, **roof(4 * alg["fwd"], t_m),
                                       "note": "four clouds of N points averaged per pixel, [D,H,W] output (PAPER.md:172: 8M x 4 x 4 = 128 M splats)"}
     centre, level, prob, root = make_octree(1 << 20, seed=21)
     dc, dl, dp = (torch.from_numpy(a).to(dev) for a in (centre, level, prob))
@@ -461,8 +472,14 @@ def next_rows(raster, wl, T, dev, stream, reps: int = 10) -> dict:
         sws["w"] = sws["o"][2]
 
     t_s = ms(f_s)
+    # per leaf: centre, level, probability in (20 B), p^ and the CDF written and read (32 B); per sample: 16 B out
+    # (the ~20 dependent CDF probes per draw hit L2 and are not counted)
     out["f4_sampler"] = {"ms": t_s, "leaves": 1 << 20, "samples": N, "samples_per_sec": N / (t_s * 1e-3),
-                         "valid": raster.inpc_sample_get_stats(sws["w"])["n_valid"]}
+                         "valid": raster.inpc_sample_get_stats(sws["w"])["n_valid"], **roof(52 * (1 << 20) + 16 * N, t_s)}
+    t_s1 = ms(lambda: raster.inpc_sample_view(dc, dl, dp, root, cam, seed=7, N=N, workspace=sws["w"], flags=raster.SAMPLE_NO_RESAMPLE))
+    out["f4_sampler_no_resample"] = {"ms": t_s1, "samples_per_sec": N / (t_s1 * 1e-3),
+                                     "valid": raster.inpc_sample_get_stats(sws["w"])["n_valid"],
+                                     "note": "INPC_SAMPLE_NO_RESAMPLE: one draw per sample (inference, PAPER.md:322)"}
     return out
 
 
@@ -744,7 +761,7 @@ def run_ours(args) -> int:
         "clocks": clock_info,
     }
     if world == 1 and wl.backward and not args.no_next_rows:
-        line["next_rows"] = next_rows(raster, wl, T, dev, stream)
+        line["next_rows"] = next_rows(raster, wl, T, dev, stream, n_frag=n_frag, peak_gbs=peak)
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(wl)
         line["cpu_baseline_all_cores"] = cpu_baseline(wl, openmp=True)

@@ -100,7 +100,9 @@ int inpc_raster_forward(const float* pos, const float* opacity, const float* fea
 /* Backward pass of L = <grad_out_feat, out_feat> + <grad_out_alpha, out_alpha>.
  *   Same pos / opacity / feat / N / D / cam and the workspace as left by a forward that had
  *   INPC_SAVE_FOR_BACKWARD set.  grad_out_alpha may be NULL (= 0).
- *   grad_feat[N][D], grad_opacity[N], grad_uv[N][2] = dL/d(u, v) in pixels; all three required.
+ *   grad_feat[N][D], grad_opacity[N], grad_uv[N][2] = dL/d(u, v) in pixels.  Any of the three may be NULL: that
+ *   gradient is then not written (its stores are skipped; the others are bit-identical to a call that asks for all).
+ *   The same holds for every backward entry point below (grad_sh_coeff included).
  *   Culled points and fragments behind the cut-off get exactly 0. */
 int inpc_raster_backward(const float* pos, const float* opacity, const float* feat, int64_t N, int32_t D,
                          const inpc_camera* cam,
@@ -227,6 +229,15 @@ int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const 
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
 int inpc_sample_get_stats(const void* workspace, uint64_t* n_valid, uint64_t* cdf_total, double* max_weight,
                           void* cuda_stream);
+/* inpc_sample_view with flags.  INPC_SAMPLE_NO_RESAMPLE: the inference mode of PAPER.md:322 ("During inference, we use
+ * multisampled point clouds and can therefore omit resampling, which also boosts performance"): every sample is drawn
+ * ONCE; a position outside the frustum is returned as NaN / leaf -1 and culled by the rasterizer.  The random counters
+ * are those of the first attempt of inpc_sample_view, so a sample whose first draw is inside the frustum is the same
+ * bits in both modes.  flags = 0 is inpc_sample_view. */
+#define INPC_SAMPLE_NO_RESAMPLE 1u
+int inpc_sample_view_ex(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
+                        float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
+                        void* workspace, size_t workspace_bytes, uint32_t flags, void* cuda_stream);
 
 /* ---- The sampler for callers that cannot allocate device memory. ---------------------------------------------
  * inpc_sample_view needs a workspace, and somebody has to cudaMalloc it.  Not every caller can: a plugin inside a

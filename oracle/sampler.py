@@ -119,8 +119,9 @@ def integer_cdf(phat):
     return np.cumsum(w, dtype=np.uint64)
 
 
-def sample_view(centre, level, prob, root_side, cam, seed: int, N: int):
-    """-> pos[N,3] float32 (NaN where all attempts failed), leaf[N] int32 (-1 there)."""
+def sample_view(centre, level, prob, root_side, cam, seed: int, N: int, attempts: int = ATTEMPTS):
+    """-> pos[N,3] float32 (NaN where all attempts failed), leaf[N] int32 (-1 there).
+    attempts = 1 is the inference mode of PAPER.md:322 ("omit resampling"): one draw, outside the frustum -> NaN."""
     centre = np.asarray(centre, dtype=np.float32).reshape(-1, 3)
     level = np.asarray(level, dtype=np.int64)
     cdf = integer_cdf(leaf_weights(centre, level, prob, root_side, cam))
@@ -130,7 +131,7 @@ def sample_view(centre, level, prob, root_side, cam, seed: int, N: int):
     if total == 0:
         return pos, leaf
     todo = np.arange(N, dtype=np.uint64)
-    for a in range(ATTEMPTS):
+    for a in range(attempts):
         if len(todo) == 0:
             break
         c0 = (todo * np.uint64(ATTEMPTS) + np.uint64(a)) * np.uint64(4)

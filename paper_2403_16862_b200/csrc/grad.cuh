@@ -184,19 +184,19 @@ __global__ void __launch_bounds__(256) k_split(const Header* __restrict__ hdr, c
             for (int v = 0; v < D / 4; ++v) f[v] = __ldcs(&in[v]);
             o = __ldcs(&in[D / 4]);
         }
-        if (SH) {
+        if (SH && d_feat) {
             float Y[kShBasis];
             sh_basis9(__ldg(&pos[3 * i]) - view.cx, __ldg(&pos[3 * i + 1]) - view.cy, __ldg(&pos[3 * i + 2]) - view.cz, Y);
 #pragma unroll
             for (int b = 0; b < kShBasis; ++b)
                 __stcs(reinterpret_cast<float4*>(d_feat + (size_t)i * kShCoeffs) + b,
                        make_float4(Y[b] * f[0].x, Y[b] * f[0].y, Y[b] * f[0].z, Y[b] * f[0].w));
-        } else {
+        } else if (d_feat) {
 #pragma unroll
             for (int v = 0; v < D / 4; ++v) __stcs(reinterpret_cast<float4*>(d_feat + (size_t)i * D) + v, f[v]);
         }
-        __stcs(&d_opacity[i], o.x);
-        __stcs(reinterpret_cast<float2*>(d_uv) + i, make_float2(o.y, o.z));
+        if (d_opacity) __stcs(&d_opacity[i], o.x);          // any of the outputs may be NULL: its stores are skipped
+        if (d_uv) __stcs(reinterpret_cast<float2*>(d_uv) + i, make_float2(o.y, o.z));
         if (blend_weight) __stcs(&blend_weight[i], o.w);
     }
 }

@@ -621,7 +621,7 @@ int inpc_raster_backward_sh(const float* pos, const float* opacity, const float*
     int rc = check_common(N, 4, cam);
     if (rc != INPC_OK) return rc;
     if (!grad_out_feat || !workspace) return INPC_ERR_INVALID_ARG;
-    if (N > 0 && (!pos || !grad_sh_coeff || !grad_opacity || !grad_uv)) return INPC_ERR_INVALID_ARG;
+    if (N > 0 && !pos) return INPC_ERR_INVALID_ARG;             // (any of the gradient outputs may be NULL)
     if (flags & ~INPC_OUT_PLANAR) return INPC_ERR_INVALID_ARG;
     if (!aligned16(pos) || !aligned16(grad_out_feat) || !aligned16(grad_out_alpha) || !aligned16(grad_sh_coeff) ||
         !aligned16(grad_opacity) || !aligned16(grad_uv) || !aligned16(blend_weight) ||
@@ -687,7 +687,6 @@ static int backward_entry(int64_t N, int32_t D, const inpc_camera* cam, const fl
     int rc = check_common(N, D, cam);
     if (rc != INPC_OK) return rc;
     if (!grad_out_feat || !workspace) return INPC_ERR_INVALID_ARG;
-    if (N > 0 && (!grad_feat || !grad_opacity || !grad_uv)) return INPC_ERR_INVALID_ARG;
     if (flags & ~INPC_OUT_PLANAR) return INPC_ERR_INVALID_ARG;
     if (!aligned16(grad_out_feat) || !aligned16(grad_out_alpha) || !aligned16(grad_feat) || !aligned16(grad_opacity) ||
         !aligned16(grad_uv) || !aligned16(blend_weight) || (reinterpret_cast<uintptr_t>(workspace) & 255u))
@@ -833,9 +832,10 @@ size_t inpc_sample_workspace_bytes(int64_t n_leaves) {
     return sample_layout(n_leaves).total;
 }
 
-int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
-                     float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
-                     void* workspace, size_t workspace_bytes, void* cuda_stream) {
+static int sample_view_impl(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
+                            float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
+                            void* workspace, size_t workspace_bytes, uint32_t flags, void* cuda_stream) {
+    if (flags & ~INPC_SAMPLE_NO_RESAMPLE) return INPC_ERR_INVALID_ARG;
     if (!cam || !leaf_centre || !leaf_level || !leaf_prob || !workspace || N < 0 || N >= (1ll << 31)) return INPC_ERR_INVALID_ARG;
     if (n_leaves < 1 || n_leaves > (1ll << 24) || !(root_side > 0.f)) return INPC_ERR_INVALID_ARG;
     if (cam->width <= 0 || cam->height <= 0 || !(cam->near_z < cam->far_z)) return INPC_ERR_INVALID_ARG;
@@ -866,10 +866,25 @@ int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const 
     INPC_LAUNCHED("k_cdf_add");
     if (N > 0) {
         k_sample<<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 8), 256, 0, st>>>(
-            cdf, L, head + 1, leaf_centre, leaf_level, root_side, camk, (unsigned long long)seed, (long long)N, pos, leaf, head + 2);
+            cdf, L, head + 1, leaf_centre, leaf_level, root_side, camk, (unsigned long long)seed, (long long)N, pos, leaf, head + 2,
+            (flags & INPC_SAMPLE_NO_RESAMPLE) ? 1 : kSampleAttempts);
         INPC_LAUNCHED("k_sample");
     }
     return INPC_OK;
+}
+
+int inpc_sample_view(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
+                     float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    return sample_view_impl(leaf_centre, leaf_level, leaf_prob, n_leaves, root_side, cam, seed, N, pos, leaf, workspace,
+                            workspace_bytes, 0u, cuda_stream);
+}
+
+int inpc_sample_view_ex(const float* leaf_centre, const int32_t* leaf_level, const float* leaf_prob, int64_t n_leaves,
+                        float root_side, const inpc_camera* cam, uint64_t seed, int64_t N, float* pos, int32_t* leaf,
+                        void* workspace, size_t workspace_bytes, uint32_t flags, void* cuda_stream) {
+    return sample_view_impl(leaf_centre, leaf_level, leaf_prob, n_leaves, root_side, cam, seed, N, pos, leaf, workspace,
+                            workspace_bytes, flags, cuda_stream);
 }
 
 // ---- inpc_sample_view for callers that cannot allocate device memory ------------------------------------------------

@@ -173,13 +173,13 @@ __global__ void __launch_bounds__(256) k_sample(const unsigned long long* __rest
                                                  const float* __restrict__ centre, const int32_t* __restrict__ level,
                                                  float root_side, Camera cam, unsigned long long seed, long long N,
                                                  float* __restrict__ pos, int32_t* __restrict__ leaf_out,
-                                                 unsigned long long* __restrict__ n_valid) {
+                                                 unsigned long long* __restrict__ n_valid, int attempts) {
     const unsigned long long total = *total_p;
     unsigned int ok = 0;
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < N; j += (long long)gridDim.x * blockDim.x) {
         float px = __int_as_float(0x7fc00000), py = px, pz = px;
         int32_t leaf = -1;
-        for (int a = 0; a < kSampleAttempts && total > 0; ++a) {
+        for (int a = 0; a < attempts && total > 0; ++a) {      // attempts = kSampleAttempts, or 1 (INPC_SAMPLE_NO_RESAMPLE); same counters
             const unsigned long long c0 = ((unsigned long long)j * kSampleAttempts + a) * 4ull;
             const unsigned long long r = __umul64hi(splitmix64(seed, c0), total);        // floor(rng * total / 2^64)
             uint32_t lo = 0, hi = L - 1;                                                  // first i with cdf[i] > r

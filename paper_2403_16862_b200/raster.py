@@ -19,6 +19,7 @@ SAVE_SORTED = 2
 OUT_PLANAR = 4          # _ex / _levels / _multisample entry points: feature image as [D][H][W]
 ACCUMULATE = 8          # _ex: add to the image already in the output buffers
 FUSED_SH = 16           # workspace sizing of the _sh entry points
+SAMPLE_NO_RESAMPLE = 1  # inpc_sample_view_ex: one draw per sample (inference mode)
 SH_COEFFS = 36          # M: 9 basis functions x 4 channels, basis-major
 
 EXPORTS = (
@@ -26,7 +27,7 @@ EXPORTS = (
     "inpc_raster_forward_ex", "inpc_raster_backward_ex", "inpc_raster_level_camera", "inpc_raster_forward_levels",
     "inpc_raster_forward_multisample", "inpc_raster_forward_sh", "inpc_raster_backward_sh",
     "inpc_sample_workspace_bytes", "inpc_sample_view", "inpc_sample_get_stats",
-    "inpc_sample_static_max_leaves", "inpc_sample_view_static",
+    "inpc_sample_static_max_leaves", "inpc_sample_view_static", "inpc_sample_view_ex",
     "inpc_raster_get_counts", "inpc_raster_get_blended_counts", "inpc_raster_get_sorted", "inpc_raster_get_stats",
     "inpc_raster_get_status",
     "inpc_raster_strerror", "inpc_raster_last_cuda_error", "inpc_raster_launch_count", "inpc_raster_launched_kernels",
@@ -91,6 +92,8 @@ def load() -> C.CDLL:
         lib.inpc_sample_static_max_leaves.argtypes = []
         lib.inpc_sample_view_static.restype = C.c_int
         lib.inpc_sample_view_static.argtypes = [vp, vp, vp, i64, C.c_float, C.POINTER(InpcCamera), C.c_uint64, i64, vp, vp, vp]
+        lib.inpc_sample_view_ex.restype = C.c_int
+        lib.inpc_sample_view_ex.argtypes = [vp, vp, vp, i64, C.c_float, C.POINTER(InpcCamera), C.c_uint64, i64, vp, vp, vp, C.c_size_t, u32, vp]
         lib.inpc_sample_get_stats.restype = C.c_int
         lib.inpc_sample_get_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_double), vp]
         lib.inpc_raster_level_camera.restype = C.c_int
@@ -185,7 +188,7 @@ def _ptr_array(tensors):
 
 
 def inpc_raster_forward_levels(pos, opacity, feat, cam, n_levels: int, flags: int = SAVE_FOR_BACKWARD, out_scale: float = 1.0,
-                               stream=None):
+                               stream=None, outs=None):
     """One cloud at n_levels resolution levels -> (list of out_feat, list of out_alpha, list of workspaces, list of
     level cameras)."""
     lib = load()
@@ -194,9 +197,12 @@ def inpc_raster_forward_levels(pos, opacity, feat, cam, n_levels: int, flags: in
     cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
     cams = [inpc_raster_level_camera(cs, l) for l in range(n_levels)]
     dev = pos.device
-    imgs = [torch.empty(_img_shape(c.height, c.width, D, flags), dtype=torch.float32, device=dev) for c in cams]
-    alphas = [torch.empty((c.height, c.width), dtype=torch.float32, device=dev) for c in cams]
-    wss = [alloc_workspace(N, D, c.width, c.height, flags & 3, dev) for c in cams]
+    if outs is not None:                        # (imgs, alphas, workspaces) of an earlier call: nothing is allocated
+        imgs, alphas, wss = outs
+    else:
+        imgs = [torch.empty(_img_shape(c.height, c.width, D, flags), dtype=torch.float32, device=dev) for c in cams]
+        alphas = [torch.empty((c.height, c.width), dtype=torch.float32, device=dev) for c in cams]
+        wss = [alloc_workspace(N, D, c.width, c.height, flags & 3, dev) for c in cams]
     sizes = (C.c_size_t * n_levels)(*[w.numel() for w in wss])
     rc = lib.inpc_raster_forward_levels(_ptr(pos), _ptr(opacity), _ptr(feat), N, D, C.byref(cs), n_levels, _ptr_array(imgs),
                                         _ptr_array(alphas), _ptr_array(wss), sizes, flags, out_scale, _stream(stream))
@@ -205,17 +211,20 @@ def inpc_raster_forward_levels(pos, opacity, feat, cam, n_levels: int, flags: in
     return imgs, alphas, wss, cams
 
 
-def inpc_raster_forward_multisample(clouds, cam, n_levels: int = 1, flags: int = 0, stream=None):
+def inpc_raster_forward_multisample(clouds, cam, n_levels: int = 1, flags: int = 0, stream=None, outs=None, workspace=None):
     """clouds: list of (pos, opacity, feat) device tensors.  -> (list of averaged out_feat per level, list of alpha)."""
     lib = load()
     D = int(clouds[0][2].shape[1])
     cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
     cams = [inpc_raster_level_camera(cs, l) for l in range(n_levels)]
     dev = clouds[0][0].device
-    imgs = [torch.empty(_img_shape(c.height, c.width, D, flags), dtype=torch.float32, device=dev) for c in cams]
-    alphas = [torch.empty((c.height, c.width), dtype=torch.float32, device=dev) for c in cams]
+    if outs is not None:
+        imgs, alphas = outs
+    else:
+        imgs = [torch.empty(_img_shape(c.height, c.width, D, flags), dtype=torch.float32, device=dev) for c in cams]
+        alphas = [torch.empty((c.height, c.width), dtype=torch.float32, device=dev) for c in cams]
     Ns = [int(c[0].shape[0]) for c in clouds]
-    ws = alloc_workspace(max(Ns), D, cs.width, cs.height, 0, dev)
+    ws = workspace if workspace is not None else alloc_workspace(max(Ns), D, cs.width, cs.height, 0, dev)
     S = len(clouds)
     rc = lib.inpc_raster_forward_multisample(S, _ptr_array([c[0] for c in clouds]), _ptr_array([c[1] for c in clouds]),
                                              _ptr_array([c[2] for c in clouds]), (C.c_int64 * S)(*Ns), D, C.byref(cs),
@@ -226,8 +235,10 @@ def inpc_raster_forward_multisample(clouds, cam, n_levels: int = 1, flags: int =
     return imgs, alphas
 
 
-def inpc_sample_view(leaf_centre, leaf_level, leaf_prob, root_side: float, cam, seed: int, N: int, workspace=None, stream=None):
-    """View-specific sampling (Eq. 4): -> (pos[N,3] float32, leaf[N] int32, workspace).  No sync."""
+def inpc_sample_view(leaf_centre, leaf_level, leaf_prob, root_side: float, cam, seed: int, N: int, workspace=None, stream=None,
+                     flags: int = 0):
+    """View-specific sampling (Eq. 4): -> (pos[N,3] float32, leaf[N] int32, workspace).  No sync.
+    flags = SAMPLE_NO_RESAMPLE: one draw per sample (inpc_sample_view_ex)."""
     lib = load()
     _check(leaf_centre, torch.float32, "leaf_centre"); _check(leaf_level, torch.int32, "leaf_level")
     _check(leaf_prob, torch.float32, "leaf_prob")
@@ -238,8 +249,13 @@ def inpc_sample_view(leaf_centre, leaf_level, leaf_prob, root_side: float, cam, 
         workspace = torch.empty(int(lib.inpc_sample_workspace_bytes(L)), dtype=torch.uint8, device=dev)
     pos = torch.empty((N, 3), dtype=torch.float32, device=dev)
     leaf = torch.empty((N,), dtype=torch.int32, device=dev)
-    rc = lib.inpc_sample_view(_ptr(leaf_centre), _ptr(leaf_level), _ptr(leaf_prob), L, float(root_side), C.byref(cs),
-                              C.c_uint64(seed), N, _ptr(pos), _ptr(leaf), _ptr(workspace), workspace.numel(), _stream(stream))
+    if flags:
+        rc = lib.inpc_sample_view_ex(_ptr(leaf_centre), _ptr(leaf_level), _ptr(leaf_prob), L, float(root_side), C.byref(cs),
+                                     C.c_uint64(seed), N, _ptr(pos), _ptr(leaf), _ptr(workspace), workspace.numel(), flags,
+                                     _stream(stream))
+    else:
+        rc = lib.inpc_sample_view(_ptr(leaf_centre), _ptr(leaf_level), _ptr(leaf_prob), L, float(root_side), C.byref(cs),
+                                  C.c_uint64(seed), N, _ptr(pos), _ptr(leaf), _ptr(workspace), workspace.numel(), _stream(stream))
     if rc != 0:
         raise InpcError(rc, "inpc_sample_view")
     return pos, leaf, workspace
@@ -285,16 +301,20 @@ def inpc_sample_get_stats(workspace, stream=None) -> dict:
     return {"n_valid": int(nv.value), "cdf_total": int(tot.value), "max_weight": float(mx.value)}
 
 
-def inpc_raster_forward_sh(pos, opacity, sh_coeff, cam, flags: int = SAVE_FOR_BACKWARD, out_scale: float = 1.0, stream=None):
-    """Forward with the SH evaluation fused in: sh_coeff[N,36] instead of feat.  -> (out_feat, out_alpha, workspace)."""
+def inpc_raster_forward_sh(pos, opacity, sh_coeff, cam, flags: int = SAVE_FOR_BACKWARD, out_scale: float = 1.0, stream=None,
+                           out_feat=None, out_alpha=None, workspace=None):
+    """Forward with the SH evaluation fused in: sh_coeff[N,36] instead of feat.  -> (out_feat, out_alpha, workspace);
+    the three are allocated here unless passed in."""
     lib = load()
     _check(pos, torch.float32, "pos"); _check(opacity, torch.float32, "opacity"); _check(sh_coeff, torch.float32, "sh_coeff")
     N = int(pos.shape[0])
     cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
     W, H = cs.width, cs.height
-    ws = alloc_workspace(N, 4, W, H, (flags & 3) | FUSED_SH, pos.device)
-    out_feat = torch.empty(_img_shape(H, W, 4, flags), dtype=torch.float32, device=pos.device)
-    out_alpha = torch.empty((H, W), dtype=torch.float32, device=pos.device)
+    ws = workspace if workspace is not None else alloc_workspace(N, 4, W, H, (flags & 3) | FUSED_SH, pos.device)
+    if out_feat is None:
+        out_feat = torch.empty(_img_shape(H, W, 4, flags), dtype=torch.float32, device=pos.device)
+    if out_alpha is None:
+        out_alpha = torch.empty((H, W), dtype=torch.float32, device=pos.device)
     rc = lib.inpc_raster_forward_sh(_ptr(pos), _ptr(opacity), _ptr(sh_coeff), N, C.byref(cs), _ptr(out_feat), _ptr(out_alpha),
                                     _ptr(ws), ws.numel(), flags, out_scale, _stream(stream))
     if rc != 0:
@@ -312,15 +332,19 @@ def _raise_on_device_status(workspace, stream, where: str):
 
 
 def inpc_raster_backward_sh(pos, opacity, sh_coeff, cam, grad_out_feat, grad_out_alpha, workspace, flags: int = 0,
-                            grad_scale: float = 1.0, blend_weight: bool = False, stream=None, check: bool = False):
+                            grad_scale: float = 1.0, blend_weight: bool = False, stream=None, check: bool = False,
+                            grads=None):
     """-> (grad_sh_coeff[N,36], grad_opacity[N], grad_uv[N,2][, blend_weight[N]]).  check=True: see inpc_raster_backward."""
     lib = load()
     N = int(pos.shape[0])
     cs = cam if isinstance(cam, InpcCamera) else camera_struct(cam)
     dev = pos.device
-    g_c = torch.empty((N, SH_COEFFS), dtype=torch.float32, device=dev)
-    g_o = torch.empty((N,), dtype=torch.float32, device=dev)
-    g_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
+    if grads is not None:                       # (grad_sh_coeff, grad_opacity, grad_uv) of the caller
+        g_c, g_o, g_uv = grads
+    else:
+        g_c = torch.empty((N, SH_COEFFS), dtype=torch.float32, device=dev)
+        g_o = torch.empty((N,), dtype=torch.float32, device=dev)
+        g_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
     bw = torch.empty((N,), dtype=torch.float32, device=dev) if blend_weight else None
     rc = lib.inpc_raster_backward_sh(_ptr(pos), _ptr(opacity), _ptr(sh_coeff), N, C.byref(cs), _ptr(grad_out_feat),
                                      _ptr(grad_out_alpha), _ptr(g_c), _ptr(g_o), _ptr(g_uv), _ptr(bw), _ptr(workspace),
@@ -374,12 +398,16 @@ def inpc_raster_backward(pos, opacity, feat, cam, grad_out_feat, grad_out_alpha,
     if grad_out_alpha is not None:
         _check(grad_out_alpha, torch.float32, "grad_out_alpha")
     dev = pos.device
+    # None = allocate it; False = "not wanted": NULL goes to the library, which skips that gradient's stores
     if grad_feat is None:
         grad_feat = torch.empty((N, D), dtype=torch.float32, device=dev)
     if grad_opacity is None:
         grad_opacity = torch.empty((N,), dtype=torch.float32, device=dev)
     if grad_uv is None:
         grad_uv = torch.empty((N, 2), dtype=torch.float32, device=dev)
+    grad_feat = None if grad_feat is False else grad_feat
+    grad_opacity = None if grad_opacity is False else grad_opacity
+    grad_uv = None if grad_uv is False else grad_uv
     if blend_weight is True:
         blend_weight = torch.empty((N,), dtype=torch.float32, device=dev)
     elif blend_weight is False:

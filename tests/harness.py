@@ -96,18 +96,20 @@ def ambiguous_bound(n_pixels: int) -> int:
     return max(8, int(2 * MARGIN / 0.01 * 0.1 * n_pixels))
 
 
-def oracle_reference(wl, st, ref, report=None):
-    """Blend the oracle, resolve the termination-ambiguous pixels with the GPU's blended counts (run A) and
-    return the reference image / alpha / blended counts every run of this workload is compared with."""
-    W, H = wl.cam.width, wl.cam.height
+def resolve_ambiguous(ref, nb_gpu, W, H, check_bound=True):
+    """THE rule for termination-ambiguous pixels (reading R7), used by every parity test and by smoke():
+    blend the oracle; outside the ambiguous pixels (margin >= MARGIN) the GPU's blended count must equal the oracle's;
+    inside, it must lie between the oracle's counts at the cut-off moved by -+2 MARGIN, and the oracle is re-run with
+    exactly the GPU's count there, so that image, alpha and gradients are compared in every pixel.
+    -> (img_r, alpha_r, nb_r, n_ambiguous); `ref` keeps the forced state for a later ref.backward()."""
     img_r, alpha_r, nb_r, margin = ref.blend()
     amb = margin < MARGIN
-    nb_gpu = raster.inpc_raster_get_blended_counts(st["ws"], W, H).cpu().numpy().view(np.uint32)
     bad = (nb_gpu != nb_r) & ~amb
     assert not bad.any(), (f"blended fragment counts differ in {int(bad.sum())} unambiguous pixels, first "
                            f"{np.argwhere(bad)[:5].tolist()}: gpu {nb_gpu[bad][:5]} oracle {nb_r[bad][:5]}")
     n_amb = int(amb.sum())
-    assert n_amb <= ambiguous_bound(W * H), f"too many termination-ambiguous pixels: {n_amb}"
+    if check_bound:
+        assert n_amb <= ambiguous_bound(W * H), f"too many termination-ambiguous pixels: {n_amb}"
     if n_amb:
         # the GPU's count must be one the cut-off moved by -+2 MARGIN can produce ...
         nb_few = ref.blend(oracle.T_MIN * (1 + 2 * MARGIN))[2]      # higher cut-off: stops earlier
@@ -120,6 +122,15 @@ def oracle_reference(wl, st, ref, report=None):
         force[amb] = nb_gpu[amb]
         img_r, alpha_r, nb_r, _ = ref.blend(force_nb=force)
         assert np.array_equal(nb_r, nb_gpu)
+    return img_r, alpha_r, nb_r, n_amb
+
+
+def oracle_reference(wl, st, ref, report=None):
+    """Blend the oracle, resolve the termination-ambiguous pixels with the GPU's blended counts (run A) and
+    return the reference image / alpha / blended counts every run of this workload is compared with."""
+    W, H = wl.cam.width, wl.cam.height
+    nb_gpu = raster.inpc_raster_get_blended_counts(st["ws"], W, H).cpu().numpy().view(np.uint32)
+    img_r, alpha_r, nb_r, n_amb = resolve_ambiguous(ref, nb_gpu, W, H)
     if report is not None:
         report.update(n_ambiguous=n_amb, n_blended=int(nb_r.sum(dtype=np.int64)))
     return img_r, alpha_r, nb_r

@@ -128,3 +128,14 @@ def test_static_scratch_sampler_limit_is_checked_on_the_host(lib):
     assert lib.inpc_sample_workspace_bytes(mx) == 4195840          # the size the header states for the array
     rc = lib.inpc_sample_view_static(fake, fake, fake, mx + 1, 8.0, C.byref(cam), 1, 16, fake, fake, None)
     assert rc == -6 and b"inpc_sample_static_max_leaves" in lib.inpc_raster_strerror(rc)
+
+
+def test_backward_accepts_null_gradient_outputs_on_the_host(lib):
+    """SURVEY.md:321-322: grad_feat / grad_opacity / grad_uv "or NULL".  With all three NULL the host-side validation
+    still passes (the next failure is the workspace size, checked after the pointers)."""
+    cam = raster.InpcCamera()
+    cam.fx = cam.fy = 64.0; cam.cx = cam.cy = 32.0
+    cam.near_z, cam.far_z, cam.width, cam.height = 0.01, 100.0, 64, 64
+    fake = C.c_void_p(0x1000)
+    assert lib.inpc_raster_backward(fake, fake, fake, 16, 4, C.byref(cam), fake, None, None, None, None, fake, 64, None) == -2
+    assert lib.inpc_raster_backward(fake, fake, fake, 16, 4, C.byref(cam), None, None, None, None, None, fake, 64, None) == -1

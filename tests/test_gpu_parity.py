@@ -207,15 +207,10 @@ def _dev(a):
 
 
 def _reference_with_gpu_counts(ref, ws, W, H):
-    """Oracle image / alpha with the termination-ambiguous pixels resolved as in harness.oracle_reference."""
-    img_r, alpha_r, nb_r, margin = ref.blend()
-    amb = margin < harness.MARGIN
-    if amb.any():
-        nb = raster.inpc_raster_get_blended_counts(ws, W, H).cpu().numpy().view(np.uint32)
-        assert np.array_equal(nb[~amb], nb_r[~amb])
-        force = np.full((H, W), oracle.NO_FORCE, dtype=np.uint32)
-        force[amb] = nb[amb]
-        img_r, alpha_r, _, _ = ref.blend(force_nb=force)
+    """Oracle image / alpha with the termination-ambiguous pixels resolved by harness.resolve_ambiguous (the one rule:
+    counts equal outside the ambiguous pixels, inside them bounded by the cut-off moved by -+2 MARGIN, then forced)."""
+    nb = raster.inpc_raster_get_blended_counts(ws, W, H).cpu().numpy().view(np.uint32)
+    img_r, alpha_r, _, _ = harness.resolve_ambiguous(ref, nb, W, H, check_bound=False)
     return img_r, alpha_r
 
 
@@ -408,6 +403,26 @@ def test_sampler_sees_leaves_the_frustum_only_crosses():
         assert not np.isin(rleaf, [2, 3]).any()
 
 
+def test_sampler_without_resampling_is_bit_exact():
+    """INPC_SAMPLE_NO_RESAMPLE (inference): one draw per sample, against the oracle's attempts = 1."""
+    from oracle import sampler as osampler
+    from paper_2403_16862_b200.workloads import make_octree
+    centre, level, prob, root = make_octree(1 << 14, seed=3)
+    cam = Camera(fx=1100.0, fy=1100.0, cx=648.5, cy=420.0, width=1297, height=840).with_pose(*second_pose())
+    N = 300_001
+    pos, leaf, ws = raster.inpc_sample_view(_dev(centre), _dev(level), _dev(prob), root, cam, seed=77, N=N,
+                                            flags=raster.SAMPLE_NO_RESAMPLE)
+    torch.cuda.synchronize()
+    rpos, rleaf = osampler.sample_view(centre, level, prob, root, cam, seed=77, N=N, attempts=1)
+    assert np.array_equal(leaf.cpu().numpy(), rleaf)
+    assert np.array_equal(pos.cpu().numpy().view(np.uint32)[rleaf >= 0], rpos.view(np.uint32)[rleaf >= 0])
+    assert np.isnan(pos.cpu().numpy()[rleaf < 0]).all() and (rleaf < 0).any()
+    assert raster.inpc_sample_get_stats(ws)["n_valid"] == int((rleaf >= 0).sum())
+    with pytest.raises(raster.InpcError) as e:
+        raster.inpc_sample_view(_dev(centre), _dev(level), _dev(prob), root, cam, seed=77, N=N, flags=2)
+    assert e.value.status == -1
+
+
 def test_sampler_edge_cases():
     from paper_2403_16862_b200.workloads import make_octree
     cam = make_workload("tiny").cam
@@ -518,6 +533,30 @@ def test_results_do_not_depend_on_workspace_contents():
     for other in results[1:]:
         for a, b in zip(results[0], other):
             assert torch.equal(a, b)
+
+
+def test_null_gradient_outputs_are_skipped():
+    """Any of grad_feat / grad_opacity / grad_uv may be NULL: the others come out bit-identical, a buffer that was not
+    passed is not touched, and all-NULL is a valid (if pointless) call."""
+    wl = make_workload("1m", n_points=1 << 17)
+    st = gpu_forward(wl)
+    g_img, g_a = torch.from_numpy(wl.g_img).cuda(), torch.from_numpy(wl.g_alpha).cuda()
+    full = raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g_img, g_a, st["ws"], check=True)
+    for skip in range(3):
+        kw = {("grad_feat", "grad_opacity", "grad_uv")[skip]: False}
+        got = raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g_img, g_a, st["ws"], check=True, **kw)
+        for k in range(3):
+            if k == skip:
+                assert got[k] is None
+            else:
+                assert torch.equal(got[k], full[k])
+    only_uv = raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g_img, g_a, st["ws"], grad_feat=False,
+                                          grad_opacity=False, check=True)
+    assert only_uv[0] is None and only_uv[1] is None and torch.equal(only_uv[2], full[2])
+    none = raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g_img, g_a, st["ws"], grad_feat=False,
+                                       grad_opacity=False, grad_uv=False, blend_weight=True, check=True)
+    bw = raster.inpc_raster_backward(st["pos"], st["op"], st["feat"], wl.cam, g_img, g_a, st["ws"], blend_weight=True)[3]
+    assert none[:3] == (None, None, None) and torch.equal(none[3], bw)
 
 
 def test_error_codes():

@@ -163,3 +163,18 @@ def test_visibility_never_misses_a_leaf_the_frustum_enters():
 def test_leaf_level_outside_0_30_is_never_sampled():
     w = sampler.leaf_weights(np.tile([[0, 0, 5.0]], (4, 1)), np.array([-1, 31, 200, 6]), np.ones(4), 64.0, CAM)
     assert list(w[:3]) == [0.0, 0.0, 0.0] and w[3] > 0
+
+
+def test_no_resample_mode_is_the_first_attempt():
+    """inference omits re-sampling.  attempts = 1 keeps exactly the samples whose first draw was inside the
+    frustum (same bits as the re-sampling mode there) and returns NaN / -1 for the others -- which the re-sampling
+    mode had re-drawn, so it has strictly more valid samples on a tree with leaves across the frustum's faces."""
+    centre, level, prob, root = make_octree(4096, seed=9)
+    N = 50_000
+    p8, l8 = sampler.sample_view(centre, level, prob, root, CAM, seed=5, N=N)
+    p1, l1 = sampler.sample_view(centre, level, prob, root, CAM, seed=5, N=N, attempts=1)
+    ok1 = l1 >= 0
+    assert 0.5 < ok1.mean() < 1.0 and (l8 >= 0).sum() > ok1.sum()
+    assert np.array_equal(l1[ok1], l8[ok1]) and np.array_equal(p1[ok1], p8[ok1])
+    assert np.isnan(p1[~ok1]).all()
+    assert sampler.inside_frustum(CAM, p1[ok1])[0].all()
