@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(kBinThreads) k_project_count(const float* __re
 // on cursor[cell] (a copy of the exclusive cell offsets, so slots of a cell are handed out in arrival order;
 // afterwards cursor[c] == celloff[c + 1]) and write ONE full 32-byte sector per point:
 // { depth_bits, idx, tx, ty | opacity, cell, 0, 0 }.  (Anything narrower than a sector scattered by slot costs a
-// DRAM read-modify-write: profiles/r01_v1_baseline.md.)  All of a thread's atomics and opacity loads are
+// DRAM read-modify-write: DESIGN.md section 10, round-1 facts.)  All of a thread's atomics and opacity loads are
 // issued before the first store.
 // SH (NEXT row f2, sh.cuh): the pass also evaluates every kept point's view-dependent feature from its 36 SH
 // coefficients (read once, here, coalesced) and leaves it in shfeat[point] for the cell sort to pick up.

@@ -8,7 +8,7 @@
 //      a_c = opacity * w_c (Eq. 7) in place, so the merge loop reads ONE float per fragment;
 //   2. the tile's pixels are handed to lanes in descending order of their fragment count (counting sort on
 //      count / 4), so that the 32 pixels of a warp run about equally long
-//      (profiles/r01_v2_cellsort_merge.md: neighbouring pixels gave 10 of 32 lanes active);
+//      (round-1 facts: neighbouring pixels gave 10 of 32 lanes active);
 //   3. ONE THREAD PER PIXEL merges its four lists.  The iteration is branch-free: every list's cursor and
 //      end are packed into one register (byte offset of the fragment's alpha | end << 16), the minimum
 //      head key selects the list with predicates, and only "two heads with equal depth bits" (ascending

@@ -389,7 +389,7 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
       INPC_CUDA(cudaMemsetAsync(ws + L.header, 0, L.zero_end - L.header, st));
       k_write_header<<<1, 1, 0, st>>>(hdr, flags, W, H, D, (uint32_t)N); }
     INPC_LAUNCHED("k_write_header");
-    // grid sizes in CTAs per SM are measured optima (profiles/r01_v3b_sector_stores.md): the passes that scatter
+    // grid sizes in CTAs per SM are measured optima (round-1 facts): the passes that scatter
     // (k_scatter, k_cellsort) are fastest with ONE resident wave of 4 CTAs per SM, the streaming count pass with 8
     const int bin_grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 8);
     const int scatter_grid = (int)std::min<int64_t>((N + kBinChunk - 1) / kBinChunk, (int64_t)di.sms * 4);

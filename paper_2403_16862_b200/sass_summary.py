@@ -1,0 +1,95 @@
+"""Per-kernel SASS / resource summary of the built library (evidence for profiles/, no GPU needed):
+
+    python -m paper_2403_16862_b200.sass_summary > profiles/r03_sass.md
+
+Runs `cuobjdump -res-usage` and `cuobjdump -sass` on libinpc_raster.so and prints, per kernel, registers, static shared
+memory, spills and the counts of the instructions that show how the kernel moves data: UBLKCP (cp.async.bulk, the 1-D
+TMA copies; UTMALDG would be the tensor-map form, which the ragged cell rows do not use), SYNCS (mbarrier), LDS / STS
+(shared memory), LDG / STG (global), ATOM / ATOMG / RED (atomics and fire-and-forget reductions), BAR (CTA barriers).
+"""
+from __future__ import annotations
+
+import collections
+import re
+import subprocess
+import sys
+
+from . import build as _build
+
+PATTERNS = [("UBLKCP", r"\bUBLKCP"), ("UTMALDG", r"\bUTMALDG"), ("SYNCS", r"\bSYNCS"), ("LDS", r"\bLDS"), ("STS", r"\bSTS"),
+            ("LDG", r"\bLDG"), ("STG", r"\bSTG"), ("ATOM", r"\bATOM[GS]?\b|\bATOM\."), ("RED", r"\bRED\b|\bRED\."),
+            ("BAR", r"\bBAR\."), ("SHFL", r"\bSHFL"), ("FFMA", r"\bFFMA"), ("total", r"^\s+/\*[0-9a-f]{4}\*/")]
+
+
+def _demangle(names):
+    try:
+        out = subprocess.run(["cu++filt"] + names, capture_output=True, text=True, check=True).stdout.splitlines()
+        return dict(zip(names, out))
+    except Exception:
+        return {n: n for n in names}
+
+
+def _short(d: str) -> str:
+    d = re.sub(r"^void\s+", "", d).replace("inpc::", "")
+    d = re.sub(r"\((?:int|bool|unsigned int)\)", "", d)          # k_back<(int)4>(BackArgs) -> k_back<4>
+    return re.sub(r"\(.*$", "", d)
+
+
+def main() -> int:
+    lib = _build.build()
+    res = subprocess.run(["cuobjdump", "-res-usage", lib], capture_output=True, text=True, check=True).stdout
+    usage = {}
+    for m in re.finditer(r"Function (\S+):\n\s+(.*)", res):
+        usage[m.group(1)] = dict(kv.split(":") for kv in m.group(2).split() if ":" in kv)
+    sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
+    counts = collections.OrderedDict()
+    cur = None
+    for line in sass.splitlines():
+        m = re.match(r"\s+Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            counts[cur] = collections.Counter()
+            continue
+        if cur is None:
+            continue
+        for key, pat in PATTERNS:
+            if re.search(pat, line):
+                counts[cur][key] += 1
+    arch = re.search(r"arch = (\S+)", res)
+    names = _demangle(list(counts))
+    cols = [k for k, _ in PATTERNS]
+    print("# SASS / resource summary of libinpc_raster.so\n")
+    print("Command (committed files only): `python -m paper_2403_16862_b200.sass_summary > profiles/r03_sass.md`")
+    print(f"(`cuobjdump -res-usage` + `cuobjdump -sass`, counted per kernel; arch = {arch.group(1) if arch else '?'}; "
+          f"{len(counts)} kernels; kernel sources hash {_source_hash()}).\n")
+    print("| kernel | regs | static smem B | spill st/ld B | " + " | ".join(cols) + " |")
+    print("|---|---|---|---|" + "---|" * len(cols))
+    tot = collections.Counter()
+    for fn, c in sorted(counts.items(), key=lambda kv: _short(names[kv[0]])):
+        u = usage.get(fn, {})
+        print(f"| `{_short(names[fn])}` | {u.get('REG', '?')} | {u.get('SHARED', '?')} | "
+              f"{u.get('STACK', '0')} stack | " + " | ".join(str(c[k]) for k in cols) + " |")
+        tot.update(c)
+    print("| **all kernels** | | | | " + " | ".join(str(tot[k]) for k in cols) + " |")
+    print("\nReading: the staging kernels (`k_blend`, `k_back`) move their tiles with `UBLKCP` (1-D `cp.async.bulk`, global -> "
+          "shared on an mbarrier = `SYNCS`; `k_blend<.,1,.>` also shared -> global for the saved order); there is no `UTMALDG` "
+          "because the copies are ragged 1-D ranges without a tensor map.  STACK = bytes of local memory per thread "
+          "(0 = no spills).")
+    return 0
+
+
+def _source_hash() -> str:
+    """The hash bench.py prints as kernel_source_hash: sha256 over csrc/* and include/*.h."""
+    import hashlib
+    import os
+    h = hashlib.sha256()
+    for d in (_build.CSRC, os.path.join(_build.HERE, "..", "include")):
+        for fn in sorted(os.listdir(d)):
+            if fn.endswith((".cu", ".cuh", ".h")):
+                h.update(fn.encode())
+                h.update(open(os.path.join(d, fn), "rb").read())
+    return h.hexdigest()[:16]
+
+
+if __name__ == "__main__":
+    sys.exit(main())

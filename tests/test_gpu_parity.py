@@ -559,6 +559,49 @@ def test_null_gradient_outputs_are_skipped():
     assert none[:3] == (None, None, None) and torch.equal(none[3], bw)
 
 
+def test_two_host_threads_on_two_streams():
+    """The library keeps one side stream per device and a process-wide mutex around the enqueue of calls that use it
+    (deviations).  Two host threads that rasterise different clouds on their own streams at the
+    same time must neither deadlock nor disturb each other: every result equals the one the same call gives alone."""
+    import threading
+    wls = [make_workload("1m", n_points=1 << 17), make_workload("train", n_points=1 << 17)]
+    alone = []
+    for wl in wls:
+        st = gpu_forward(wl, flags=raster.SAVE_FOR_BACKWARD)
+        g = gpu_backward(wl, st)
+        alone.append((st["img"].clone(), st["alpha"].clone(), [x.clone() for x in g]))
+    errors, results = [], [None, None]
+
+    def work(k):
+        try:
+            wl = wls[k]
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                pos, op, feat = _dev(wl.pos), _dev(wl.opacity), _dev(wl.feat)
+                g_img, g_a = _dev(wl.g_img), _dev(wl.g_alpha)
+                for _ in range(20):
+                    img, alpha, ws = raster.inpc_raster_forward(pos, op, feat, wl.cam, flags=raster.SAVE_FOR_BACKWARD, stream=stream)
+                    grads = raster.inpc_raster_backward(pos, op, feat, wl.cam, g_img, g_a, ws, stream=stream)
+                stream.synchronize()
+                assert raster.inpc_raster_get_status(ws, stream=stream) == 0
+                results[k] = (img, alpha, grads)
+        except Exception as e:                                   # noqa: BLE001 -- reported by the main thread
+            errors.append(e)
+
+    threads = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=120)
+        assert not t.is_alive(), "a rasterising thread did not finish: deadlock on the side stream?"
+    assert not errors, errors
+    for k in range(2):
+        img, alpha, grads = results[k]
+        assert torch.equal(img, alone[k][0]) and torch.equal(alpha, alone[k][1])
+        for a, b in zip(grads, alone[k][2]):
+            assert torch.equal(a, b)
+
+
 def test_error_codes():
     wl = make_workload("tiny")
     st = gpu_forward(wl, flags=0)
