@@ -4,8 +4,8 @@
 // Forward  = memset | k_write_header | k_project_count | k_scan_u32 | k_scatter | k_classify | k_cellsort |
 //            k_cellsort_big x2 | [k_scan_u32 (dump)] | k_build_items | k_blend | k_big<fwd>
 // Backward = k_check_backward | k_big<bwd> | k_back | memset(queue) | k_combine | k_split
-// All ordered on the caller's stream (k_classify / k_build_items run on a library-owned side stream that is forked from
-// and joined back into it with events), no host synchronisation.  No device memory is allocated here, no state is kept
+// All ordered on the caller's stream (in the forward pass k_classify / k_build_items run on a library-owned side stream that
+// is forked from and joined back into it with events; the backward pass is one chain), no host synchronisation.  No device memory is allocated here, no state is kept
 // on the host between calls (what a later call needs to know about a workspace is read from the Header the
 // forward pass wrote into it), and there is no CPU fallback.
 #include "../../include/inpc_raster.h"
@@ -466,11 +466,14 @@ static int forward_impl(const float* pos, const float* opacity, const float* fea
             INPC_LAUNCHED(kname<D>("k_cellsort"));
             u0 = u1;
         }
-        INPC_CUDA(fork(st, s2));                                              // band b is sorted: blend it
+        // (Measured in round 3: with one band, launching the blend on the caller's stream instead of hopping to the side
+        // stream and back is no faster -- train 1.370 -> 1.380 ms -- so the hop stays.)
+        cudaStream_t sb = s2;
+        INPC_CUDA(fork(st, sb));                                              // band b is sorted: blend it
         A.items = items + B.plan.item_base[b]; A.n_items = &hdr->band_items[b]; A.item_cursor = &hdr->band_cursor[b];
         if (save) A.ordinfo = reinterpret_cast<uint2*>(ws + L.ordinfo) + B.plan.item_base[b];
-        int rc = dump ? (save ? launch_blend<D, true, true>(A, di, s2) : launch_blend<D, false, true>(A, di, s2))
-                      : (save ? launch_blend<D, true, false>(A, di, s2) : launch_blend<D, false, false>(A, di, s2));
+        int rc = dump ? (save ? launch_blend<D, true, true>(A, di, sb) : launch_blend<D, false, true>(A, di, sb))
+                      : (save ? launch_blend<D, true, false>(A, di, sb) : launch_blend<D, false, false>(A, di, sb));
         if (rc != INPC_OK) return rc;
     }
     INPC_CUDA(fork(s2, st));                                                  // join
@@ -493,10 +496,7 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
       k_check_backward<<<1, 1, 0, st>>>(hdr, W, H, D, (uint32_t)N); }
     INPC_LAUNCHED("k_check_backward");
     if (N == 0) return INPC_OK;
-    std::unique_lock<std::mutex> side_lock(g_side_mu, std::defer_lock);
-    Side* side = nullptr;
-    if (!g_timing) { side_lock.lock(); side = side_for(di); if (!side) return cuda_fail(cudaGetLastError()); }
-    cudaStream_t s2 = side ? side->stream : st;
+    // (the backward pass is one chain of kernels on the caller's stream: it does not use the library's side stream)
     const uint32_t* celloff = reinterpret_cast<uint32_t*>(ws + L.cellcnt);
     const float4* Ra = reinterpret_cast<float4*>(ws + L.Ra);
     const float4* Rf = reinterpret_cast<float4*>(ws + L.Rf);
@@ -505,13 +505,6 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
     uint4* pcur = reinterpret_cast<uint4*>(ws + L.pcur);
     float* gpt = reinterpret_cast<float*>(ws + L.gpt);
     uint32_t* items = reinterpret_cast<uint32_t*>(ws + L.items);
-    int ev = 0;
-    auto fork = [&](cudaStream_t from, cudaStream_t to) -> cudaError_t {
-        if (from == to) return cudaSuccess;
-        cudaEvent_t e = side->ev[ev++ % kSideEvents];
-        cudaError_t rc = cudaEventRecord(e, from);
-        return rc != cudaSuccess ? rc : cudaStreamWaitEvent(to, e, 0);
-    };
     // long-run pixels first: they need nothing but the forward state, and every combine below may touch their cells
     BigArgs Bg{};
     Bg.hdr = hdr; Bg.bigpix = reinterpret_cast<uint32_t*>(ws + L.bigpix); Bg.celloff = celloff;
@@ -538,7 +531,6 @@ static int backward_impl(int64_t N, const inpc_camera* cam, const float* g_feat,
           hdr, celloff, L.C, 0u, n_units, W, H, Ra, reinterpret_cast<const float4*>(gT),
           reinterpret_cast<const float4*>(gD), pcur, g_feat, io, gpt, reinterpret_cast<unsigned long long*>(ws + L.bigkeys)); }
     INPC_LAUNCHED(kname<D>("k_combine"));
-    INPC_CUDA(fork(s2, st));                                                  // join
     { StageTimer tm(kStSplit, st);
       const int grid = (int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 16);
       const uint32_t* kept = reinterpret_cast<const uint32_t*>(ws + L.kept);
