@@ -308,17 +308,17 @@ def source_hash() -> str:
     return h.hexdigest()[:16]
 
 
-TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")      # raw `ncu --csv` output, see r02_traffic.md
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r03_traffic.csv")      # raw `ncu --csv` output, see r03_traffic.md
 
 
 def ncu_traffic(workload: str) -> dict:
-    """{stage name: mean dram read+write bytes per launch} from profiles/r02_traffic.csv, or {} (with the reason)
-    when the capture is for other kernel sources or another workload (profiles/r02_traffic.md records both)."""
+    """{stage name: mean dram read+write bytes per launch} from profiles/r03_traffic.csv, or {} (with the reason)
+    when the capture is for other kernel sources or another workload (profiles/r03_traffic.md records both)."""
     import csv
     import re
     md = TRAFFIC_CSV[:-4] + ".md"
     if not (os.path.exists(TRAFFIC_CSV) and os.path.exists(md)):
-        return {"_note": "no committed capture (profiles/r02_traffic.csv)"}
+        return {"_note": "no committed capture (profiles/r03_traffic.csv)"}
     text = open(md).read()
     m_hash = re.search(r"source_hash:\s*`?([0-9a-f]{16})", text)
     m_wl = re.search(r"workload:\s*`?(\w+)", text)
@@ -339,7 +339,7 @@ def ncu_traffic(workload: str) -> dict:
         if r[im].startswith("dram__bytes_read"):
             cnt[name] = cnt.get(name, 0) + 1
     out = {k: acc[k] / max(cnt.get(k, 1), 1) for k in acc}
-    out["_note"] = f"profiles/r02_traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean per launch; sources {source_hash()})"
+    out["_note"] = f"profiles/r03_traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean per launch; sources {source_hash()})"
     return out
 
 
