@@ -473,7 +473,7 @@ def next_rows(raster, wl, T, dev, stream, reps: int = 10, n_frag: int = 0, peak_
 
     t_s = ms(f_s)
     # per leaf: centre, level, probability in (20 B), p^ and the CDF written and read (32 B); per sample: 16 B out
-    # (the ~20 dependent CDF probes per draw hit L2 and are not counted)
+    # (the CDF probes of a draw -- guide table, then ~4 of them -- hit L2 and are not counted)
     out["f4_sampler"] = {"ms": t_s, "leaves": 1 << 20, "samples": N, "samples_per_sec": N / (t_s * 1e-3),
                          "valid": raster.inpc_sample_get_stats(sws["w"])["n_valid"], **roof(52 * (1 << 20) + 16 * N, t_s)}
     t_s1 = ms(lambda: raster.inpc_sample_view(dc, dl, dp, root, cam, seed=7, N=N, workspace=sws["w"], flags=raster.SAMPLE_NO_RESAMPLE))

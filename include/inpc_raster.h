@@ -247,7 +247,7 @@ int inpc_sample_view_ex(const float* leaf_centre, const int32_t* leaf_level, con
  * library image, so the call itself and everything under it allocates and frees nothing.
  *   Limit:  n_leaves <= inpc_sample_static_max_leaves() = 262,144 (2^18).  More returns INPC_ERR_STATIC_LIMIT
  *           and enqueues nothing; use inpc_sample_view with a workspace of your own then.
- *   Cost:   the array is 4,195,840 bytes (16 per leaf + 1.5 KB) of every GPU that loads this library, from module
+ *   Cost:   the array is 4,458,240 bytes (16 per leaf + 258 KB) of every GPU that loads this library, from module
  *           load to process exit, used or not.
  *   Set-up: the first call on each device looks up that device's address of the array (cudaGetSymbolAddress, with
  *           that device current; no allocation, but it may make the runtime load the module).  Make that first

@@ -806,7 +806,7 @@ int inpc_raster_get_sorted(const void* workspace, int32_t W, int32_t H, uint32_t
 }
 
 // ---- NEXT row f4: view-specific sampling (sampler.cuh) ---------------------------------------------------------------
-struct SampleLayout { size_t head, phat, cdf, tiles, total; uint32_t n_tiles; };
+struct SampleLayout { size_t head, phat, cdf, tiles, guide, total; uint32_t n_tiles; };
 static SampleLayout sample_layout(int64_t L) {
     SampleLayout S{};
     S.n_tiles = (uint32_t)((L + kScan64Tile - 1) / kScan64Tile);
@@ -815,6 +815,7 @@ static SampleLayout sample_layout(int64_t L) {
     S.phat = o;  o = align_up(o + (size_t)L * 8);
     S.cdf = o;   o = align_up(o + (size_t)L * 8);
     S.tiles = o; o = align_up(o + ((size_t)S.n_tiles + 1) * 8);
+    S.guide = o; o = align_up(o + ((size_t)kGuide + 1) * 4);   // guide table of the inverse CDF (sampler.cuh)
     S.total = o;
     return S;
 }
@@ -844,6 +845,7 @@ static int sample_view_impl(const float* leaf_centre, const int32_t* leaf_level,
     double* phat = reinterpret_cast<double*>(ws + S.phat);
     unsigned long long* cdf = reinterpret_cast<unsigned long long*>(ws + S.cdf);
     unsigned long long* tiles = reinterpret_cast<unsigned long long*>(ws + S.tiles);
+    uint32_t* guide = reinterpret_cast<uint32_t*>(ws + S.guide);
     const Camera camk = to_camera(cam);
     const uint32_t L = (uint32_t)n_leaves;
     INPC_CUDA(cudaMemsetAsync(head, 0, 64, st));
@@ -857,9 +859,11 @@ static int sample_view_impl(const float* leaf_centre, const int32_t* leaf_level,
     k_cdf_add<<<S.n_tiles, kScan64Threads, 0, st>>>(cdf, L, tiles);
     INPC_LAUNCHED("k_cdf_add");
     if (N > 0) {
+        k_cdf_guide<<<kGuide / 256 + 1, 256, 0, st>>>(cdf, L, head + 1, guide);
+        INPC_LAUNCHED("k_cdf_guide");
         k_sample<<<(int)std::min<int64_t>((N + 255) / 256, (int64_t)di.sms * 8), 256, 0, st>>>(
             cdf, L, head + 1, leaf_centre, leaf_level, root_side, camk, (unsigned long long)seed, (long long)N, pos, leaf, head + 2,
-            (flags & INPC_SAMPLE_NO_RESAMPLE) ? 1 : kSampleAttempts);
+            (flags & INPC_SAMPLE_NO_RESAMPLE) ? 1 : kSampleAttempts, guide);
         INPC_LAUNCHED("k_sample");
     }
     return INPC_OK;
@@ -883,16 +887,17 @@ int inpc_sample_view_ex(const float* leaf_centre, const int32_t* leaf_level, con
 // Some users of the sampler have no way to obtain a workspace: a renderer plugin running inside a host application
 // that has handed the whole GPU to its own memory pool, a real-time loop in which cudaMalloc's implicit device-wide
 // synchronisation is forbidden, code that runs after the process has hit its memory budget.  For them the sampler's
-// scratch (p^, the integer CDF, the tile sums and the three statistics words: 16 bytes per leaf plus 1.5 KB) is carved
-// out of the library image itself: the array below is part of the module, so every device that loads the library pays
-// its 4 MiB from the moment the module is loaded until the process exits, whether or not this entry point is ever used.
+// scratch (p^, the integer CDF, the tile sums, the guide table and the three statistics words: 16 bytes per leaf plus
+// 258 KB) is carved out of the library image itself: the array below is part of the module, so every device that loads
+// the library pays its 4.25 MiB from the moment the module is loaded until the process exits, whether or not this entry point is ever used.
 //
 // g_sample_scratch is a DEVICE symbol.  The name, used in host code, is only the host-side shadow the runtime keeps
 // for it -- not an address a kernel may dereference -- so the device address is looked up per device with
 // cudaGetSymbolAddress (each device has its own copy of the array) and it is that address the kernels are given.
 constexpr int64_t kStaticSampleMaxLeaves = 1ll << 18;
 constexpr size_t kStaticSampleBytes =       // sample_layout(kStaticSampleMaxLeaves).total, spelled out so that it is a constant
-    256 + 2 * (size_t)kStaticSampleMaxLeaves * 8 + ((kStaticSampleMaxLeaves / kScan64Tile + 1) * 8 + 255) / 256 * 256;
+    256 + 2 * (size_t)kStaticSampleMaxLeaves * 8 + ((kStaticSampleMaxLeaves / kScan64Tile + 1) * 8 + 255) / 256 * 256 +
+    (((size_t)kGuide + 1) * 4 + 255) / 256 * 256;
 static __device__ __align__(256) unsigned char g_sample_scratch[kStaticSampleBytes];
 
 static void* static_sample_scratch(const DeviceInfo& di, cudaError_t* err) {

@@ -167,13 +167,38 @@ __global__ void __launch_bounds__(kScan64Threads) k_cdf_add(unsigned long long* 
     for (uint32_t q = threadIdx.x; q < kScan64Tile; q += kScan64Threads) if (base + q < L) cdf[base + q] += off;
 }
 
-// one thread per sample: draw a leaf (inverse CDF by binary search), jitter inside it, re-draw while outside the frustum
+// Guide table of the inverse CDF: the top kGuideBits bits b of the 64-bit random number confine the draw
+// r = floor(rng * total / 2^64) to [lo_b, lo_{b+1}] with lo_b = floor((b << (64 - kGuideBits)) * total / 2^64) (mulhi is
+// monotone in rng), so the drawn leaf -- the first i with cdf[i] > r -- lies in [guide[b], guide[b + 1]] where
+// guide[b] = first i with cdf[i] > lo_b and guide[2^kGuideBits] = L - 1.  The search inside that range finds the SAME
+// leaf as a search over the whole CDF (it is the unique first i with cdf[i] > r), in ~4 probes instead of 20 for 2^20 leaves.
+constexpr int kGuideBits = 16;
+constexpr uint32_t kGuide = 1u << kGuideBits;
+
+__global__ void __launch_bounds__(256) k_cdf_guide(const unsigned long long* __restrict__ cdf, uint32_t L,
+                                                    const unsigned long long* __restrict__ total_p,
+                                                    uint32_t* __restrict__ guide) {
+    const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b > kGuide) return;
+    const unsigned long long total = *total_p;
+    uint32_t lo = 0, hi = L - 1;
+    if (b < kGuide && total > 0) {
+        const unsigned long long r = __umul64hi((unsigned long long)b << (64 - kGuideBits), total);   // < total
+        while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (__ldg(&cdf[mid]) > r) hi = mid; else lo = mid + 1; }
+    } else {
+        lo = L - 1;
+    }
+    guide[b] = lo;
+}
+
+// one thread per sample: draw a leaf (inverse CDF: guide table, then binary search), jitter inside it, re-draw while outside the frustum
 __global__ void __launch_bounds__(256) k_sample(const unsigned long long* __restrict__ cdf, uint32_t L,
                                                  const unsigned long long* __restrict__ total_p,
                                                  const float* __restrict__ centre, const int32_t* __restrict__ level,
                                                  float root_side, Camera cam, unsigned long long seed, long long N,
                                                  float* __restrict__ pos, int32_t* __restrict__ leaf_out,
-                                                 unsigned long long* __restrict__ n_valid, int attempts) {
+                                                 unsigned long long* __restrict__ n_valid, int attempts,
+                                                 const uint32_t* __restrict__ guide) {
     const unsigned long long total = *total_p;
     unsigned int ok = 0;
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < N; j += (long long)gridDim.x * blockDim.x) {
@@ -181,8 +206,10 @@ __global__ void __launch_bounds__(256) k_sample(const unsigned long long* __rest
         int32_t leaf = -1;
         for (int a = 0; a < attempts && total > 0; ++a) {      // attempts = kSampleAttempts, or 1 (INPC_SAMPLE_NO_RESAMPLE); same counters
             const unsigned long long c0 = ((unsigned long long)j * kSampleAttempts + a) * 4ull;
-            const unsigned long long r = __umul64hi(splitmix64(seed, c0), total);        // floor(rng * total / 2^64)
-            uint32_t lo = 0, hi = L - 1;                                                  // first i with cdf[i] > r
+            const unsigned long long rng0 = splitmix64(seed, c0);
+            const unsigned long long r = __umul64hi(rng0, total);                         // floor(rng * total / 2^64)
+            const uint32_t gb = (uint32_t)(rng0 >> (64 - kGuideBits));
+            uint32_t lo = __ldg(&guide[gb]), hi = __ldg(&guide[gb + 1]);                  // first i with cdf[i] > r lies in [lo, hi]
             while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (__ldg(&cdf[mid]) > r) hi = mid; else lo = mid + 1; }
             const int l = level[lo];
             const float side = __fmul_rn(root_side, __int_as_float((127 - l) << 23));

@@ -268,7 +268,7 @@ def inpc_sample_static_max_leaves() -> int:
 def inpc_sample_view_static(leaf_centre, leaf_level, leaf_prob, root_side: float, cam, seed: int, N: int, pos=None, leaf=None,
                             stream=None):
     """inpc_sample_view without a workspace, for callers that cannot allocate device memory (a plugin under a host
-    application's memory pool, a frame loop that may not touch cudaMalloc): the scratch is a fixed 4 MiB array inside
+    application's memory pool, a frame loop that may not touch cudaMalloc): the scratch is a fixed 4.25 MiB array inside
     the library, good for up to inpc_sample_static_max_leaves() = 2^18 leaves (InpcError -6 beyond that).  Pass
     pre-allocated pos[N,3] float32 / leaf[N] int32 and the call allocates nothing at all; without them this wrapper
     makes the two output tensors (the C entry point never does).  All calls on a device share the one array: keep them

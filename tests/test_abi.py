@@ -125,7 +125,7 @@ def test_static_scratch_sampler_limit_is_checked_on_the_host(lib):
     fake = C.c_void_p(0x1000)
     mx = lib.inpc_sample_static_max_leaves()
     assert mx == 1 << 18
-    assert lib.inpc_sample_workspace_bytes(mx) == 4195840          # the size the header states for the array
+    assert lib.inpc_sample_workspace_bytes(mx) == 4458240          # the size the header states for the array
     rc = lib.inpc_sample_view_static(fake, fake, fake, mx + 1, 8.0, C.byref(cam), 1, 16, fake, fake, None)
     assert rc == -6 and b"inpc_sample_static_max_leaves" in lib.inpc_raster_strerror(rc)
 

@@ -3,7 +3,7 @@
 Who that is: code that lives inside somebody else's process and memory pool (a renderer plugin, an engine whose
 allocator has taken the whole GPU at start-up), or a frame loop in which cudaMalloc's device-wide synchronisation is
 not acceptable.  Such a caller cannot provide the workspace inpc_sample_view asks for, so this entry point keeps its
-scratch in a fixed 4 MiB array inside the library (at most 2^18 leaves) and allocates nothing.
+scratch in a fixed 4.25 MiB array inside the library (at most 2^18 leaves) and allocates nothing.
 
 What is checked: the drawn leaves and positions are the SAME BITS as inpc_sample_view's (the sampler's parity bar in
 test_gpu_parity.py is bit-exactness; inpc_sample_view itself is compared with the oracle there), on two calls in a
