@@ -139,3 +139,28 @@ def test_backward_accepts_null_gradient_outputs_on_the_host(lib):
     fake = C.c_void_p(0x1000)
     assert lib.inpc_raster_backward(fake, fake, fake, 16, 4, C.byref(cam), fake, None, None, None, None, fake, 64, None) == -2
     assert lib.inpc_raster_backward(fake, fake, fake, 16, 4, C.byref(cam), None, None, None, None, None, fake, 64, None) == -1
+
+
+def test_staging_kernels_use_bulk_copies_and_nothing_spills(lib):
+    """The built library's SASS, per kernel (python -m paper_2403_16862_b200.sass_summary, the table of
+    profiles/r03_sass.md): the tile kernels stage with cp.async.bulk on an mbarrier (UBLKCP + SYNCS), the saving forward
+    also stores the order lists with one, and no hot kernel spills registers to local memory."""
+    import contextlib
+    import io
+    from paper_2403_16862_b200 import sass_summary
+    buf = io.StringIO()
+    with contextlib.redirect_stdout(buf):
+        assert sass_summary.main() == 0
+    rows = {}
+    for line in buf.getvalue().splitlines():
+        if line.startswith("| `"):
+            c = [x.strip() for x in line.strip("|").split("|")]
+            rows[c[0].strip("`")] = c
+    head = [x.strip() for x in next(l for l in buf.getvalue().splitlines() if l.startswith("| kernel")).strip("|").split("|")]
+    col = {n: i for i, n in enumerate(head)}
+    for k in ("k_blend<4, 1, 0>", "k_blend<4, 0, 0>", "k_blend<8, 0, 0>", "k_back<4>", "k_back<8>"):
+        assert int(rows[k][col["UBLKCP"]]) >= 3 and int(rows[k][col["SYNCS"]]) >= 3, k
+    assert int(rows["k_blend<4, 1, 0>"][col["UBLKCP"]]) > int(rows["k_blend<4, 0, 0>"][col["UBLKCP"]])   # + the bulk store
+    for k in ("k_blend<4, 1, 0>", "k_blend<4, 0, 0>", "k_back<4>", "k_combine<4>", "k_cellsort<4>", "k_scatter<0>", "k_project_count"):
+        assert rows[k][col["spill st/ld B"]].startswith("0 "), f"{k} spills"
+    assert int(rows["k_project_count"][col["RED"]]) >= 1                   # fire-and-forget reductions in the count pass
